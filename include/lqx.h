@@ -1,0 +1,191 @@
+/* ==============================================================================================
+ * lqx -- site-parallel evaluation of QDP++-style lattice field expressions on one B200 (sm_100a).
+ *
+ * C-ABI boundary of the hot path of arXiv 1105.2279 (F. Winter, "Accelerating QDP++ using GPUs").
+ * The paper's method evaluates an expression over lattice-wide objects by running the whole
+ * expression once per site, with no temporaries (PAPER.md:61-63 sec.3, :115 sec.5.4), including
+ * the nearest-neighbour `shift` operator that reads its operand through a periodic site table
+ * (sec.5.2).  This library is that evaluation for a fixed catalogue of
+ * expressions (BASELINE.json north_star / configs; SURVEY.md sec.8(a),(b)): every call below is
+ * ONE fused CUDA kernel pass (plus a tiny deterministic second stage for reductions).
+ *
+ * Conventions (all calls)
+ *   * return 0 (LQX_OK) on success, a negative lqx_status otherwise; nothing is printed, nothing
+ *     aborts, no exception crosses the boundary.  lqx_last_error(ctx) holds a detail string.
+ *   * `host` pointers are caller-owned host memory, touched only during the call.
+ *     `dev`  pointers are device memory on the context's device.
+ *   * External ("QDP++ order", reading A7) layout of a host field:
+ *     site-major array of structs, sites lexicographic with x0 fastest,
+ *     site(x) = x0 + L0*(x1 + L1*(x2 + L2*x3)); inside a site, outer->inner:
+ *     [spin][colour row][colour column][re,im]; real index of a colour matrix element
+ *     ((s*3+i)*3+j)*2+c, fermion ((s*4+a)*3+i)*2+c, colour vector (s*3+i)*2+c, complex s*2+c.
+ *   * Internal device layout: site-fastest structure of arrays, one plane per real component,
+ *     plane index = (QDP-order real index inside the site), plane stride = lqx_plane_stride()
+ *     elements (V rounded up to 32).  Element (component r, site s) lives at r*stride + s.
+ *   * shift(f, LQX_FORWARD, mu)(x) = f(x + mu^), shift(f, LQX_BACKWARD, mu)(x) = f(x - mu^)
+ *     (fixed by Listing 1 line 25 against Eq. 2), periodic in every
+ *     direction.
+ *   * Evaluation calls are asynchronous on the context's stream.  pop, the reductions and the
+ *     *_host calls synchronise that stream.  A context is used from one host thread at a time.
+ *   * All operands of a call must belong to the same context and have the same precision
+ *     (QDP++ fixes the precision per build): otherwise LQX_ETYPE / LQX_EGEOM.
+ *   * Site-local forms may alias destination and operands; anything that reads an operand
+ *     through a shift must be out of place (LQX_EALIAS).
+ *   * Real scalars arrive as double and are rounded once to the field precision (reading A10).
+ * ============================================================================================== */
+#ifndef LQX_H
+#define LQX_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct lqx_ctx lqx_ctx;     /* opaque; owned by the library, destroyed by lqx_finalize   */
+typedef struct lqx_field lqx_field; /* opaque handle; storage owned by the library or borrowed   */
+
+typedef enum { LQX_F32 = 4, LQX_F64 = 8 } lqx_prec; /* bytes per real */
+/* complex numbers per site: LatticeComplex, LatticeColorVector, LatticeColorMatrix, LatticeFermion
+ * (PAPER.md:69 sec.4, :138-145 Listing 1; BASELINE.json configs[1],[4]) */
+typedef enum { LQX_COMPLEX = 1, LQX_COLORVEC = 3, LQX_COLORMAT = 9, LQX_FERMION = 12 } lqx_kind;
+typedef enum { LQX_BACKWARD = -1, LQX_FORWARD = +1 } lqx_dir;
+
+typedef enum {
+    LQX_OK = 0,
+    LQX_EINVAL = -1,  /* null pointer, mu outside 0..3, dir not +-1, nsteps < 0, bad enum        */
+    LQX_ETYPE = -2,   /* operand kind / precision does not fit the expression                   */
+    LQX_EGEOM = -3,   /* extent < 1, V >= 2^31, operands from different contexts                */
+    LQX_EALIAS = -4,  /* destination aliases an operand that is read through a shift            */
+    LQX_ECUDA = -5,   /* a CUDA call failed; lqx_last_error has cudaGetErrorString              */
+    LQX_ENOMEM = -6   /* host or device allocation failed                                       */
+} lqx_status;
+
+/* ---------------------------------------------------------------------------------------------
+ * Geometry (the paper's "layout" + site tables)
+ * ------------------------------------------------------------------------------------------- */
+/* Create a context for an L0 x L1 x L2 x L3 periodic lattice on CUDA device `device`.
+ * `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream); the library
+ * never creates or destroys it.  Host pointer in (dims), handle out. */
+int lqx_init(const int dims[4], int device, void* cuda_stream, lqx_ctx** out);
+/* Frees every field handle still alive, library-owned device memory and scratch
+ * (the paper's theDeviceStorage::freeAll). */
+int lqx_finalize(lqx_ctx* ctx);
+int lqx_set_stream(lqx_ctx* ctx, void* cuda_stream);
+int64_t lqx_volume(const lqx_ctx* ctx);       /* V = L0*L1*L2*L3, or negative status            */
+int64_t lqx_plane_stride(const lqx_ctx* ctx); /* elements between component planes              */
+/* Bytes of device memory a field of this kind/precision occupies in the internal layout. */
+int64_t lqx_field_bytes(const lqx_ctx* ctx, lqx_kind kind, lqx_prec prec);
+/* Periodic neighbour table computed ON THE DEVICE by the same index arithmetic the kernels use:
+ * host_out[s] = site index of x(s) + dir*mu^ .  host_out: V int32, host memory.  Synchronises. */
+int lqx_neighbor_table(lqx_ctx* ctx, lqx_dir dir, int mu, int32_t* host_out);
+
+/* ---------------------------------------------------------------------------------------------
+ * Device field store (pushToDevice / popFromDevice / freeDeviceMem,
+ * PAPER.md:195-202 sec.6)
+ * ------------------------------------------------------------------------------------------- */
+int lqx_field_alloc(lqx_ctx* ctx, lqx_kind kind, lqx_prec prec, lqx_field** out);
+/* Borrow caller-owned device memory (e.g. a torch tensor) of at least lqx_field_bytes() bytes,
+ * 256-byte aligned; it is interpreted in the internal layout and never freed by the library. */
+int lqx_field_attach(lqx_ctx* ctx, lqx_kind kind, lqx_prec prec, void* dev_ptr, size_t bytes,
+                     lqx_field** out);
+int lqx_field_free(lqx_field* f);
+void* lqx_field_data(const lqx_field* f); /* device pointer of plane 0 (NULL on bad handle)     */
+int lqx_field_kind(const lqx_field* f);
+int lqx_field_prec(const lqx_field* f);
+/* host QDP order -> device SoA.  host: V*2*kind reals of the field precision.  Bit-exact. */
+int lqx_field_push(lqx_field* f, const void* host_qdp_order);
+/* device SoA -> host QDP order.  Synchronises.  Bit-exact.  Does not free (reading A4). */
+int lqx_field_pop(const lqx_field* f, void* host_qdp_order);
+/* Same converters between two DEVICE buffers (dev_qdp_order: V*2*kind reals, AoS). Asynchronous. */
+int lqx_field_import_dev(lqx_field* f, const void* dev_qdp_order);
+int lqx_field_export_dev(const lqx_field* f, void* dev_qdp_order);
+
+/* ---------------------------------------------------------------------------------------------
+ * Expression catalogue.  Destination first.
+ * ------------------------------------------------------------------------------------------- */
+/* E0 of Listing 1: r = a.  Any kind. */
+int lqx_copy(lqx_field* r, const lqx_field* a);
+/* r = shift(a, dir, mu): r(x) = a(x + dir*mu^).  Any kind.  Bit-exact.  r must not alias a. */
+int lqx_shift(lqx_field* r, const lqx_field* a, lqx_dir dir, int mu);
+/* form (i)  R = A*B + C*adj(D), colour matrices (BASELINE.json configs[4]) */
+int lqx_mm_plus_madj(lqx_field* r, const lqx_field* a, const lqx_field* b, const lqx_field* c,
+                     const lqx_field* d);
+/* form (ii) c = trace(A*B): colour matrices -> LatticeComplex */
+int lqx_trace_mm(lqx_field* c, const lqx_field* a, const lqx_field* b);
+/* form (iii) R = alpha*A - shift(B, dir, mu), colour matrices (configs[4]: alpha=2.5, BACKWARD, 2) */
+int lqx_ax_minus_shift(lqx_field* r, double alpha, const lqx_field* a, const lqx_field* b,
+                       lqx_dir dir, int mu);
+/* form (iv) w = M*v: colour matrix times colour vector, or times fermion (per spin component) */
+int lqx_mat_vec(lqx_field* w, const lqx_field* m, const lqx_field* v);
+/* The paper's hot expression E1/E2 (Listing 1 lines 25/27; Eq. 2 :215) fused
+ * over mu (BASELINE.json configs[1]):
+ *   chi(x) = sum_mu U_mu(x) psi(x+mu^) + adj(U_mu(x-mu^)) psi(x-mu^).
+ * psi, chi: fermion or colour vector; u[4]: colour matrices.  chi must not alias psi. */
+int lqx_hop(lqx_field* chi, const lqx_field* const u[4], const lqx_field* psi);
+/* The same with norm2(chi) fused into the pass; *norm2_out (host double) after a sync. */
+int lqx_hop_norm2(lqx_field* chi, const lqx_field* const u[4], const lqx_field* psi,
+                  double* norm2_out);
+/* E3 (reading A3): r = s0 + kappa*h.  Any kind. */
+int lqx_axpy(lqx_field* r, const lqx_field* s0, double kappa, const lqx_field* h);
+/* r = s*a (real scalar scaling) and E4 r = a / nrm as a true division (A22). */
+int lqx_scale(lqx_field* r, double s, const lqx_field* a);
+int lqx_divide(lqx_field* r, const lqx_field* a, double nrm);
+
+/* ---------------------------------------------------------------------------------------------
+ * Global reductions.  fp64 accumulation for both precisions, fixed summation
+ * tree (deterministic run to run).  Results to host double; these calls synchronise.
+ * ------------------------------------------------------------------------------------------- */
+int lqx_sum(const lqx_field* f, double* out);   /* out: 2*kind doubles, one site object, QDP order */
+int lqx_norm2(const lqx_field* f, double* out); /* sum_x sum_components |c|^2                      */
+int lqx_trace(const lqx_field* m, double out[2]); /* sum_x tr M(x) (reading A12)                   */
+/* P = sum_x sum_{mu<nu} Re tr[U_mu(x) U_nu(x+mu^) adj(U_mu(x+nu^)) adj(U_nu(x))];
+ * *plaq_sum = P, *plaq_avg = P/(18 V) (reading A11).  Either pointer may be NULL. */
+int lqx_plaquette(const lqx_field* const u[4], double* plaq_sum, double* plaq_avg);
+
+/* ---------------------------------------------------------------------------------------------
+ * Staple sum and smearing (BASELINE.json configs[0],[2],[3])
+ *   S_mu(x)  = sum_{nu != mu} [ U_nu(x) U_mu(x+nu^) adj(U_nu(x+mu^))
+ *                             + adj(U_nu(x-nu^)) U_mu(x-nu^) U_nu(x-nu^+mu^) ]
+ *   U'_mu(x) = (1-alpha) U_mu(x) + (alpha/6) S_mu(x)          (no projection, reading A9)
+ * ------------------------------------------------------------------------------------------- */
+/* out = S_mu for one direction (test/diagnostic entry). */
+int lqx_staple_sum(lqx_field* out, const lqx_field* const u[4], int mu);
+/* One smearing step, all four directions, out of place.  If plaq_in_or_null != NULL the plaquette
+ * sum of the INPUT field is accumulated in the same pass and stored there (host double; the call
+ * then synchronises). */
+int lqx_smear_step(lqx_field* const uout[4], const lqx_field* const uin[4], double alpha,
+                   double* plaq_in_or_null);
+/* nsteps iterated steps (configs[3]): result ends in u; tmp is ping-pong scratch.
+ * plaq_avg_after_each (host, nsteps doubles, may be NULL) = plaquette average of the field after
+ * every step.  One synchronisation at the end. */
+int lqx_smear_iterate(lqx_field* const u[4], lqx_field* const tmp[4], double alpha, int nsteps,
+                      double* plaq_avg_after_each);
+/* End-to-end form with HOST buffers (bench `e2e`): host_u_in[4] / host_u_out[4] are host colour
+ * matrix fields in QDP order of precision `prec`; pushes, iterates, pops. */
+int lqx_smear_iterate_host(lqx_ctx* ctx, lqx_prec prec, const void* const host_u_in[4],
+                           void* const host_u_out[4], double alpha, int nsteps,
+                           double* plaq_avg_after_each);
+
+/* ---------------------------------------------------------------------------------------------
+ * Harness support: device micro-benchmarks that give the roofline denominators.
+ * ------------------------------------------------------------------------------------------- */
+/* kind: 0 = fp32 FMA, 1 = packed fp32x2 FMA, 2 = fp64 FMA.  Returns achieved FMA lane-ops/s
+ * (one fused multiply-add on one real = 1 lane-op = 2 flop) in *lane_ops_per_s. */
+int lqx_bench_fma_peak(lqx_ctx* ctx, int kind, double* lane_ops_per_s);
+/* Plain device copy of `bytes` bytes (read + write counted): achieved bytes/s. */
+int lqx_bench_copy_peak(lqx_ctx* ctx, size_t bytes, double* bytes_per_s);
+/* Number of kernels this context has launched since init (for bench.py's gpu_launches). */
+int64_t lqx_launch_count(const lqx_ctx* ctx);
+/* Tuning knob for the smear kernel variant (0 = default/best). */
+int lqx_set_option(lqx_ctx* ctx, const char* key, int value);
+
+const char* lqx_strerror(int code);
+const char* lqx_last_error(const lqx_ctx* ctx);
+const char* lqx_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LQX_H */

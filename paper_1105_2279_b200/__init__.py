@@ -1,0 +1,366 @@
+"""paper_1105_2279_b200 -- thin Python binding of the lqx C-ABI library (include/lqx.h).
+
+Argument marshalling only: every step of the hot path runs in the CUDA kernels of liblqx.so.
+The raw layer mirrors the C names without the `lqx_` prefix (`init`, `field_alloc`, `smear_step`,
+...) and raises `LqxError` on a non-zero status.  `Lattice` / `Field` are small conveniences on
+top (torch supplies device memory and the stream; numpy/torch arrays in QDP order go in and out).
+
+There is no CPU fallback: if liblqx.so cannot be loaded or built, importing this package raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+F32, F64 = 4, 8
+COMPLEX, COLORVEC, COLORMAT, FERMION = 1, 3, 9, 12
+BACKWARD, FORWARD = -1, +1
+KIND_SHAPE = {COMPLEX: (), COLORVEC: (3,), COLORMAT: (3, 3), FERMION: (4, 3)}
+_NP = {F32: np.float32, F64: np.float64}
+
+
+class LqxError(RuntimeError):
+    def __init__(self, code, detail=""):
+        self.code = int(code)
+        msg = _lib.lqx_strerror(int(code)).decode()
+        super().__init__(f"lqx status {code} ({msg})" + (f": {detail}" if detail else ""))
+
+
+def _load():
+    path = _build.LIB
+    if not os.path.exists(path) or _build._stale(path, [os.path.join(_build.CSRC, s) for s in _build.SOURCES] + _build.HEADERS):
+        try:
+            path = _build.build()
+        except Exception as e:  # no nvcc on this machine: use the shipped .so if there is one
+            if not os.path.exists(_build.LIB):
+                raise ImportError(f"liblqx.so is missing and could not be built: {e}") from e
+            path = _build.LIB
+    return C.CDLL(path)
+
+
+_lib = _load()
+_vp, _i, _d, _i64 = C.c_void_p, C.c_int, C.c_double, C.c_int64
+_pvp = C.POINTER(C.c_void_p)
+_pd = C.POINTER(C.c_double)
+
+# name -> (restype, argtypes); every symbol include/lqx.h declares
+SIGNATURES = {
+    "lqx_init": (_i, [C.POINTER(C.c_int), _i, _vp, _pvp]),
+    "lqx_finalize": (_i, [_vp]),
+    "lqx_set_stream": (_i, [_vp, _vp]),
+    "lqx_volume": (_i64, [_vp]),
+    "lqx_plane_stride": (_i64, [_vp]),
+    "lqx_field_bytes": (_i64, [_vp, _i, _i]),
+    "lqx_neighbor_table": (_i, [_vp, _i, _i, _vp]),
+    "lqx_field_alloc": (_i, [_vp, _i, _i, _pvp]),
+    "lqx_field_attach": (_i, [_vp, _i, _i, _vp, C.c_size_t, _pvp]),
+    "lqx_field_free": (_i, [_vp]),
+    "lqx_field_data": (_vp, [_vp]),
+    "lqx_field_kind": (_i, [_vp]),
+    "lqx_field_prec": (_i, [_vp]),
+    "lqx_field_push": (_i, [_vp, _vp]),
+    "lqx_field_pop": (_i, [_vp, _vp]),
+    "lqx_field_import_dev": (_i, [_vp, _vp]),
+    "lqx_field_export_dev": (_i, [_vp, _vp]),
+    "lqx_copy": (_i, [_vp, _vp]),
+    "lqx_shift": (_i, [_vp, _vp, _i, _i]),
+    "lqx_mm_plus_madj": (_i, [_vp, _vp, _vp, _vp, _vp]),
+    "lqx_trace_mm": (_i, [_vp, _vp, _vp]),
+    "lqx_ax_minus_shift": (_i, [_vp, _d, _vp, _vp, _i, _i]),
+    "lqx_mat_vec": (_i, [_vp, _vp, _vp]),
+    "lqx_hop": (_i, [_vp, _pvp, _vp]),
+    "lqx_hop_norm2": (_i, [_vp, _pvp, _vp, _pd]),
+    "lqx_axpy": (_i, [_vp, _vp, _d, _vp]),
+    "lqx_scale": (_i, [_vp, _d, _vp]),
+    "lqx_divide": (_i, [_vp, _vp, _d]),
+    "lqx_sum": (_i, [_vp, _pd]),
+    "lqx_norm2": (_i, [_vp, _pd]),
+    "lqx_trace": (_i, [_vp, _pd]),
+    "lqx_plaquette": (_i, [_pvp, _pd, _pd]),
+    "lqx_staple_sum": (_i, [_vp, _pvp, _i]),
+    "lqx_smear_step": (_i, [_pvp, _pvp, _d, _pd]),
+    "lqx_smear_iterate": (_i, [_pvp, _pvp, _d, _i, _pd]),
+    "lqx_smear_iterate_host": (_i, [_vp, _i, _pvp, _pvp, _d, _i, _pd]),
+    "lqx_bench_fma_peak": (_i, [_vp, _i, _pd]),
+    "lqx_bench_copy_peak": (_i, [_vp, C.c_size_t, _pd]),
+    "lqx_launch_count": (_i64, [_vp]),
+    "lqx_set_option": (_i, [_vp, C.c_char_p, _i]),
+    "lqx_strerror": (C.c_char_p, [_i]),
+    "lqx_last_error": (C.c_char_p, [_vp]),
+    "lqx_version": (C.c_char_p, []),
+}
+for _name, (_res, _args) in SIGNATURES.items():
+    _fn = getattr(_lib, _name)
+    _fn.restype = _res
+    _fn.argtypes = _args
+
+
+def library_path() -> str:
+    return _lib._name
+
+
+def version() -> str:
+    return _lib.lqx_version().decode()
+
+
+def _check(rc, ctx=None):
+    if rc != 0:
+        detail = _lib.lqx_last_error(ctx).decode() if ctx else ""
+        raise LqxError(rc, detail)
+
+
+def _h(f):
+    return f.handle if isinstance(f, Field) else f
+
+
+def _arr4(fields):
+    return (C.c_void_p * 4)(*[_h(f) for f in fields])
+
+
+def _ctx_of(f):
+    return f.lat.ctx if isinstance(f, Field) else None
+
+
+# ------------------------------------------------------------------------------------------------
+# conveniences
+# ------------------------------------------------------------------------------------------------
+class Lattice:
+    """A context (lqx_init) bound to a CUDA device and to torch's current stream."""
+
+    def __init__(self, dims, device: int = 0, stream=None):
+        import torch
+
+        if not torch.cuda.is_available():
+            raise RuntimeError("lqx needs a CUDA device (there is no CPU fallback)")
+        self.dims = tuple(int(d) for d in dims)
+        self.device = int(device)
+        torch.cuda.set_device(self.device)
+        torch.cuda.init()
+        if stream is None:
+            stream = torch.cuda.current_stream(self.device)
+        self.stream = stream
+        out = C.c_void_p()
+        _check(_lib.lqx_init((C.c_int * 4)(*self.dims), self.device, C.c_void_p(stream.cuda_stream), C.byref(out)))
+        self.ctx = out
+        self.volume = int(_lib.lqx_volume(self.ctx))
+        self.stride = int(_lib.lqx_plane_stride(self.ctx))
+        self._fields = []
+
+    def close(self):
+        if self.ctx:
+            for f in self._fields:
+                f.handle = None
+                f._mem = None
+            _check(_lib.lqx_finalize(self.ctx))
+            self.ctx = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+    def field_bytes(self, kind, prec) -> int:
+        return int(_lib.lqx_field_bytes(self.ctx, kind, prec))
+
+    def alloc(self, kind, prec, torch_memory: bool = True) -> "Field":
+        """New zero field.  torch_memory=True: a torch uint8 tensor owns the bytes and the library
+        borrows them (lqx_field_attach); False: the library allocates (lqx_field_alloc)."""
+        out = C.c_void_p()
+        mem = None
+        if torch_memory:
+            import torch
+
+            nbytes = self.field_bytes(kind, prec)
+            with torch.cuda.stream(self.stream):
+                mem = torch.zeros(nbytes, dtype=torch.uint8, device=f"cuda:{self.device}")
+            _check(_lib.lqx_field_attach(self.ctx, kind, prec, C.c_void_p(mem.data_ptr()), nbytes, C.byref(out)), self.ctx)
+        else:
+            _check(_lib.lqx_field_alloc(self.ctx, kind, prec, C.byref(out)), self.ctx)
+        f = Field(self, out, kind, prec, mem)
+        self._fields.append(f)
+        return f
+
+    def from_host(self, array, kind=None) -> "Field":
+        """Push a QDP-order host array ([V, *shape, 2], float32/float64, numpy or torch CPU)."""
+        a = _as_numpy(array)
+        if kind is None:
+            kind = {(): COMPLEX, (3,): COLORVEC, (3, 3): COLORMAT, (4, 3): FERMION}[tuple(a.shape[1:-1])]
+        prec = {np.dtype(np.float32): F32, np.dtype(np.float64): F64}[a.dtype]
+        f = self.alloc(kind, prec)
+        f.push(a)
+        return f
+
+    def neighbor_table(self, direction, mu):
+        out = np.empty(self.volume, dtype=np.int32)
+        _check(_lib.lqx_neighbor_table(self.ctx, direction, mu, out.ctypes.data_as(C.c_void_p)), self.ctx)
+        return out
+
+    def set_option(self, key: str, value: int):
+        _check(_lib.lqx_set_option(self.ctx, key.encode(), int(value)), self.ctx)
+
+    def launch_count(self) -> int:
+        return int(_lib.lqx_launch_count(self.ctx))
+
+    def bench_fma_peak(self, kind: int) -> float:
+        out = C.c_double()
+        _check(_lib.lqx_bench_fma_peak(self.ctx, kind, C.byref(out)), self.ctx)
+        return out.value
+
+    def bench_copy_peak(self, nbytes: int) -> float:
+        out = C.c_double()
+        _check(_lib.lqx_bench_copy_peak(self.ctx, nbytes, C.byref(out)), self.ctx)
+        return out.value
+
+
+def _as_numpy(array):
+    if hasattr(array, "detach"):
+        array = array.detach().cpu().numpy()
+    return np.ascontiguousarray(array)
+
+
+class Field:
+    def __init__(self, lat, handle, kind, prec, mem=None):
+        self.lat, self.handle, self.kind, self.prec, self._mem = lat, handle, kind, prec, mem
+
+    @property
+    def host_shape(self):
+        return (self.lat.volume,) + KIND_SHAPE[self.kind] + (2,)
+
+    def push(self, array):
+        a = _as_numpy(array)
+        if a.dtype != _NP[self.prec] or a.size != int(np.prod(self.host_shape)):
+            raise TypeError(f"push wants {_NP[self.prec].__name__} with {self.host_shape}, got {a.dtype} {a.shape}")
+        _check(_lib.lqx_field_push(self.handle, a.ctypes.data_as(C.c_void_p)), self.lat.ctx)
+        return self
+
+    def pop(self):
+        out = np.empty(self.host_shape, dtype=_NP[self.prec])
+        _check(_lib.lqx_field_pop(self.handle, out.ctypes.data_as(C.c_void_p)), self.lat.ctx)
+        return out
+
+    def import_dev(self, dev_tensor):
+        """AoS QDP-order torch CUDA tensor -> this field (device to device)."""
+        _check(_lib.lqx_field_import_dev(self.handle, C.c_void_p(dev_tensor.data_ptr())), self.lat.ctx)
+        return self
+
+    def export_dev(self, dev_tensor):
+        _check(_lib.lqx_field_export_dev(self.handle, C.c_void_p(dev_tensor.data_ptr())), self.lat.ctx)
+        return dev_tensor
+
+    def free(self):
+        if self.handle:
+            _check(_lib.lqx_field_free(self.handle), self.lat.ctx)
+            self.handle = None
+            self._mem = None
+            if self in self.lat._fields:
+                self.lat._fields.remove(self)
+
+
+# ------------------------------------------------------------------------------------------------
+# raw layer: the C names without the prefix
+# ------------------------------------------------------------------------------------------------
+def copy(r, a):
+    _check(_lib.lqx_copy(_h(r), _h(a)), _ctx_of(r))
+
+
+def shift(r, a, direction, mu):
+    _check(_lib.lqx_shift(_h(r), _h(a), direction, mu), _ctx_of(r))
+
+
+def mm_plus_madj(r, a, b, c, d):
+    _check(_lib.lqx_mm_plus_madj(_h(r), _h(a), _h(b), _h(c), _h(d)), _ctx_of(r))
+
+
+def trace_mm(c, a, b):
+    _check(_lib.lqx_trace_mm(_h(c), _h(a), _h(b)), _ctx_of(c))
+
+
+def ax_minus_shift(r, alpha, a, b, direction, mu):
+    _check(_lib.lqx_ax_minus_shift(_h(r), float(alpha), _h(a), _h(b), direction, mu), _ctx_of(r))
+
+
+def mat_vec(w, m, v):
+    _check(_lib.lqx_mat_vec(_h(w), _h(m), _h(v)), _ctx_of(w))
+
+
+def hop(chi, u, psi):
+    _check(_lib.lqx_hop(_h(chi), _arr4(u), _h(psi)), _ctx_of(chi))
+
+
+def hop_norm2(chi, u, psi) -> float:
+    out = C.c_double()
+    _check(_lib.lqx_hop_norm2(_h(chi), _arr4(u), _h(psi), C.byref(out)), _ctx_of(chi))
+    return out.value
+
+
+def axpy(r, s0, kappa, h):
+    _check(_lib.lqx_axpy(_h(r), _h(s0), float(kappa), _h(h)), _ctx_of(r))
+
+
+def scale(r, s, a):
+    _check(_lib.lqx_scale(_h(r), float(s), _h(a)), _ctx_of(r))
+
+
+def divide(r, a, nrm):
+    _check(_lib.lqx_divide(_h(r), _h(a), float(nrm)), _ctx_of(r))
+
+
+def sum(f):  # noqa: A001 - mirrors the C name
+    n = 2 * f.kind
+    out = (C.c_double * n)()
+    _check(_lib.lqx_sum(_h(f), out), _ctx_of(f))
+    return np.array(out[:], dtype=np.float64).reshape(KIND_SHAPE[f.kind] + (2,))
+
+
+def norm2(f) -> float:
+    out = C.c_double()
+    _check(_lib.lqx_norm2(_h(f), C.byref(out)), _ctx_of(f))
+    return out.value
+
+
+def trace(m):
+    out = (C.c_double * 2)()
+    _check(_lib.lqx_trace(_h(m), out), _ctx_of(m))
+    return np.array(out[:], dtype=np.float64)
+
+
+def plaquette(u):
+    """-> (plaq_sum, plaq_avg)"""
+    s, a = C.c_double(), C.c_double()
+    _check(_lib.lqx_plaquette(_arr4(u), C.byref(s), C.byref(a)), _ctx_of(u[0]))
+    return s.value, a.value
+
+
+def staple_sum(out, u, mu):
+    _check(_lib.lqx_staple_sum(_h(out), _arr4(u), mu), _ctx_of(out))
+
+
+def smear_step(uout, uin, alpha, want_plaq_in: bool = False):
+    """One smearing step; returns the plaquette SUM of the input field if want_plaq_in."""
+    p = C.c_double()
+    _check(_lib.lqx_smear_step(_arr4(uout), _arr4(uin), float(alpha), C.byref(p) if want_plaq_in else None), _ctx_of(uin[0]))
+    return p.value if want_plaq_in else None
+
+
+def smear_iterate(u, tmp, alpha, nsteps, want_plaq: bool = True):
+    """nsteps steps in place (tmp = ping-pong scratch); returns plaquette averages after each step."""
+    out = (C.c_double * max(1, nsteps))()
+    _check(_lib.lqx_smear_iterate(_arr4(u), _arr4(tmp), float(alpha), int(nsteps), out if want_plaq else None), _ctx_of(u[0]))
+    return list(out[:nsteps]) if want_plaq else None
+
+
+def smear_iterate_host(lat: Lattice, prec, host_u_in, host_u_out, alpha, nsteps):
+    """End-to-end call with HOST buffers in QDP order (numpy or pinned torch CPU tensors)."""
+    def ptr(a):
+        return a.data_ptr() if hasattr(a, "data_ptr") else a.ctypes.data
+
+    pin = (C.c_void_p * 4)(*[ptr(a) for a in host_u_in])
+    pout = (C.c_void_p * 4)(*[ptr(a) for a in host_u_out])
+    out = (C.c_double * max(1, nsteps))()
+    _check(_lib.lqx_smear_iterate_host(lat.ctx, prec, pin, pout, float(alpha), int(nsteps), out), lat.ctx)
+    return list(out[:nsteps])

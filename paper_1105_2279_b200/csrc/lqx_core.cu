@@ -1,0 +1,381 @@
+// lqx core: context, geometry, device field store with QDP-order <-> SoA converters
+// (SURVEY 8(a) a1, a2; PAPER.md:101-103 site tables, :195-202 push/pop/free), error handling and
+// the shared second stage of the reductions.
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <algorithm>
+#include <new>
+
+#include "lqx_internal.cuh"
+
+// --------------------------------------------------------------------------------------------
+// errors
+// --------------------------------------------------------------------------------------------
+int lqx_fail(lqx_ctx* ctx, int code, const char* what) {
+    if (ctx) ctx->last_error = what ? what : "";
+    return code;
+}
+int lqx_cuda_fail(lqx_ctx* ctx, cudaError_t e, const char* where) {
+    if (ctx) {
+        ctx->last_error = std::string(where ? where : "cuda") + ": " + cudaGetErrorString(e);
+    }
+    return LQX_ECUDA;
+}
+
+extern "C" const char* lqx_strerror(int code) {
+    switch (code) {
+        case LQX_OK: return "ok";
+        case LQX_EINVAL: return "invalid argument";
+        case LQX_ETYPE: return "operand kind or precision mismatch";
+        case LQX_EGEOM: return "geometry mismatch or unsupported lattice";
+        case LQX_EALIAS: return "destination aliases a shifted operand";
+        case LQX_ECUDA: return "CUDA error";
+        case LQX_ENOMEM: return "out of memory";
+        default: return "unknown lqx status";
+    }
+}
+extern "C" const char* lqx_last_error(const lqx_ctx* ctx) { return ctx ? ctx->last_error.c_str() : ""; }
+extern "C" const char* lqx_version(void) { return "lqx 0.1 (sm_100a)"; }
+
+// --------------------------------------------------------------------------------------------
+// geometry
+// --------------------------------------------------------------------------------------------
+static FastDiv make_fastdiv(uint32_t d) {
+    FastDiv f;
+    f.d = d;
+    uint32_t sh = 0;
+    while ((1ull << sh) < d) ++sh;
+    f.sh = sh;
+    unsigned __int128 num = (unsigned __int128)1 << (31 + sh);
+    f.mul = (uint32_t)((num + d - 1) / d);
+    return f;
+}
+
+extern "C" int lqx_init(const int dims[4], int device, void* cuda_stream, lqx_ctx** out) {
+    if (!dims || !out) return LQX_EINVAL;
+    *out = nullptr;
+    int64_t v = 1;
+    for (int d = 0; d < 4; ++d) {
+        if (dims[d] < 1) return LQX_EGEOM;
+        v *= dims[d];
+        if (v >= ((int64_t)1 << 31) - 64) return LQX_EGEOM;
+    }
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return LQX_ECUDA;
+    if (cudaSetDevice(device) != cudaSuccess) return LQX_ECUDA;
+    lqx_ctx* c = new (std::nothrow) lqx_ctx();
+    if (!c) return LQX_ENOMEM;
+    Geo& g = c->geo;
+    int st = 1;
+    for (int d = 0; d < 4; ++d) {
+        g.L[d] = dims[d];
+        g.stride_site[d] = st;
+        st *= dims[d];
+    }
+    g.V = (int)v;
+    g.stride = (int)((v + 31) & ~(int64_t)31);
+    g.d0 = make_fastdiv((uint32_t)dims[0]);
+    g.d1 = make_fastdiv((uint32_t)dims[1]);
+    g.d2 = make_fastdiv((uint32_t)dims[2]);
+    c->device = device;
+    c->stream = (cudaStream_t)cuda_stream;
+    c->d_partials = nullptr;
+    c->partials_cap = 0;
+    c->d_result = nullptr;
+    c->h_result = nullptr;
+    c->launches = 0;
+    c->opt_smear_variant = 0;
+    c->opt_block = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) {
+        delete c;
+        return LQX_ECUDA;
+    }
+    c->num_sms = prop.multiProcessorCount;
+    if (cudaMalloc(&c->d_result, 64 * sizeof(double)) != cudaSuccess ||
+        cudaMallocHost(&c->h_result, 64 * sizeof(double)) != cudaSuccess) {
+        if (c->d_result) cudaFree(c->d_result);
+        delete c;
+        return LQX_ENOMEM;
+    }
+    *out = c;
+    return LQX_OK;
+}
+
+extern "C" int lqx_finalize(lqx_ctx* ctx) {
+    if (!ctx) return LQX_EINVAL;
+    cudaSetDevice(ctx->device);
+    cudaStreamSynchronize(ctx->stream);
+    for (lqx_field* f : ctx->fields) {
+        if (f->owned && f->data) cudaFree(f->data);
+        delete f;
+    }
+    if (ctx->d_partials) cudaFree(ctx->d_partials);
+    if (ctx->d_result) cudaFree(ctx->d_result);
+    if (ctx->h_result) cudaFreeHost(ctx->h_result);
+    delete ctx;
+    return LQX_OK;
+}
+
+extern "C" int lqx_set_stream(lqx_ctx* ctx, void* cuda_stream) {
+    if (!ctx) return LQX_EINVAL;
+    ctx->stream = (cudaStream_t)cuda_stream;
+    return LQX_OK;
+}
+extern "C" int64_t lqx_volume(const lqx_ctx* ctx) { return ctx ? ctx->geo.V : (int64_t)LQX_EINVAL; }
+extern "C" int64_t lqx_plane_stride(const lqx_ctx* ctx) { return ctx ? ctx->geo.stride : (int64_t)LQX_EINVAL; }
+extern "C" int64_t lqx_launch_count(const lqx_ctx* ctx) { return ctx ? ctx->launches : (int64_t)LQX_EINVAL; }
+
+static bool valid_kind(int k) { return k == LQX_COMPLEX || k == LQX_COLORVEC || k == LQX_COLORMAT || k == LQX_FERMION; }
+static bool valid_prec(int p) { return p == LQX_F32 || p == LQX_F64; }
+
+extern "C" int64_t lqx_field_bytes(const lqx_ctx* ctx, lqx_kind kind, lqx_prec prec) {
+    if (!ctx || !valid_kind(kind) || !valid_prec(prec)) return LQX_EINVAL;
+    return (int64_t)ctx->geo.stride * 2 * (int)kind * (int)prec;
+}
+
+extern "C" int lqx_set_option(lqx_ctx* ctx, const char* key, int value) {
+    if (!ctx || !key) return LQX_EINVAL;
+    if (!strcmp(key, "smear_variant")) ctx->opt_smear_variant = value;
+    else if (!strcmp(key, "block")) ctx->opt_block = value;
+    else return lqx_fail(ctx, LQX_EINVAL, "unknown option");
+    return LQX_OK;
+}
+
+__global__ void k_neighbor_table(const __grid_constant__ Geo g, int dir, int mu, int32_t* __restrict__ out) {
+    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= g.V) return;
+    int x[4];
+    site_coords(g, s, x);
+    out[s] = dir > 0 ? nbr_fwd(g, s, x, mu) : nbr_bwd(g, s, x, mu);
+}
+
+extern "C" int lqx_neighbor_table(lqx_ctx* ctx, lqx_dir dir, int mu, int32_t* host_out) {
+    if (!ctx || !host_out) return LQX_EINVAL;
+    if (mu < 0 || mu > 3 || (dir != LQX_FORWARD && dir != LQX_BACKWARD)) return lqx_fail(ctx, LQX_EINVAL, "mu/dir");
+    LQX_CUDA(ctx, cudaSetDevice(ctx->device));
+    int32_t* d = nullptr;
+    const int V = ctx->geo.V;
+    if (cudaMalloc(&d, (size_t)V * sizeof(int32_t)) != cudaSuccess) return lqx_fail(ctx, LQX_ENOMEM, "neighbor table");
+    k_neighbor_table<<<(V + 255) / 256, 256, 0, ctx->stream>>>(ctx->geo, (int)dir, mu, d);
+    ctx->launches++;
+    cudaError_t e = cudaMemcpyAsync(host_out, d, (size_t)V * sizeof(int32_t), cudaMemcpyDeviceToHost, ctx->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    cudaFree(d);
+    if (e != cudaSuccess) return lqx_cuda_fail(ctx, e, "neighbor table");
+    return LQX_OK;
+}
+
+// --------------------------------------------------------------------------------------------
+// fields
+// --------------------------------------------------------------------------------------------
+static int new_field(lqx_ctx* ctx, lqx_kind kind, lqx_prec prec, void* ptr, bool owned, lqx_field** out) {
+    lqx_field* f = new (std::nothrow) lqx_field();
+    if (!f) return lqx_fail(ctx, LQX_ENOMEM, "field handle");
+    f->ctx = ctx;
+    f->kind = kind;
+    f->prec = prec;
+    f->data = ptr;
+    f->owned = owned;
+    ctx->fields.push_back(f);
+    *out = f;
+    return LQX_OK;
+}
+
+extern "C" int lqx_field_alloc(lqx_ctx* ctx, lqx_kind kind, lqx_prec prec, lqx_field** out) {
+    if (!ctx || !out) return LQX_EINVAL;
+    *out = nullptr;
+    if (!valid_kind(kind) || !valid_prec(prec)) return lqx_fail(ctx, LQX_EINVAL, "kind/prec");
+    LQX_CUDA(ctx, cudaSetDevice(ctx->device));
+    void* p = nullptr;
+    size_t bytes = (size_t)lqx_field_bytes(ctx, kind, prec);
+    if (cudaMalloc(&p, bytes) != cudaSuccess) {
+        cudaGetLastError();
+        return lqx_fail(ctx, LQX_ENOMEM, "cudaMalloc field");
+    }
+    // the pad between V and the plane stride is never read for results, but keep it defined
+    cudaError_t e = cudaMemsetAsync(p, 0, bytes, ctx->stream);
+    if (e != cudaSuccess) {
+        cudaFree(p);
+        return lqx_cuda_fail(ctx, e, "memset");
+    }
+    int rc = new_field(ctx, kind, prec, p, true, out);
+    if (rc != LQX_OK) cudaFree(p);
+    return rc;
+}
+
+extern "C" int lqx_field_attach(lqx_ctx* ctx, lqx_kind kind, lqx_prec prec, void* dev_ptr, size_t bytes,
+                                lqx_field** out) {
+    if (!ctx || !out || !dev_ptr) return LQX_EINVAL;
+    *out = nullptr;
+    if (!valid_kind(kind) || !valid_prec(prec)) return lqx_fail(ctx, LQX_EINVAL, "kind/prec");
+    if ((int64_t)bytes < lqx_field_bytes(ctx, kind, prec)) return lqx_fail(ctx, LQX_EINVAL, "attached buffer too small");
+    if (((uintptr_t)dev_ptr & 255) != 0) return lqx_fail(ctx, LQX_EINVAL, "attached buffer not 256-byte aligned");
+    return new_field(ctx, kind, prec, dev_ptr, false, out);
+}
+
+extern "C" int lqx_field_free(lqx_field* f) {
+    if (!f) return LQX_EINVAL;
+    lqx_ctx* ctx = f->ctx;
+    auto it = std::find(ctx->fields.begin(), ctx->fields.end(), f);
+    if (it == ctx->fields.end()) return lqx_fail(ctx, LQX_EINVAL, "unknown field handle");
+    ctx->fields.erase(it);
+    if (f->owned && f->data) {
+        cudaSetDevice(ctx->device);
+        cudaStreamSynchronize(ctx->stream);
+        cudaFree(f->data);
+    }
+    delete f;
+    return LQX_OK;
+}
+extern "C" void* lqx_field_data(const lqx_field* f) { return f ? f->data : nullptr; }
+extern "C" int lqx_field_kind(const lqx_field* f) { return f ? (int)f->kind : LQX_EINVAL; }
+extern "C" int lqx_field_prec(const lqx_field* f) { return f ? (int)f->prec : LQX_EINVAL; }
+
+// AoS (QDP order) <-> SoA.  One block handles 32 consecutive sites through shared memory so that
+// both the AoS side (32*NR contiguous reals) and the SoA side (NR runs of 32 reals) are coalesced.
+template <typename T, bool TO_SOA>
+__global__ void k_transpose(int V, int stride, int nreal, const T* __restrict__ src, T* __restrict__ dst) {
+    extern __shared__ unsigned char smem_raw[];
+    T* tile = reinterpret_cast<T*>(smem_raw);  // [32][nreal+1]
+    const int s0 = blockIdx.x * 32;
+    const int ns = min(32, V - s0);
+    const int pitch = nreal + 1;
+    if (TO_SOA) {
+        const T* a = src + (size_t)s0 * nreal;
+        for (int i = threadIdx.x; i < ns * nreal; i += blockDim.x) tile[(i / nreal) * pitch + (i % nreal)] = a[i];
+        __syncthreads();
+        for (int i = threadIdx.x; i < 32 * nreal; i += blockDim.x) {
+            int r = i >> 5, ls = i & 31;
+            if (ls < ns) dst[(size_t)r * stride + s0 + ls] = tile[ls * pitch + r];
+        }
+    } else {
+        for (int i = threadIdx.x; i < 32 * nreal; i += blockDim.x) {
+            int r = i >> 5, ls = i & 31;
+            if (ls < ns) tile[ls * pitch + r] = src[(size_t)r * stride + s0 + ls];
+        }
+        __syncthreads();
+        T* a = dst + (size_t)s0 * nreal;
+        for (int i = threadIdx.x; i < ns * nreal; i += blockDim.x) a[i] = tile[(i / nreal) * pitch + (i % nreal)];
+    }
+}
+
+static int transpose_launch(lqx_ctx* ctx, const lqx_field* f, const void* src, void* dst, bool to_soa) {
+    const Geo& g = ctx->geo;
+    const int nreal = 2 * (int)f->kind;
+    const int nblk = (g.V + 31) / 32;
+    const size_t sm = (size_t)32 * (nreal + 1) * (int)f->prec;
+    if (f->prec == LQX_F32) {
+        if (to_soa) k_transpose<float, true><<<nblk, 256, sm, ctx->stream>>>(g.V, g.stride, nreal, (const float*)src, (float*)dst);
+        else k_transpose<float, false><<<nblk, 256, sm, ctx->stream>>>(g.V, g.stride, nreal, (const float*)src, (float*)dst);
+    } else {
+        if (to_soa) k_transpose<double, true><<<nblk, 256, sm, ctx->stream>>>(g.V, g.stride, nreal, (const double*)src, (double*)dst);
+        else k_transpose<double, false><<<nblk, 256, sm, ctx->stream>>>(g.V, g.stride, nreal, (const double*)src, (double*)dst);
+    }
+    LQX_LAUNCH_CHECK(ctx);
+    return LQX_OK;
+}
+
+extern "C" int lqx_field_import_dev(lqx_field* f, const void* dev_qdp_order) {
+    if (!f || !dev_qdp_order) return LQX_EINVAL;
+    LQX_CUDA(f->ctx, cudaSetDevice(f->ctx->device));
+    return transpose_launch(f->ctx, f, dev_qdp_order, f->data, true);
+}
+extern "C" int lqx_field_export_dev(const lqx_field* f, void* dev_qdp_order) {
+    if (!f || !dev_qdp_order) return LQX_EINVAL;
+    LQX_CUDA(f->ctx, cudaSetDevice(f->ctx->device));
+    return transpose_launch(f->ctx, f, f->data, dev_qdp_order, false);
+}
+
+extern "C" int lqx_field_push(lqx_field* f, const void* host) {
+    if (!f || !host) return LQX_EINVAL;
+    lqx_ctx* ctx = f->ctx;
+    LQX_CUDA(ctx, cudaSetDevice(ctx->device));
+    const size_t bytes = (size_t)ctx->geo.V * 2 * (int)f->kind * (int)f->prec;
+    void* stage = nullptr;
+    if (cudaMalloc(&stage, bytes) != cudaSuccess) {
+        cudaGetLastError();
+        return lqx_fail(ctx, LQX_ENOMEM, "push staging buffer");
+    }
+    cudaError_t e = cudaMemcpyAsync(stage, host, bytes, cudaMemcpyHostToDevice, ctx->stream);
+    int rc = LQX_OK;
+    if (e != cudaSuccess) rc = lqx_cuda_fail(ctx, e, "push H2D");
+    if (rc == LQX_OK) rc = transpose_launch(ctx, f, stage, f->data, true);
+    e = cudaStreamSynchronize(ctx->stream);  // host buffer is only touched during the call
+    if (rc == LQX_OK && e != cudaSuccess) rc = lqx_cuda_fail(ctx, e, "push sync");
+    cudaFree(stage);
+    return rc;
+}
+
+extern "C" int lqx_field_pop(const lqx_field* f, void* host) {
+    if (!f || !host) return LQX_EINVAL;
+    lqx_ctx* ctx = f->ctx;
+    LQX_CUDA(ctx, cudaSetDevice(ctx->device));
+    const size_t bytes = (size_t)ctx->geo.V * 2 * (int)f->kind * (int)f->prec;
+    void* stage = nullptr;
+    if (cudaMalloc(&stage, bytes) != cudaSuccess) {
+        cudaGetLastError();
+        return lqx_fail(ctx, LQX_ENOMEM, "pop staging buffer");
+    }
+    int rc = transpose_launch(ctx, f, f->data, stage, false);
+    cudaError_t e = cudaSuccess;
+    if (rc == LQX_OK) e = cudaMemcpyAsync(host, stage, bytes, cudaMemcpyDeviceToHost, ctx->stream);
+    if (rc == LQX_OK && e != cudaSuccess) rc = lqx_cuda_fail(ctx, e, "pop D2H");
+    e = cudaStreamSynchronize(ctx->stream);
+    if (rc == LQX_OK && e != cudaSuccess) rc = lqx_cuda_fail(ctx, e, "pop sync");
+    cudaFree(stage);
+    return rc;
+}
+
+// --------------------------------------------------------------------------------------------
+// reduction second stage
+// --------------------------------------------------------------------------------------------
+int lqx_ensure_partials(lqx_ctx* ctx, size_t ndoubles) {
+    if (ctx->partials_cap >= ndoubles) return LQX_OK;
+    if (ctx->d_partials) {
+        cudaStreamSynchronize(ctx->stream);
+        cudaFree(ctx->d_partials);
+        ctx->d_partials = nullptr;
+        ctx->partials_cap = 0;
+    }
+    size_t cap = std::max<size_t>(ndoubles, 1 << 16);
+    if (cudaMalloc(&ctx->d_partials, cap * sizeof(double)) != cudaSuccess) {
+        cudaGetLastError();
+        return lqx_fail(ctx, LQX_ENOMEM, "reduction scratch");
+    }
+    ctx->partials_cap = cap;
+    return LQX_OK;
+}
+
+// one block per component; fixed strided accumulation + fixed tree => deterministic
+__global__ void k_reduce_finish(const double* __restrict__ partials, int nblocks, double* __restrict__ out) {
+    __shared__ double sh[32];
+    const double* p = partials + (size_t)blockIdx.x * nblocks;
+    double t = 0.0;
+    for (int i = threadIdx.x; i < nblocks; i += blockDim.x) t += p[i];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = t;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        t = (threadIdx.x < (blockDim.x >> 5)) ? sh[threadIdx.x] : 0.0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+        if (threadIdx.x == 0) out[blockIdx.x] = t;
+    }
+}
+
+int lqx_reduce_finish(lqx_ctx* ctx, int nblocks, int ncomp, double* d_out) {
+    k_reduce_finish<<<ncomp, 1024, 0, ctx->stream>>>(ctx->d_partials, nblocks, d_out);
+    LQX_LAUNCH_CHECK(ctx);
+    return LQX_OK;
+}
+
+int lqx_fetch_result(lqx_ctx* ctx, int n, double* out) {
+    LQX_CUDA(ctx, cudaMemcpyAsync(ctx->h_result, ctx->d_result, n * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    LQX_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    for (int i = 0; i < n; ++i) out[i] = ctx->h_result[i];
+    return LQX_OK;
+}

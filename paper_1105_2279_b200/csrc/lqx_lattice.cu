@@ -1,0 +1,405 @@
+// lqx nearest-neighbour kernels: hop, plaquette (a8), staple sum + smear step (a7)
+// and the iterated smearing driver (a10).  Each is a single pass in which one thread evaluates the
+// whole expression of its site, reading shifted operands at the periodic
+// neighbour computed in-kernel (the role of the paper's site tables).
+#include "lqx_internal.cuh"
+
+namespace {
+
+template <typename T>
+struct Links {
+    const T* u[4];
+};
+template <typename T>
+struct LinksOut {
+    T* u[4];
+};
+
+// ---------------------------------------------------------------------------------------------
+// hop: chi(x) = sum_mu U_mu(x) psi(x+mu^) + adj(U_mu(x-mu^)) psi(x-mu^)
+// (Listing 1 lines 25/27 summed over mu; Eq. 2; BASELINE configs[1])
+// ---------------------------------------------------------------------------------------------
+template <typename T, int NSPIN, bool NORM2>
+__global__ void __launch_bounds__(128) k_hop(const __grid_constant__ Geo g, const __grid_constant__ Links<T> u, const T* __restrict__ psi, T* __restrict__ chi,
+                                             double* __restrict__ partials) {
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    double n2[1] = {0.0};
+    if (s < g.V) {
+        int x[4];
+        site_coords(g, s, x);
+        Vec3<T> acc[NSPIN];
+#pragma unroll
+        for (int a = 0; a < NSPIN; ++a)
+#pragma unroll
+            for (int i = 0; i < 3; ++i) acc[a].re[i] = acc[a].im[i] = T(0);
+#pragma unroll
+        for (int mu = 0; mu < 4; ++mu) {
+            const int f = nbr_fwd(g, s, x, mu), b = nbr_bwd(g, s, x, mu);
+            {
+                Mat3<T> m = load_mat(u.u[mu], g.stride, s);
+#pragma unroll
+                for (int a = 0; a < NSPIN; ++a) mac_mv(acc[a], m, load_vec(psi, g.stride, f, a));
+            }
+            {
+                Mat3<T> m = load_mat(u.u[mu], g.stride, b);
+#pragma unroll
+                for (int a = 0; a < NSPIN; ++a) mac_adj_mv(acc[a], m, load_vec(psi, g.stride, b, a));
+            }
+        }
+#pragma unroll
+        for (int a = 0; a < NSPIN; ++a) {
+            store_vec(chi, g.stride, s, a, acc[a]);
+            if (NORM2) {
+#pragma unroll
+                for (int i = 0; i < 3; ++i) {
+                    n2[0] = fma((double)acc[a].re[i], (double)acc[a].re[i], n2[0]);
+                    n2[0] = fma((double)acc[a].im[i], (double)acc[a].im[i], n2[0]);
+                }
+            }
+        }
+    }
+    if (NORM2) block_reduce_store<1>(n2, partials, gridDim.x, blockIdx.x);
+}
+
+// ---------------------------------------------------------------------------------------------
+// plaquette: sum_{mu<nu} Re tr[U_mu(x) U_nu(x+mu^) adj(U_mu(x+nu^)) adj(U_nu(x))]
+//          = sum_{mu<nu} Re tr[Q_munu(x) adj(Q_numu(x))],  Q_ab(x) = U_a(x) U_b(x+a^)
+// ---------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void __launch_bounds__(128) k_plaquette(const __grid_constant__ Geo g, const __grid_constant__ Links<T> u, double* __restrict__ partials) {
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    double p[1] = {0.0};
+    if (s < g.V) {
+        int x[4];
+        site_coords(g, s, x);
+        T acc = T(0);
+#pragma unroll 1
+        for (int mu = 0; mu < 3; ++mu) {
+            const Mat3<T> a = load_mat(u.u[mu], g.stride, s);
+            const int xpmu = nbr_fwd(g, s, x, mu);
+#pragma unroll 1
+            for (int nu = mu + 1; nu < 4; ++nu) {
+                const int xpnu = nbr_fwd(g, s, x, nu);
+                Mat3<T> q1 = mul_nn(a, load_mat(u.u[nu], g.stride, xpmu));
+                Mat3<T> q2 = mul_nn(load_mat(u.u[nu], g.stride, s), load_mat(u.u[mu], g.stride, xpnu));
+                acc += re_tr_na(q1, q2);
+            }
+        }
+        p[0] = (double)acc;
+    }
+    block_reduce_store<1>(p, partials, gridDim.x, blockIdx.x);
+}
+
+// ---------------------------------------------------------------------------------------------
+// staple sum + smear step, literal gather form (variant 1): one thread per site, mu and nu loops
+// inside; every staple is a chain of two products kept in registers.
+//   S_mu(x) = sum_{nu!=mu} U_nu(x) U_mu(x+nu^) adj(U_nu(x+mu^)) + adj(U_nu(x-nu^)) U_mu(x-nu^) U_nu(x-nu^+mu^)
+//   U'_mu(x) = c0 U_mu(x) + c1 S_mu(x)
+// PLAQ: the plaquette of the INPUT field is accumulated on the way:
+//   Re tr[U_mu U_nu(x+mu) adj(U_mu(x+nu)) adj(U_nu)] = Re tr[U_mu(x) adj(upper staple_{mu,nu}(x))], mu<nu.
+// ONLY_MU >= 0: write the bare staple sum of that direction into out.u[0] (diagnostic entry).
+// ---------------------------------------------------------------------------------------------
+template <typename T, bool PLAQ>
+__global__ void __launch_bounds__(128) k_smear_gather(const __grid_constant__ Geo g, const __grid_constant__ Links<T> u, const __grid_constant__ LinksOut<T> out, T c0, T c1, int only_mu,
+                                                      double* __restrict__ partials) {
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    double p[1] = {0.0};
+    if (s < g.V) {
+        int x[4];
+        site_coords(g, s, x);
+        T pl = T(0);
+        const int mu_lo = only_mu >= 0 ? only_mu : 0, mu_hi = only_mu >= 0 ? only_mu + 1 : 4;
+#pragma unroll 1
+        for (int mu = mu_lo; mu < mu_hi; ++mu) {
+            const int xpmu = nbr_fwd(g, s, x, mu);
+            const Mat3<T> umu = load_mat(u.u[mu], g.stride, s);
+            Mat3<T> acc = zero_mat<T>();
+#pragma unroll 1
+            for (int nu = 0; nu < 4; ++nu) {
+                if (nu == mu) continue;
+                const int xpnu = nbr_fwd(g, s, x, nu);
+                const int xmnu = nbr_bwd(g, s, x, nu);
+                // x - nu^ + mu^ : step forward in mu from xmnu (coordinates differ from x only in nu)
+                const int xmnupmu = xmnu + (xpmu - s);
+                {
+                    Mat3<T> t = mul_nn(load_mat(u.u[nu], g.stride, s), load_mat(u.u[mu], g.stride, xpnu));
+                    if (PLAQ && mu < nu) {
+                        Mat3<T> up = mul_na(t, load_mat(u.u[nu], g.stride, xpmu));
+                        pl += re_tr_na(umu, up);
+#pragma unroll
+                        for (int i = 0; i < 3; ++i)
+#pragma unroll
+                            for (int j = 0; j < 3; ++j) {
+                                acc.re[i][j] += up.re[i][j];
+                                acc.im[i][j] += up.im[i][j];
+                            }
+                    } else {
+                        mac_na(acc, t, load_mat(u.u[nu], g.stride, xpmu));
+                    }
+                }
+                {
+                    Mat3<T> t = mul_an(load_mat(u.u[nu], g.stride, xmnu), load_mat(u.u[mu], g.stride, xmnu));
+                    mac_nn(acc, t, load_mat(u.u[nu], g.stride, xmnupmu));
+                }
+            }
+            if (only_mu >= 0) {
+                store_mat(out.u[0], g.stride, s, acc);
+            } else {
+                Mat3<T> r;
+#pragma unroll
+                for (int i = 0; i < 3; ++i)
+#pragma unroll
+                    for (int j = 0; j < 3; ++j) {
+                        r.re[i][j] = fma(c1, acc.re[i][j], c0 * umu.re[i][j]);
+                        r.im[i][j] = fma(c1, acc.im[i][j], c0 * umu.im[i][j]);
+                    }
+                store_mat(out.u[mu], g.stride, s, r);
+            }
+        }
+        p[0] = (double)pl;
+    }
+    if (PLAQ) block_reduce_store<1>(p, partials, gridDim.x, blockIdx.x);
+}
+
+int check_links(lqx_ctx** ctx_out, const lqx_field* const u[4]) {
+    if (!u) return LQX_EINVAL;
+    lqx_ctx* ctx = nullptr;
+    for (int mu = 0; mu < 4; ++mu) {
+        if (!u[mu]) return LQX_EINVAL;
+        if (!ctx) ctx = u[mu]->ctx;
+        if (u[mu]->ctx != ctx) return lqx_fail(ctx, LQX_EGEOM, "links belong to different contexts");
+        if (u[mu]->kind != LQX_COLORMAT) return lqx_fail(ctx, LQX_ETYPE, "links must be colour matrices");
+        if (u[mu]->prec != u[0]->prec) return lqx_fail(ctx, LQX_ETYPE, "mixed precision links");
+    }
+    *ctx_out = ctx;
+    return LQX_OK;
+}
+
+template <typename T>
+Links<T> make_links(const lqx_field* const u[4]) {
+    Links<T> l;
+    for (int mu = 0; mu < 4; ++mu) l.u[mu] = (const T*)u[mu]->data;
+    return l;
+}
+
+template <typename T>
+int plaquette_launch(lqx_ctx* ctx, const lqx_field* const u[4], double* d_out) {
+    const Geo& g = ctx->geo;
+    const int grid = (g.V + 127) / 128;
+    int rc = lqx_ensure_partials(ctx, (size_t)grid);
+    if (rc) return rc;
+    k_plaquette<T><<<grid, 128, 0, ctx->stream>>>(g, make_links<T>(u), ctx->d_partials);
+    LQX_LAUNCH_CHECK(ctx);
+    return lqx_reduce_finish(ctx, grid, 1, d_out);
+}
+
+// one smear step on the stream; if d_plaq != nullptr the input plaquette sum lands there
+template <typename T>
+int smear_launch(lqx_ctx* ctx, lqx_field* const uout[4], const lqx_field* const uin[4], double alpha, int only_mu,
+                 double* d_plaq) {
+    const Geo& g = ctx->geo;
+    const int grid = (g.V + 127) / 128;
+    LinksOut<T> o;
+    for (int mu = 0; mu < 4; ++mu) o.u[mu] = uout[mu] ? (T*)uout[mu]->data : nullptr;
+    const T c0 = (T)(1.0 - alpha), c1 = (T)(alpha / 6.0);
+    if (d_plaq) {
+        int rc = lqx_ensure_partials(ctx, (size_t)grid);
+        if (rc) return rc;
+        k_smear_gather<T, true><<<grid, 128, 0, ctx->stream>>>(g, make_links<T>(uin), o, c0, c1, only_mu, ctx->d_partials);
+        LQX_LAUNCH_CHECK(ctx);
+        return lqx_reduce_finish(ctx, grid, 1, d_plaq);
+    }
+    k_smear_gather<T, false><<<grid, 128, 0, ctx->stream>>>(g, make_links<T>(uin), o, c0, c1, only_mu, nullptr);
+    LQX_LAUNCH_CHECK(ctx);
+    return LQX_OK;
+}
+
+int smear_dispatch(lqx_ctx* ctx, lqx_field* const uout[4], const lqx_field* const uin[4], double alpha, int only_mu,
+                   double* d_plaq) {
+    return uin[0]->prec == LQX_F32 ? smear_launch<float>(ctx, uout, uin, alpha, only_mu, d_plaq)
+                                   : smear_launch<double>(ctx, uout, uin, alpha, only_mu, d_plaq);
+}
+
+}  // namespace
+
+// =============================================================================================
+// C entry points
+// =============================================================================================
+static int hop_impl(lqx_field* chi, const lqx_field* const u[4], const lqx_field* psi, double* norm2_out) {
+    lqx_ctx* ctx;
+    int rc = check_links(&ctx, u);
+    if (rc) return rc;
+    if (!chi || !psi) return LQX_EINVAL;
+    if (chi->ctx != ctx || psi->ctx != ctx) return lqx_fail(ctx, LQX_EGEOM, "hop: different contexts");
+    if (chi->prec != u[0]->prec || psi->prec != u[0]->prec) return lqx_fail(ctx, LQX_ETYPE, "hop: mixed precision");
+    if (chi->kind != psi->kind || (psi->kind != LQX_FERMION && psi->kind != LQX_COLORVEC))
+        return lqx_fail(ctx, LQX_ETYPE, "hop: psi/chi must both be fermions or colour vectors");
+    if (lqx_same(chi, psi)) return lqx_fail(ctx, LQX_EALIAS, "hop: chi aliases psi");
+    LQX_CUDA(ctx, cudaSetDevice(ctx->device));
+    const Geo& g = ctx->geo;
+    const int grid = (g.V + 127) / 128;
+    const bool n2 = norm2_out != nullptr;
+    if (n2) {
+        rc = lqx_ensure_partials(ctx, (size_t)grid);
+        if (rc) return rc;
+    }
+    const bool ferm = psi->kind == LQX_FERMION;
+#define LQX_HOP(T, NSPIN, N2) \
+    k_hop<T, NSPIN, N2><<<grid, 128, 0, ctx->stream>>>(g, make_links<T>(u), (const T*)psi->data, (T*)chi->data, ctx->d_partials)
+    if (psi->prec == LQX_F32) {
+        if (ferm) { if (n2) LQX_HOP(float, 4, true); else LQX_HOP(float, 4, false); }
+        else      { if (n2) LQX_HOP(float, 1, true); else LQX_HOP(float, 1, false); }
+    } else {
+        if (ferm) { if (n2) LQX_HOP(double, 4, true); else LQX_HOP(double, 4, false); }
+        else      { if (n2) LQX_HOP(double, 1, true); else LQX_HOP(double, 1, false); }
+    }
+#undef LQX_HOP
+    LQX_LAUNCH_CHECK(ctx);
+    if (n2) {
+        rc = lqx_reduce_finish(ctx, grid, 1, ctx->d_result);
+        if (rc) return rc;
+        return lqx_fetch_result(ctx, 1, norm2_out);
+    }
+    return LQX_OK;
+}
+
+extern "C" int lqx_hop(lqx_field* chi, const lqx_field* const u[4], const lqx_field* psi) {
+    return hop_impl(chi, u, psi, nullptr);
+}
+extern "C" int lqx_hop_norm2(lqx_field* chi, const lqx_field* const u[4], const lqx_field* psi, double* norm2_out) {
+    if (!norm2_out) return LQX_EINVAL;
+    return hop_impl(chi, u, psi, norm2_out);
+}
+
+extern "C" int lqx_plaquette(const lqx_field* const u[4], double* plaq_sum, double* plaq_avg) {
+    lqx_ctx* ctx;
+    int rc = check_links(&ctx, u);
+    if (rc) return rc;
+    LQX_CUDA(ctx, cudaSetDevice(ctx->device));
+    rc = u[0]->prec == LQX_F32 ? plaquette_launch<float>(ctx, u, ctx->d_result) : plaquette_launch<double>(ctx, u, ctx->d_result);
+    if (rc) return rc;
+    double p;
+    rc = lqx_fetch_result(ctx, 1, &p);
+    if (rc) return rc;
+    if (plaq_sum) *plaq_sum = p;
+    if (plaq_avg) *plaq_avg = p / (18.0 * (double)ctx->geo.V);
+    return LQX_OK;
+}
+
+static int check_smear_args(lqx_ctx** ctx_out, lqx_field* const uout[4], const lqx_field* const uin[4]) {
+    lqx_ctx* ctx;
+    int rc = check_links(&ctx, uin);
+    if (rc) return rc;
+    rc = check_links(&ctx, (const lqx_field* const*)uout);
+    if (rc) return rc;
+    if (uout[0]->ctx != uin[0]->ctx) return lqx_fail(ctx, LQX_EGEOM, "smear: different contexts");
+    if (uout[0]->prec != uin[0]->prec) return lqx_fail(ctx, LQX_ETYPE, "smear: mixed precision");
+    for (int a = 0; a < 4; ++a)
+        for (int b = 0; b < 4; ++b) {
+            if (lqx_same(uout[a], uin[b])) return lqx_fail(ctx, LQX_EALIAS, "smear: output aliases an input link field");
+            if (a != b && lqx_same(uout[a], uout[b])) return lqx_fail(ctx, LQX_EALIAS, "smear: outputs alias each other");
+        }
+    *ctx_out = ctx;
+    return LQX_OK;
+}
+
+extern "C" int lqx_staple_sum(lqx_field* out, const lqx_field* const u[4], int mu) {
+    lqx_ctx* ctx;
+    int rc = check_links(&ctx, u);
+    if (rc) return rc;
+    if (!out) return LQX_EINVAL;
+    if (mu < 0 || mu > 3) return lqx_fail(ctx, LQX_EINVAL, "mu");
+    if (out->ctx != ctx) return lqx_fail(ctx, LQX_EGEOM, "staple_sum: different contexts");
+    if (out->kind != LQX_COLORMAT || out->prec != u[0]->prec) return lqx_fail(ctx, LQX_ETYPE, "staple_sum: output type");
+    for (int b = 0; b < 4; ++b)
+        if (lqx_same(out, u[b])) return lqx_fail(ctx, LQX_EALIAS, "staple_sum: output aliases a link field");
+    LQX_CUDA(ctx, cudaSetDevice(ctx->device));
+    lqx_field* o[4] = {out, nullptr, nullptr, nullptr};
+    return smear_dispatch(ctx, o, u, 0.0, mu, nullptr);
+}
+
+extern "C" int lqx_smear_step(lqx_field* const uout[4], const lqx_field* const uin[4], double alpha,
+                              double* plaq_in_or_null) {
+    if (!uout || !uin) return LQX_EINVAL;
+    lqx_ctx* ctx;
+    int rc = check_smear_args(&ctx, uout, uin);
+    if (rc) return rc;
+    LQX_CUDA(ctx, cudaSetDevice(ctx->device));
+    rc = smear_dispatch(ctx, uout, uin, alpha, -1, plaq_in_or_null ? ctx->d_result : nullptr);
+    if (rc) return rc;
+    if (plaq_in_or_null) return lqx_fetch_result(ctx, 1, plaq_in_or_null);
+    return LQX_OK;
+}
+
+extern "C" int lqx_smear_iterate(lqx_field* const u[4], lqx_field* const tmp[4], double alpha, int nsteps,
+                                 double* plaq_avg_after_each) {
+    if (!u || !tmp) return LQX_EINVAL;
+    lqx_ctx* ctx;
+    int rc = check_smear_args(&ctx, tmp, (const lqx_field* const*)u);
+    if (rc) return rc;
+    if (nsteps < 0) return lqx_fail(ctx, LQX_EINVAL, "nsteps < 0");
+    if (nsteps == 0) return LQX_OK;
+    LQX_CUDA(ctx, cudaSetDevice(ctx->device));
+    double* d_plaq = nullptr;
+    const bool want = plaq_avg_after_each != nullptr;
+    if (want) {
+        if (cudaMalloc(&d_plaq, (size_t)nsteps * sizeof(double)) != cudaSuccess) {
+            cudaGetLastError();
+            return lqx_fail(ctx, LQX_ENOMEM, "plaquette results");
+        }
+    }
+    // Ping-pong u -> tmp -> u ...  The plaquette of the field after step k is the plaquette of the
+    // INPUT of step k+1, which that step's kernel accumulates for free; only the last one needs its
+    // own pass.
+    lqx_field* const* src = u;
+    lqx_field* const* dst = tmp;
+    for (int k = 0; k < nsteps && rc == LQX_OK; ++k) {
+        double* dp = (want && k > 0) ? d_plaq + (k - 1) : nullptr;
+        rc = smear_dispatch(ctx, dst, (const lqx_field* const*)src, alpha, -1, dp);
+        std::swap(src, dst);
+    }
+    // result is in src now; if that is tmp (odd nsteps), copy back into u
+    if (rc == LQX_OK && src != u) {
+        for (int mu = 0; mu < 4 && rc == LQX_OK; ++mu) rc = lqx_copy(u[mu], tmp[mu]);
+    }
+    if (rc == LQX_OK && want) {
+        rc = u[0]->prec == LQX_F32 ? plaquette_launch<float>(ctx, (const lqx_field* const*)u, d_plaq + (nsteps - 1))
+                                   : plaquette_launch<double>(ctx, (const lqx_field* const*)u, d_plaq + (nsteps - 1));
+    }
+    if (rc == LQX_OK && want) {
+        std::vector<double> h((size_t)nsteps);
+        cudaError_t e = cudaMemcpyAsync(h.data(), d_plaq, (size_t)nsteps * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+        if (e != cudaSuccess) rc = lqx_cuda_fail(ctx, e, "smear_iterate results");
+        const double norm = 18.0 * (double)ctx->geo.V;
+        for (int k = 0; k < nsteps && rc == LQX_OK; ++k) plaq_avg_after_each[k] = h[k] / norm;
+    } else if (rc == LQX_OK) {
+        cudaError_t e = cudaStreamSynchronize(ctx->stream);
+        if (e != cudaSuccess) rc = lqx_cuda_fail(ctx, e, "smear_iterate sync");
+    }
+    if (d_plaq) cudaFree(d_plaq);
+    return rc;
+}
+
+extern "C" int lqx_smear_iterate_host(lqx_ctx* ctx, lqx_prec prec, const void* const host_u_in[4],
+                                      void* const host_u_out[4], double alpha, int nsteps,
+                                      double* plaq_avg_after_each) {
+    if (!ctx || !host_u_in || !host_u_out) return LQX_EINVAL;
+    for (int mu = 0; mu < 4; ++mu)
+        if (!host_u_in[mu] || !host_u_out[mu]) return LQX_EINVAL;
+    lqx_field* u[4] = {nullptr, nullptr, nullptr, nullptr};
+    lqx_field* t[4] = {nullptr, nullptr, nullptr, nullptr};
+    int rc = LQX_OK;
+    for (int mu = 0; mu < 4 && rc == LQX_OK; ++mu) {
+        rc = lqx_field_alloc(ctx, LQX_COLORMAT, prec, &u[mu]);
+        if (rc == LQX_OK) rc = lqx_field_alloc(ctx, LQX_COLORMAT, prec, &t[mu]);
+        if (rc == LQX_OK) rc = lqx_field_push(u[mu], host_u_in[mu]);
+    }
+    if (rc == LQX_OK) rc = lqx_smear_iterate(u, t, alpha, nsteps, plaq_avg_after_each);
+    for (int mu = 0; mu < 4 && rc == LQX_OK; ++mu) rc = lqx_field_pop(u[mu], host_u_out[mu]);
+    for (int mu = 0; mu < 4; ++mu) {
+        if (u[mu]) lqx_field_free(u[mu]);
+        if (t[mu]) lqx_field_free(t[mu]);
+    }
+    return rc;
+}

@@ -1,0 +1,353 @@
+"""GPU parity: the CUDA path (through the C-ABI, via the thin binding) against the CPU oracle,
+element by element on the same seeded inputs.  Index / copy work is bit-exact; floating point is
+compared with the DESIGN.md A14 site-normalised error against the WIDE-arithmetic oracle variant
+(t32 / t64), tolerance 1e-5 (fp32) and 1e-12 (fp64) as BASELINE.json north_star states; reductions
+1e-4 / 1e-10 with the A15 normalisation."""
+import numpy as np
+import pytest
+
+import lattice_inputs as li
+import oracle as orc
+from helpers import site_rel_err
+
+pytestmark = pytest.mark.gpu
+
+TOL = {"f32": 1e-5, "f64": 1e-12}
+RTOL = {"f32": 1e-4, "f64": 1e-10}
+# several tiles + a ragged tail (V = 1680, not a multiple of 32 or 128), odd extents, L0 % 4 != 0
+DIMS_RAGGED = (6, 5, 7, 8)
+DIMS_EVEN = (8, 4, 6, 4)
+ALL_DIMS = [(2, 2, 2, 2), (4, 4, 4, 4), DIMS_RAGGED, DIMS_EVEN, (3, 1, 2, 5)]
+
+
+@pytest.fixture(scope="module")
+def lqx():
+    import paper_1105_2279_b200 as m
+
+    return m
+
+
+def _prec(lqx, prec):
+    return {"f32": lqx.F32, "f64": lqx.F64}[prec]
+
+
+def _np(t):
+    return t.numpy()
+
+
+def _gauss(seed, fid, dims, kind, prec):
+    return _np(li.gaussian_field(seed, fid, dims, kind, prec))
+
+
+def _links(seed, dims, prec, recipe="haar"):
+    return [_np(t) for t in li.gauge_field(seed, dims, prec, recipe)]
+
+
+# ------------------------------------------------------------------------------------------------
+# a1 geometry
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dims", ALL_DIMS + [(16, 16, 16, 32)])
+def test_neighbor_tables_bit_exact(lqx, dims):
+    with lqx.Lattice(dims) as lat:
+        for mu in range(4):
+            for d in (+1, -1):
+                got = lat.neighbor_table(d, mu)
+                want = orc.neighbor_table(dims, d, mu)
+                assert np.array_equal(got, want), (dims, mu, d)
+
+
+# ------------------------------------------------------------------------------------------------
+# a2 field store
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dims", [DIMS_RAGGED, (4, 4, 4, 4)])
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+@pytest.mark.parametrize("kind", ["c", "cv", "cm", "f"])
+def test_push_pop_round_trip_bit_exact(lqx, dims, prec, kind):
+    a = _gauss(11, 0, dims, kind, prec)
+    with lqx.Lattice(dims) as lat:
+        f = lat.from_host(a)
+        assert np.array_equal(f.pop(), a)
+        g = lat.alloc(f.kind, f.prec, torch_memory=False)  # library-owned memory path
+        g.push(a)
+        assert np.array_equal(g.pop(), a)
+        lqx.copy(g, f)
+        assert np.array_equal(g.pop(), a)
+
+
+def test_internal_layout_is_site_fastest_soa(lqx):
+    import torch
+
+    dims = (4, 2, 2, 2)
+    a = _gauss(5, 0, dims, "cm", "f32")
+    with lqx.Lattice(dims) as lat:
+        f = lat.from_host(a)
+        torch.cuda.synchronize()
+        raw = f._mem.view(torch.float32).cpu().numpy().reshape(18, lat.stride)
+        assert lat.stride % 32 == 0 and lat.stride >= lat.volume
+        assert np.array_equal(raw[:, : lat.volume], a.reshape(lat.volume, 18).T)
+
+
+# ------------------------------------------------------------------------------------------------
+# a3 shift (bit-exact) and a5 form (iii)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dims", [DIMS_RAGGED, DIMS_EVEN, (2, 2, 2, 2)])
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+def test_shift_bit_exact_all_directions(lqx, dims, prec):
+    with lqx.Lattice(dims) as lat:
+        for kind in ("cm", "f", "c"):
+            a = _gauss(3, 1, dims, kind, prec)
+            fa = lat.from_host(a)
+            fr = lat.alloc(fa.kind, fa.prec)
+            for mu in range(4):
+                for d in (+1, -1):
+                    lqx.shift(fr, fa, d, mu)
+                    assert np.array_equal(fr.pop(), orc.shift(dims, a, d, mu)), (kind, mu, d)
+            # round trip
+            fb = lat.alloc(fa.kind, fa.prec)
+            lqx.shift(fr, fa, +1, 2)
+            lqx.shift(fb, fr, -1, 2)
+            assert np.array_equal(fb.pop(), a)
+
+
+@pytest.mark.parametrize("dims", [DIMS_RAGGED, DIMS_EVEN])
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+def test_form_iii_ax_minus_shift(lqx, dims, prec):
+    a, b = _gauss(7, 0, dims, "cm", prec), _gauss(7, 1, dims, "cm", prec)
+    with lqx.Lattice(dims) as lat:
+        fa, fb = lat.from_host(a), lat.from_host(b)
+        fr = lat.alloc(lqx.COLORMAT, _prec(lqx, prec))
+        for (d, mu) in [(-1, 2), (+1, 0), (-1, 0), (+1, 3), (-1, 1)]:
+            lqx.ax_minus_shift(fr, 2.5, fa, fb, d, mu)
+            got = fr.pop()
+            # same operations in the same precision: bit-exact against the native oracle
+            assert np.array_equal(got, orc.ax_minus_shift(dims, 2.5, a, b, d, mu, orc.native_variant(prec)))
+            assert site_rel_err(got, orc.ax_minus_shift(dims, 2.5, a, b, d, mu, orc.truth_variant(prec))) < TOL[prec]
+
+
+# ------------------------------------------------------------------------------------------------
+# a4 site-local catalogue
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dims", [DIMS_RAGGED, DIMS_EVEN])
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+def test_forms_i_ii_iv(lqx, dims, prec):
+    tv = orc.truth_variant(prec)
+    a, b, c, d = (_gauss(7, k, dims, "cm", prec) for k in range(4))
+    v = _gauss(7, 4, dims, "cv", prec)
+    psi = _gauss(7, 5, dims, "f", prec)
+    with lqx.Lattice(dims) as lat:
+        fa, fb, fc, fd, fv, fp = (lat.from_host(t) for t in (a, b, c, d, v, psi))
+        r = lat.alloc(lqx.COLORMAT, fa.prec)
+        lqx.mm_plus_madj(r, fa, fb, fc, fd)
+        assert site_rel_err(r.pop(), orc.mm_plus_madj(dims, a, b, c, d, tv)) < TOL[prec]
+        t = lat.alloc(lqx.COMPLEX, fa.prec)
+        lqx.trace_mm(t, fa, fb)
+        assert site_rel_err(t.pop(), orc.trace_mm(dims, a, b, tv)) < TOL[prec] * 4  # 9-term sum vs its own size
+        w = lat.alloc(lqx.COLORVEC, fa.prec)
+        lqx.mat_vec(w, fa, fv)
+        assert site_rel_err(w.pop(), orc.mat_vec(dims, a, v, tv)) < TOL[prec]
+        wf = lat.alloc(lqx.FERMION, fa.prec)
+        lqx.mat_vec(wf, fa, fp)
+        assert site_rel_err(wf.pop(), orc.mat_vec(dims, a, psi, tv)) < TOL[prec]
+        # in-place site-local evaluation is allowed (reading A21)
+        lqx.mm_plus_madj(fa, fa, fb, fc, fd)
+        assert site_rel_err(fa.pop(), orc.mm_plus_madj(dims, a, b, c, d, tv)) < TOL[prec]
+
+
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+def test_axpy_scale_divide(lqx, prec):
+    dims = DIMS_RAGGED
+    tv = orc.truth_variant(prec)
+    s0, h = _gauss(9, 0, dims, "f", prec), _gauss(9, 1, dims, "f", prec)
+    with lqx.Lattice(dims) as lat:
+        f0, fh = lat.from_host(s0), lat.from_host(h)
+        r = lat.alloc(lqx.FERMION, f0.prec)
+        lqx.axpy(r, f0, 0.37, fh)
+        assert site_rel_err(r.pop(), orc.axpy(dims, s0, 0.37, h, tv)) < TOL[prec]
+        lqx.scale(r, -1.75, f0)
+        assert np.array_equal(r.pop(), orc.scale(dims, -1.75, s0, orc.native_variant(prec)))
+        lqx.divide(r, f0, 3.3)
+        assert site_rel_err(r.pop(), orc.divide(dims, 3.3, s0, tv)) < TOL[prec]
+
+
+# ------------------------------------------------------------------------------------------------
+# a9 reductions
+# ------------------------------------------------------------------------------------------------
+def _red_err(got, want, scale):
+    got, want = np.asarray(got, dtype=np.float64), np.asarray(want, dtype=np.float64)
+    return float(np.abs(got - want).max() / max(np.abs(want).max(), scale))
+
+
+@pytest.mark.parametrize("dims", [DIMS_RAGGED, (16, 8, 8, 8)])
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+def test_reductions(lqx, dims, prec):
+    tv = orc.truth_variant(prec)
+    with lqx.Lattice(dims) as lat:
+        for kind in ("c", "cv", "cm", "f"):
+            a = _gauss(13, 2, dims, kind, prec)
+            f = lat.from_host(a)
+            rms = float(np.sqrt((a.astype(np.float64) ** 2).sum()))  # A15: sqrt(sum term^2)
+            assert _red_err(lqx.sum(f), orc.sum_field(dims, a, tv), rms) < RTOL[prec]
+            n2 = lqx.norm2(f)
+            assert abs(n2 - orc.norm2(dims, a, tv)) / orc.norm2(dims, a, tv) < RTOL[prec]
+            if kind == "cm":
+                assert _red_err(lqx.trace(f), orc.trace(dims, a, tv), rms) < RTOL[prec]
+            # deterministic: same bits on a second call
+            assert lqx.norm2(f) == n2
+
+
+# ------------------------------------------------------------------------------------------------
+# a6 hop
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dims", [DIMS_RAGGED, DIMS_EVEN, (2, 2, 2, 2)])
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+def test_hop(lqx, dims, prec):
+    tv = orc.truth_variant(prec)
+    u = _links(2, dims, prec)
+    with lqx.Lattice(dims) as lat:
+        fu = [lat.from_host(t) for t in u]
+        for kind in ("f", "cv"):
+            psi = _gauss(2, 10, dims, kind, prec)
+            fp = lat.from_host(psi)
+            chi = lat.alloc(fp.kind, fp.prec)
+            want = orc.hop(dims, u, psi, tv)
+            lqx.hop(chi, fu, fp)
+            assert site_rel_err(chi.pop(), want) < TOL[prec]
+            n2 = lqx.hop_norm2(chi, fu, fp)
+            assert site_rel_err(chi.pop(), want) < TOL[prec]
+            want_n2 = float((want.astype(np.float64) ** 2).sum())
+            assert abs(n2 - want_n2) / want_n2 < RTOL[prec]
+            assert abs(n2 - lqx.norm2(chi)) / want_n2 < 1e-13  # fused == two-call up to summation order
+
+
+def test_c2_hop_full_size(lqx):
+    """BASELINE.json configs[1]: 16^3x32 fp32, Haar links, Gaussian fermion; hop then norm2."""
+    cfg = li.CONFIGS["c2"]
+    dims = cfg["dims"]
+    u = _links(cfg["seed"], dims, "f32")
+    psi = _gauss(cfg["seed"], 10, dims, "f", "f32")
+    want = orc.hop(dims, u, psi, "t32")
+    with lqx.Lattice(dims) as lat:
+        fu = [lat.from_host(t) for t in u]
+        fp = lat.from_host(psi)
+        chi = lat.alloc(lqx.FERMION, lqx.F32)
+        n2 = lqx.hop_norm2(chi, fu, fp)
+        got = chi.pop()
+    assert site_rel_err(got, want) < TOL["f32"]
+    want_n2 = float((want ** 2).sum())
+    assert abs(n2 - want_n2) / want_n2 < RTOL["f32"]
+
+
+# ------------------------------------------------------------------------------------------------
+# a7 / a8 / a10 staple, smear, plaquette
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), DIMS_RAGGED, DIMS_EVEN, (2, 2, 2, 2), (3, 1, 2, 5)])
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+def test_staple_smear_plaquette(lqx, dims, prec):
+    tv = orc.truth_variant(prec)
+    u = _links(1, dims, prec)
+    with lqx.Lattice(dims) as lat:
+        fu = [lat.from_host(t) for t in u]
+        out = [lat.alloc(lqx.COLORMAT, fu[0].prec) for _ in range(4)]
+        st = lat.alloc(lqx.COLORMAT, fu[0].prec)
+        for mu in range(4):
+            lqx.staple_sum(st, fu, mu)
+            assert site_rel_err(st.pop(), orc.staple_sum(dims, u, mu, tv)) < TOL[prec]
+        want = orc.smear_step(dims, u, 0.5, tv)
+        psum_want = orc.plaquette_sum(dims, u, tv)
+        scale = np.sqrt(18.0 * lat.volume)  # A15: size of a zero-mean Haar plaquette sum
+        for want_plaq in (False, True):
+            for o in out:
+                lqx.scale(o, 0.0, o)
+            p = lqx.smear_step(out, fu, 0.5, want_plaq_in=want_plaq)
+            for mu in range(4):
+                assert site_rel_err(out[mu].pop(), want[mu]) < TOL[prec], (mu, want_plaq)
+            if want_plaq:
+                assert abs(p - psum_want) / max(abs(psum_want), scale) < RTOL[prec]
+        ps, pa = lqx.plaquette(fu)
+        assert abs(ps - psum_want) / max(abs(psum_want), scale) < RTOL[prec]
+        assert abs(pa - psum_want / (18.0 * lat.volume)) < RTOL[prec]
+        # plaquette of the smeared field (A11)
+        ps2, _ = lqx.plaquette(out)
+        w2 = orc.plaquette_sum(dims, want, "t64" if prec == "f64" else "n64")
+        assert abs(ps2 - w2) / max(abs(w2), scale) < RTOL[prec]
+
+
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+def test_unit_gauge_is_a_fixed_point(lqx, prec):
+    dims = DIMS_EVEN
+    u = _links(0, dims, prec, "unit")
+    with lqx.Lattice(dims) as lat:
+        fu = [lat.from_host(t) for t in u]
+        st = lat.alloc(lqx.COLORMAT, fu[0].prec)
+        lqx.staple_sum(st, fu, 1)
+        six = 6.0 * u[0]
+        assert np.array_equal(st.pop(), six)  # every staple is the identity: S = 6*1 exactly
+        out = [lat.alloc(lqx.COLORMAT, fu[0].prec) for _ in range(4)]
+        p = lqx.smear_step(out, fu, 0.5, want_plaq_in=True)
+        for mu in range(4):
+            assert np.abs(out[mu].pop() - u[mu]).max() < (1e-7 if prec == "f32" else 1e-15)
+        assert p == 18.0 * lat.volume
+        assert lqx.plaquette(fu)[1] == 1.0
+
+
+@pytest.mark.parametrize("prec,nsteps", [("f32", 4), ("f64", 3), ("f32", 1)])
+def test_smear_iterate_trajectory(lqx, prec, nsteps):
+    """configs[3] in miniature: near-unit links, iterated steps, plaquette after each (A23)."""
+    dims = (8, 6, 4, 6)
+    u = _links(4, dims, prec, "near_unit")
+    want_u, want_p = orc.smear_iterate(dims, u, 0.5, nsteps, prec)
+    with lqx.Lattice(dims) as lat:
+        fu = [lat.from_host(t) for t in u]
+        tmp = [lat.alloc(lqx.COLORMAT, fu[0].prec) for _ in range(4)]
+        plaqs = lqx.smear_iterate(fu, tmp, 0.5, nsteps)
+        for k in range(nsteps):
+            assert abs(plaqs[k] - want_p[k]) < RTOL[prec], k
+        for mu in range(4):
+            assert site_rel_err(fu[mu].pop(), want_u[mu]) < TOL[prec] * nsteps
+        # plaquette rises monotonically towards 1 under smearing of a smooth field
+        assert all(plaqs[k + 1] > plaqs[k] for k in range(nsteps - 1)) and plaqs[-1] < 1.0
+
+
+def test_smear_iterate_host_end_to_end(lqx):
+    dims = (4, 4, 4, 8)
+    u = _links(4, dims, "f32", "near_unit")
+    want_u, want_p = orc.smear_iterate(dims, u, 0.5, 2, "f32")
+    out = [np.empty_like(t) for t in u]
+    with lqx.Lattice(dims) as lat:
+        plaqs = lqx.smear_iterate_host(lat, lqx.F32, u, out, 0.5, 2)
+    for k in range(2):
+        assert abs(plaqs[k] - want_p[k]) < RTOL["f32"]
+    for mu in range(4):
+        assert site_rel_err(out[mu], want_u[mu]) < 2 * TOL["f32"]
+
+
+# ------------------------------------------------------------------------------------------------
+# error behaviour of the boundary
+# ------------------------------------------------------------------------------------------------
+def test_error_codes(lqx):
+    dims = (4, 4, 4, 4)
+    with lqx.Lattice(dims) as lat, lqx.Lattice((4, 4, 4, 2)) as lat2:
+        a32 = lat.alloc(lqx.COLORMAT, lqx.F32)
+        b32 = lat.alloc(lqx.COLORMAT, lqx.F32)
+        a64 = lat.alloc(lqx.COLORMAT, lqx.F64)
+        v32 = lat.alloc(lqx.COLORVEC, lqx.F32)
+        other = lat2.alloc(lqx.COLORMAT, lqx.F32)
+
+        def code(fn, *args):
+            with pytest.raises(lqx.LqxError) as e:
+                fn(*args)
+            return e.value.code
+
+        assert code(lqx.shift, a32, a32, +1, 0) == -4            # EALIAS
+        assert code(lqx.shift, a32, b32, +1, 4) == -1            # EINVAL mu
+        assert code(lqx.shift, a32, b32, 0, 1) == -1             # EINVAL dir
+        assert code(lqx.shift, a32, a64, +1, 0) == -2            # ETYPE precision
+        assert code(lqx.shift, a32, v32, +1, 0) == -2            # ETYPE kind
+        assert code(lqx.shift, a32, other, +1, 0) == -3          # EGEOM
+        assert code(lqx.ax_minus_shift, a32, 2.5, b32, a32, -1, 2) == -4
+        assert code(lqx.mat_vec, v32, v32, v32) == -2
+        u = [a32, b32, lat.alloc(lqx.COLORMAT, lqx.F32), lat.alloc(lqx.COLORMAT, lqx.F32)]
+        assert code(lqx.smear_step, u, u, 0.5) == -4
+        assert code(lqx.hop, v32, u, v32) == -4
+        with pytest.raises(lqx.LqxError):
+            lqx.Lattice((4, 0, 4, 4))
