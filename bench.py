@@ -1,0 +1,453 @@
+"""bench.py -- smear-step throughput of the lqx library on N B200s (one process per GPU).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c4|c3] [--no-extras]
+    python bench.py --impl reference ...        # the CPU oracle on a bounded sample of the same workload
+
+One "step" = one pass of the whole hot path over the link field: a fused staple-sum smearing step
+(alpha = 0.5, all four directions, plaquette of its input accumulated in the same pass) -- K steps
+are iterated on ping-pong buffers and the plaquette after the last step gets its own pass, exactly
+what lqx_smear_iterate does (BASELINE.json configs[3]: 48^3x96, fp32, near-unit SU(3), plaquette
+after each step).  Prints ONE JSON line (rank 0).  The path does not shard (replicas
+only): with N > 1 every rank runs an independent replica, value = N * V * K / max-over-ranks time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+ALPHA = 0.5
+# per site-update -- algorithmic bytes (read 72 + write 72 reals), canonical
+# flops of the literal 48-product evaluation, and FMA lane-ops the kernel variants execute
+SMEAR_REALS_PER_SITE = 144
+SMEAR_CANONICAL_FLOPS = 10080
+SMEAR_LANE_OPS = {"literal": 5328, "shared": 4032}
+PLAQ_REALS_PER_SITE = 72
+WORKLOADS = {
+    "c4": dict(cfg="c4", recipe="near_unit", desc="BASELINE configs[3]: 48^3x96 fp32 near-unit SU(3) (exp(0.1iH) reunitarised), "
+               "iterated smear steps a=0.5, plaquette after each"),
+    "c3": dict(cfg="c3", recipe="haar", desc="BASELINE configs[2]: 32^3x64 fp64 Haar SU(3), smear steps a=0.5 + plaquette"),
+}
+
+
+def _peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            p = json.load(f)
+        return float(p["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)", float(p.get("sm_max_mhz", 1965.0))
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)", 1965.0
+
+
+class ClockSampler(threading.Thread):
+    """Polls SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index: int, period_s: float = 0.004):
+        super().__init__(daemon=True)
+        self.index, self.period = index, period_s
+        self.samples, self.reasons = [], set()
+        self.max_mhz = None
+        self._stop_evt = threading.Event()
+        try:
+            import pynvml
+
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self.nv = None
+
+    def run(self):
+        if self.nv is None:
+            return
+        nv = self.nv
+        names = {
+            getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8): "hw_slowdown",
+            getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4): "sw_power_cap",
+        }
+        while not self._stop_evt.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                try:
+                    r = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                except Exception:
+                    r = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                for bit, name in names.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def stop(self):
+        self._stop_evt.set()
+        self.join(timeout=2.0)
+        s = sorted(self.samples)
+        return {"sm_mhz": (s[len(s) // 2] if s else None), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(s)}
+
+
+def _dist():
+    """(rank, world, local_rank, barrier_fn, max_fn) -- torch.distributed only when launched by torchrun."""
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if world <= 1:
+        return 0, 1, 0, (lambda: None), (lambda x: x)
+    import torch
+    import torch.distributed as dist
+
+    rank, local = int(os.environ["RANK"]), int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dist.init_process_group(backend="nccl", device_id=torch.device(f"cuda:{local}"))
+
+    def vmax(x):
+        t = torch.tensor([float(x)], dtype=torch.float64, device=f"cuda:{local}")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    return rank, world, local, dist.barrier, vmax
+
+
+def _gen_links(lat, lqx, li, cfgname, recipe, prec, keep_host=False):
+    """Seeded synthetic link field generated with torch on the GPU (input generator only), converted
+    AoS -> SoA by the library.  Returns (fields, pinned host copies or None)."""
+    import torch
+
+    cfg = li.CONFIGS[cfgname]
+    dev = f"cuda:{lat.device}"
+    fields, host = [], []
+    v = lat.volume
+    for mu in range(4):
+        if recipe == "haar":
+            z = li.haar_su3_complex(cfg["seed"], mu, v, dev)
+        else:
+            z = li.near_unit_su3_complex(cfg["seed"], mu, v, 0.1, dev)
+        a = li._as_real(z, prec)
+        del z
+        f = lat.alloc(lqx.COLORMAT, lqx.F32 if prec == "f32" else lqx.F64)
+        f.import_dev(a)
+        torch.cuda.synchronize()
+        if keep_host:
+            h = torch.empty(a.shape, dtype=a.dtype, pin_memory=True)
+            h.copy_(a)
+            host.append(h)
+        del a
+        fields.append(f)
+    torch.cuda.empty_cache()
+    return fields, (host if keep_host else None)
+
+
+def _cpu_baseline(orc, dims, prec, host_links, target_s=12.0):
+    """The oracle as it stands (native-precision instantiation, OpenMP over its site loop) on a bounded
+    sample of the same workload: smear_links for all four directions + the plaquette integrand on the
+    first n sites of the full-size host field."""
+    import numpy as np
+
+    variant = orc.native_variant(prec)
+    u = [h.numpy() if hasattr(h, "numpy") else h for h in host_links]
+    v = u[0].shape[0]
+
+    def run(nsites):
+        sites = np.repeat(np.arange(nsites, dtype=np.int64), 4)
+        mus = np.tile(np.arange(4, dtype=np.int32), nsites)
+        t0 = time.perf_counter()
+        orc.smear_links(dims, u, ALPHA, sites, mus, variant)
+        orc.plaquette_sites(dims, u, np.arange(nsites, dtype=np.int64), variant)
+        return time.perf_counter() - t0
+
+    n0 = min(v, 20000)
+    run(min(v, 2000))  # page in / spin up the thread pool
+    t = run(n0)
+    n = int(min(v, max(n0, n0 * target_s / max(t, 1e-6))))
+    t = run(n)
+    return {"value": n / t, "unit": "site-updates/s", "cores": orc.num_threads(), "kind": "oracle",
+            "sample": f"first {n} of {v} sites of the full-size field (all 4 directions + plaquette), "
+                      f"oracle variant {variant}, {t:.1f} s"}
+
+
+def _time_kernel(torch, fn, reps, flush=None):
+    """Median and best device time (ms) of fn() over reps launches, CUDA events on the current stream."""
+    times = []
+    for _ in range(reps):
+        if flush is not None:
+            flush.add_(1)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        fn()
+        e1.record()
+        e1.synchronize()
+        times.append(e0.elapsed_time(e1))
+    times.sort()
+    return times[len(times) // 2], times[0]
+
+
+def _extras(torch, lqx, li, hbm_gbs):
+    """Per-kernel numbers for the other BASELINE configs (same JSON line, key "kernels"): device time
+    per launch, algorithmic GB/s (SURVEY 8(d) bytes/site) and its fraction of the measured HBM peak."""
+    out = []
+    flush = torch.zeros(64 * 1024 * 1024, dtype=torch.float32, device="cuda")  # 256 MB > L2
+
+    def add(name, prec, sites, reals_per_site, flops_per_site, fn, reps=10, cold=False):
+        for _ in range(3):
+            fn()
+        torch.cuda.synchronize()
+        med, best = _time_kernel(torch, fn, reps, flush if cold else None)
+        nbytes = sites * reals_per_site * (4 if prec == "f32" else 8)
+        out.append({"kernel": name, "dtype": prec, "ms": round(med, 5), "ms_best": round(best, 5),
+                    "site_evals_per_s": sites / (med * 1e-3), "alg_gbs": nbytes / (med * 1e-3) / 1e9,
+                    "hbm_frac": nbytes / (med * 1e-3) / 1e9 / hbm_gbs, "gflops": sites * flops_per_site / (med * 1e-3) / 1e9,
+                    "l2": "flushed between launches" if cold else "inputs larger than L2"})
+
+    # ---- C2: hop, 16^3x32 fp32 (working set 63 MB < L2: cold and warm)
+    dims = li.CONFIGS["c2"]["dims"]
+    with lqx.Lattice(dims) as lat:
+        u, _ = _gen_links(lat, lqx, li, "c2", "haar", "f32")
+        psi = lat.alloc(lqx.FERMION, lqx.F32).import_dev(li.gaussian_field(2, 10, dims, "f", "f32", device="cuda"))
+        chi = lat.alloc(lqx.FERMION, lqx.F32)
+        v = lat.volume
+        add("hop c2 (L2-cold)", "f32", v, 120, 2280, lambda: lqx.hop(chi, u, psi), reps=20, cold=True)
+        out[-1]["l2"] = "flushed between launches"
+        add("hop c2 (L2-warm)", "f32", v, 120, 2280, lambda: lqx.hop(chi, u, psi), reps=20)
+        out[-1]["l2"] = "warm: 63 MB working set fits the 126 MB L2"
+        add("hop+norm2 fused c2 (L2-cold, incl. sync)", "f32", v, 120, 2328, lambda: lqx.hop_norm2(chi, u, psi), reps=20, cold=True)
+    # ---- C3: smear + plaquette, 32^3x64 fp64
+    dims = li.CONFIGS["c3"]["dims"]
+    with lqx.Lattice(dims) as lat:
+        u, _ = _gen_links(lat, lqx, li, "c3", "haar", "f64")
+        o = [lat.alloc(lqx.COLORMAT, lqx.F64) for _ in range(4)]
+        v = lat.volume
+        add("smear_step c3", "f64", v, 144, SMEAR_CANONICAL_FLOPS, lambda: lqx.smear_step(o, u, ALPHA), reps=6)
+        add("smear_step+plaquette(in) fused c3 (incl. sync)", "f64", v, 144, SMEAR_CANONICAL_FLOPS + 108,
+            lambda: lqx.smear_step(o, u, ALPHA, want_plaq_in=True), reps=6)
+        add("plaquette c3 (incl. sync)", "f64", v, 72, 2591, lambda: lqx.plaquette(u), reps=6)
+    # ---- C5: catalogue sweep, 32^3x64, both precisions
+    dims = li.CONFIGS["c5"]["dims"]
+    for prec, pcode in (("f32", lqx.F32), ("f64", lqx.F64)):
+        with lqx.Lattice(dims) as lat:
+            v = lat.volume
+            cm = [lat.alloc(lqx.COLORMAT, pcode).import_dev(li.gaussian_field(7, k, dims, "cm", prec, device="cuda")) for k in range(4)]
+            vec = lat.alloc(lqx.COLORVEC, pcode).import_dev(li.gaussian_field(7, 4, dims, "cv", prec, device="cuda"))
+            r = lat.alloc(lqx.COLORMAT, pcode)
+            c = lat.alloc(lqx.COMPLEX, pcode)
+            w = lat.alloc(lqx.COLORVEC, pcode)
+            torch.cuda.synchronize()
+            add("form i  A*B+C*adj(D) c5", prec, v, 90, 414, lambda: lqx.mm_plus_madj(r, cm[0], cm[1], cm[2], cm[3]))
+            add("form ii trace(A*B) c5", prec, v, 38, 70, lambda: lqx.trace_mm(c, cm[0], cm[1]))
+            add("form iii 2.5*A-shift(B,BACKWARD,2) c5", prec, v, 54, 36, lambda: lqx.ax_minus_shift(r, 2.5, cm[0], cm[1], lqx.BACKWARD, 2))
+            add("form iii' 2.5*A-shift(B,FORWARD,0) c5", prec, v, 54, 36, lambda: lqx.ax_minus_shift(r, 2.5, cm[0], cm[1], lqx.FORWARD, 0))
+            add("form iv M*v c5", prec, v, 30, 66, lambda: lqx.mat_vec(w, cm[0], vec))
+            add("shift(A,FORWARD,3) c5", prec, v, 36, 0, lambda: lqx.shift(r, cm[0], lqx.FORWARD, 3))
+            add("norm2(colour matrix) c5 (incl. sync)", prec, v, 18, 36, lambda: lqx.norm2(cm[0]))
+            add("sum(colour matrix) c5 (incl. sync)", prec, v, 18, 18, lambda: lqx.sum(cm[0]))
+            add("trace(colour matrix) c5 (incl. sync)", prec, v, 6, 6, lambda: lqx.trace(cm[0]))
+    del flush
+    torch.cuda.empty_cache()
+    return out
+
+
+def run_ours(args):
+    import torch
+
+    import lattice_inputs as li
+    import paper_1105_2279_b200 as lqx
+
+    rank, world, local, barrier, vmax = _dist()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the lqx library has no CPU fallback")
+    torch.cuda.set_device(local)
+    wl = WORKLOADS[args.workload]
+    cfg = li.CONFIGS[wl["cfg"]]
+    dims, prec = cfg["dims"], cfg["prec"]
+    esize = 4 if prec == "f32" else 8
+    K, W = args.steps, max(args.warmup, 3)
+    hbm_gbs, hbm_src, sm_max = _peaks()
+    want_host = (world == 1)  # e2e and cpu_baseline need the host copy
+
+    lat = lqx.Lattice(dims, device=local)
+    V = lat.volume
+    u, host = _gen_links(lat, lqx, li, wl["cfg"], wl["recipe"], prec, keep_host=want_host)
+    tmp = [lat.alloc(lqx.COLORMAT, u[0].prec) for _ in range(4)]
+
+    # roofline denominators measured in this run (reported beside the driver-written peak)
+    fma_kind = 0 if prec == "f32" else 2
+    fma_peak = lat.bench_fma_peak(fma_kind)
+    fma2_peak = lat.bench_fma_peak(1) if prec == "f32" else None
+    copy_peak = lat.bench_copy_peak(1 << 30)
+
+    lqx.smear_iterate(u, tmp, ALPHA, W)  # warm-up (>= 3 steps)
+    torch.cuda.synchronize()
+    lat.set_option("time_kernels", 1)
+    lat.kernel_time(lqx.K_SMEAR), lat.kernel_time(lqx.K_PLAQUETTE)
+    sampler = ClockSampler(local)
+    barrier()
+    torch.cuda.synchronize()
+    launches0 = lat.launch_count()
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    plaqs = lqx.smear_iterate(u, tmp, ALPHA, K)  # K steps, plaquette after each; syncs once at the end
+    e1.record()
+    torch.cuda.synchronize()
+    barrier()
+    clocks = sampler.stop()
+    ms = vmax(e0.elapsed_time(e1))
+    launches = lat.launch_count() - launches0
+    smear_ms, smear_n = lat.kernel_time(lqx.K_SMEAR)
+    plaq_ms, plaq_n = lat.kernel_time(lqx.K_PLAQUETTE)
+    lat.set_option("time_kernels", 0)
+
+    value = world * V * K / (ms * 1e-3)
+    k_ms = smear_ms / max(smear_n, 1)  # average duration of the dominant kernel inside the timed region
+    alg_bytes = V * SMEAR_REALS_PER_SITE * esize
+    variant = "literal"
+    lane_ops = V * SMEAR_LANE_OPS[variant]
+    # FP-pipe peak from unit counts and clocks: 148 SMs x 128 fp32 (64 fp64) FMA lanes x sm_max
+    alu_peak_tflops = 148 * (128 if prec == "f32" else 64) * 2 * sm_max * 1e6 / 1e12
+    roofline = {
+        "kernel": "k_smear (staple sum + smear update, fused input plaquette)",
+        "bound": "alu", "achieved": 2 * lane_ops / (k_ms * 1e-3) / 1e12, "peak": alu_peak_tflops, "unit": "TFLOP/s",
+        "frac": 2 * lane_ops / (k_ms * 1e-3) / 1e12 / alu_peak_tflops,
+        "peak_source": f"148 SMs x {128 if prec == 'f32' else 64} FMA lanes x 2 x {sm_max:.0f} MHz (DESIGN.md sec.7); "
+                       f"FMA-chain micro-benchmark in this run: {2 * fma_peak / 1e12:.1f} TFLOP/s"
+                       + (f", packed f32x2: {2 * fma2_peak / 1e12:.1f}" if fma2_peak else ""),
+        "flops_counted": f"executed FMA lane-ops x 2 ({SMEAR_LANE_OPS[variant]} lane-ops/site, {variant} evaluation)",
+        "traffic": None, "ms_per_launch": k_ms, "launches": smear_n,
+        "hbm": {"bound": "hbm", "achieved": alg_bytes / (k_ms * 1e-3) / 1e9, "peak": hbm_gbs, "unit": "GB/s",
+                "frac": alg_bytes / (k_ms * 1e-3) / 1e9 / hbm_gbs, "peak_source": hbm_src,
+                "copy_kernel_this_run_gbs": copy_peak / 1e9, "alg_bytes_per_launch": alg_bytes},
+    }
+    line = {
+        "metric": "smear-step site-updates/s", "value": value, "unit": "site-updates/s", "n_gpus": world,
+        "steps": K, "warmup": W, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": prec, "data": "synthetic",
+        "config": {"workload": wl["desc"], "dims": list(dims), "sites": V, "alpha": ALPHA, "l2": "inputs larger than L2 "
+                   f"({2 * alg_bytes / 2 / 1e9:.2f} GB read+written per step)", "parallelism": "replicas only" if world > 1 else "1 GPU",
+                   "smear_variant": variant},
+        "gflops_canonical": world * V * K * SMEAR_CANONICAL_FLOPS / (ms * 1e-3) / 1e9,
+        "hbm_gbs_algorithmic": world * (K * alg_bytes + V * PLAQ_REALS_PER_SITE * esize) / (ms * 1e-3) / 1e9,
+        "plaquette_avg_after_each_step": plaqs,
+        "clocks": clocks, "gpu_launches": launches, "roofline": roofline,
+        "step_breakdown_ms": {"smear_kernels": smear_ms, "plaquette_kernel": plaq_ms, "smear_launches": smear_n,
+                              "plaquette_launches": plaq_n, "timed_region": ms},
+    }
+
+    if world == 1:
+        # ---- e2e: the public host-buffer call, H2D + D2H inside the timed region, every step
+        hin = host
+        hout = [torch.empty(h.shape, dtype=h.dtype, pin_memory=True) for h in host]
+        lqx.smear_iterate_host(lat, u[0].prec, hin, hout, ALPHA, 1)  # warm-up
+        torch.cuda.synchronize()
+        ke = min(K, args.e2e_steps)
+        t0 = time.perf_counter()
+        for _ in range(ke):
+            lqx.smear_iterate_host(lat, u[0].prec, hin, hout, ALPHA, 1)
+            hin, hout = hout, hin
+        torch.cuda.synchronize()
+        te = time.perf_counter() - t0
+        fbytes = V * 18 * esize * 4
+        line["e2e"] = {"value": V * ke / te, "unit": "site-updates/s", "h2d_bytes_per_step": fbytes,
+                       "d2h_bytes_per_step": fbytes + 8, "steps": ke, "ms_per_step": te / ke * 1e3,
+                       "call": "lqx_smear_iterate_host(nsteps=1) on pinned host buffers in QDP order"}
+        # ---- cpu baseline: the oracle on this box's host cores
+        import oracle as orc
+
+        line["cpu_baseline"] = _cpu_baseline(orc, dims, prec, host)
+        del hout, hin
+    else:
+        line["e2e"] = None
+    for f in u + tmp:
+        f.free()
+    lat.close()
+    torch.cuda.empty_cache()
+    if world == 1 and not args.no_extras:
+        line["kernels"] = _extras(torch, lqx, li, hbm_gbs)
+    if rank == 0:
+        print(json.dumps(line))
+    if world > 1:
+        import torch.distributed as dist
+
+        dist.destroy_process_group()
+
+
+def run_reference(args):
+    """The oracle, as it stands, on this box's host cores: each step = one bounded sample of the workload
+    (smear update of all four links + plaquette integrand on the first n sites of the full-size field)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import numpy as np
+
+    import lattice_inputs as li
+    import oracle as orc
+
+    wl = WORKLOADS[args.workload]
+    cfg = li.CONFIGS[wl["cfg"]]
+    dims, prec = cfg["dims"], cfg["prec"]
+    V = li.volume(dims)
+    # the sample only touches sites within one time-slice of its range, but the oracle indexes the full
+    # lattice: generate the whole field (on the GPU if there is one -- input generation only)
+    try:
+        import torch
+
+        dev = "cuda" if torch.cuda.is_available() else "cpu"
+    except Exception:
+        dev = "cpu"
+    u = [t.cpu().numpy() for t in li.gauge_field(cfg["seed"], dims, prec, wl["recipe"], device=dev)]
+    variant = orc.native_variant(prec)
+    n = min(V, args.ref_sites)
+    sites = np.repeat(np.arange(n, dtype=np.int64), 4)
+    mus = np.tile(np.arange(4, dtype=np.int32), n)
+    only = np.arange(n, dtype=np.int64)
+
+    def step():
+        orc.smear_links(dims, u, ALPHA, sites, mus, variant)
+        orc.plaquette_sites(dims, u, only, variant)
+
+    K, W = args.steps, args.warmup
+    for _ in range(W):
+        step()
+    t0 = time.perf_counter()
+    for _ in range(K):
+        step()
+    t = time.perf_counter() - t0
+    value = n * K / t
+    sample = f"each step: first {n} of {V} sites (all 4 directions + plaquette), oracle variant {variant}"
+    print(json.dumps({
+        "impl": "reference", "metric": "smear-step site-updates/s", "value": value, "unit": "site-updates/s",
+        "n_gpus": int(os.environ.get("WORLD_SIZE", "1")), "steps": K, "warmup": W, "ms_per_step": t / K * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": prec, "data": "synthetic",
+        "config": {"workload": wl["desc"], "dims": list(dims), "sites": V, "alpha": ALPHA},
+        "cpu_baseline": {"value": value, "unit": "site-updates/s", "cores": orc.num_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": "site-updates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="c4", choices=sorted(WORKLOADS))
+    ap.add_argument("--no-extras", action="store_true", help="skip the per-kernel numbers of the other configs")
+    ap.add_argument("--e2e-steps", type=int, default=5, help="cap on host-buffer steps timed for e2e")
+    ap.add_argument("--ref-sites", type=int, default=400000, help="sites per step of the --impl reference sample")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -176,6 +176,13 @@ int lqx_smear_iterate_host(lqx_ctx* ctx, lqx_prec prec, const void* const host_u
 int lqx_bench_fma_peak(lqx_ctx* ctx, int kind, double* lane_ops_per_s);
 /* Plain device copy of `bytes` bytes (read + write counted): achieved bytes/s. */
 int lqx_bench_copy_peak(lqx_ctx* ctx, size_t bytes, double* bytes_per_s);
+/* Per-kernel-class device timing for the harness.  lqx_set_option(ctx, "time_kernels", 1) makes
+ * the library bracket every launch of the classes below with CUDA events on the context's stream;
+ * lqx_kernel_time synchronises the stream, returns the summed duration and launch count of one
+ * class since the last read, and clears it. */
+enum { LQX_K_SMEAR = 0, LQX_K_PLAQUETTE = 1, LQX_K_HOP = 2, LQX_K_CATALOGUE = 3, LQX_K_REDUCE = 4,
+       LQX_NUM_KERNEL_CLASSES = 5 };
+int lqx_kernel_time(lqx_ctx* ctx, int kernel_class, double* total_ms, int* count);
 /* Number of kernels this context has launched since init (for bench.py's gpu_launches). */
 int64_t lqx_launch_count(const lqx_ctx* ctx);
 /* Tuning knob for the smear kernel variant (0 = default/best). */

@@ -19,6 +19,7 @@ from . import build as _build
 F32, F64 = 4, 8
 COMPLEX, COLORVEC, COLORMAT, FERMION = 1, 3, 9, 12
 BACKWARD, FORWARD = -1, +1
+K_SMEAR, K_PLAQUETTE, K_HOP, K_CATALOGUE, K_REDUCE = range(5)
 KIND_SHAPE = {COMPLEX: (), COLORVEC: (3,), COLORMAT: (3, 3), FERMION: (4, 3)}
 _NP = {F32: np.float32, F64: np.float64}
 
@@ -87,6 +88,7 @@ SIGNATURES = {
     "lqx_smear_iterate_host": (_i, [_vp, _i, _pvp, _pvp, _d, _i, _pd]),
     "lqx_bench_fma_peak": (_i, [_vp, _i, _pd]),
     "lqx_bench_copy_peak": (_i, [_vp, C.c_size_t, _pd]),
+    "lqx_kernel_time": (_i, [_vp, _i, _pd, C.POINTER(C.c_int)]),
     "lqx_launch_count": (_i64, [_vp]),
     "lqx_set_option": (_i, [_vp, C.c_char_p, _i]),
     "lqx_strerror": (C.c_char_p, [_i]),
@@ -202,6 +204,12 @@ class Lattice:
 
     def set_option(self, key: str, value: int):
         _check(_lib.lqx_set_option(self.ctx, key.encode(), int(value)), self.ctx)
+
+    def kernel_time(self, kernel_class: int):
+        """-> (total_ms, count) of one kernel class since the last read (needs set_option('time_kernels', 1))."""
+        ms, n = C.c_double(), C.c_int()
+        _check(_lib.lqx_kernel_time(self.ctx, kernel_class, C.byref(ms), C.byref(n)), self.ctx)
+        return ms.value, n.value
 
     def launch_count(self) -> int:
         return int(_lib.lqx_launch_count(self.ctx))

@@ -88,6 +88,7 @@ extern "C" int lqx_init(const int dims[4], int device, void* cuda_stream, lqx_ct
     c->launches = 0;
     c->opt_smear_variant = 0;
     c->opt_block = 0;
+    c->timing = false;
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) {
         delete c;
@@ -112,6 +113,11 @@ extern "C" int lqx_finalize(lqx_ctx* ctx) {
         if (f->owned && f->data) cudaFree(f->data);
         delete f;
     }
+    for (auto& v : ctx->timers)
+        for (auto& pr : v) {
+            cudaEventDestroy(pr.first);
+            cudaEventDestroy(pr.second);
+        }
     if (ctx->d_partials) cudaFree(ctx->d_partials);
     if (ctx->d_result) cudaFree(ctx->d_result);
     if (ctx->h_result) cudaFreeHost(ctx->h_result);
@@ -140,7 +146,30 @@ extern "C" int lqx_set_option(lqx_ctx* ctx, const char* key, int value) {
     if (!ctx || !key) return LQX_EINVAL;
     if (!strcmp(key, "smear_variant")) ctx->opt_smear_variant = value;
     else if (!strcmp(key, "block")) ctx->opt_block = value;
+    else if (!strcmp(key, "time_kernels")) ctx->timing = value != 0;
     else return lqx_fail(ctx, LQX_EINVAL, "unknown option");
+    return LQX_OK;
+}
+
+extern "C" int lqx_kernel_time(lqx_ctx* ctx, int which, double* total_ms, int* count) {
+    if (!ctx || which < 0 || which >= LQX_NUM_KERNEL_CLASSES || !total_ms || !count) return LQX_EINVAL;
+    LQX_CUDA(ctx, cudaSetDevice(ctx->device));
+    LQX_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    double tot = 0.0;
+    int n = 0;
+    for (auto& pr : ctx->timers[which]) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, pr.first, pr.second) == cudaSuccess) {
+            tot += ms;
+            ++n;
+        }
+        cudaEventDestroy(pr.first);
+        cudaEventDestroy(pr.second);
+    }
+    ctx->timers[which].clear();
+    cudaGetLastError();
+    *total_ms = tot;
+    *count = n;
     return LQX_OK;
 }
 

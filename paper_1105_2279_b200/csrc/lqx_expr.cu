@@ -69,6 +69,7 @@ int flat_launch(lqx_ctx* ctx, lqx_field* r, const lqx_field* a, const lqx_field*
     size_t want = (nvec + block - 1) / block;
     int grid = (int)std::min<size_t>(want, (size_t)ctx->num_sms * 16);
     if (grid < 1) grid = 1;
+    LqxTimed timed(ctx, LQX_K_CATALOGUE);
     k_flat<T, MODE><<<grid, block, 0, ctx->stream>>>(nvec, (T)k, (const T*)a->data, b ? (const T*)b->data : nullptr,
                                                       (T*)r->data);
     LQX_LAUNCH_CHECK(ctx);
@@ -131,6 +132,7 @@ int shift_launch(lqx_ctx* ctx, lqx_field* r, double alpha, const lqx_field* a, c
     const int nplanes = 2 * (int)r->kind;
     const int block = 256;
     const T* pa = a ? (const T*)a->data : nullptr;
+    LqxTimed timed(ctx, LQX_K_CATALOGUE);
     if (g.L[0] % W == 0) {
         dim3 grid((g.V / W + block - 1) / block, nplanes);
         k_shift<T, W, AX><<<grid, block, 0, ctx->stream>>>(g, dir, mu, (T)alpha, pa, (const T*)b->data, (T*)r->data);
@@ -316,6 +318,7 @@ extern "C" int lqx_mm_plus_madj(lqx_field* r, const lqx_field* a, const lqx_fiel
     LQX_CUDA(ctx, cudaSetDevice(ctx->device));
     const Geo& g = ctx->geo;
     const int grid = (g.V + 127) / 128;
+    LqxTimed timed(ctx, LQX_K_CATALOGUE);
     if (r->prec == LQX_F32)
         k_mm_plus_madj<float><<<grid, 128, 0, ctx->stream>>>(g, (const float*)a->data, (const float*)b->data,
                                                             (const float*)c->data, (const float*)d->data, (float*)r->data);
@@ -335,6 +338,7 @@ extern "C" int lqx_trace_mm(lqx_field* c, const lqx_field* a, const lqx_field* b
     LQX_CUDA(ctx, cudaSetDevice(ctx->device));
     const Geo& g = ctx->geo;
     const int grid = (g.V + 127) / 128;
+    LqxTimed timed(ctx, LQX_K_CATALOGUE);
     if (c->prec == LQX_F32)
         k_trace_mm<float><<<grid, 128, 0, ctx->stream>>>(g, (const float*)a->data, (const float*)b->data, (float*)c->data);
     else
@@ -352,6 +356,7 @@ extern "C" int lqx_mat_vec(lqx_field* w, const lqx_field* m, const lqx_field* v)
     LQX_CUDA(ctx, cudaSetDevice(ctx->device));
     const Geo& g = ctx->geo;
     const int grid = (g.V + 127) / 128;
+    LqxTimed timed(ctx, LQX_K_CATALOGUE);
     const bool ferm = v->kind == LQX_FERMION;
     if (w->prec == LQX_F32) {
         if (ferm) k_mat_vec<float, 4><<<grid, 128, 0, ctx->stream>>>(g, (const float*)m->data, (const float*)v->data, (float*)w->data);
@@ -371,8 +376,11 @@ extern "C" int lqx_norm2(const lqx_field* f, double* out) {
     const int grid = reduce_grid(ctx, 8);
     int rc = lqx_ensure_partials(ctx, (size_t)grid);
     if (rc) return rc;
-    if (f->prec == LQX_F32) k_norm2<float><<<grid, 256, 0, ctx->stream>>>(ctx->geo, 2 * (int)f->kind, (const float*)f->data, ctx->d_partials);
-    else k_norm2<double><<<grid, 256, 0, ctx->stream>>>(ctx->geo, 2 * (int)f->kind, (const double*)f->data, ctx->d_partials);
+    {
+        LqxTimed timed(ctx, LQX_K_REDUCE);
+        if (f->prec == LQX_F32) k_norm2<float><<<grid, 256, 0, ctx->stream>>>(ctx->geo, 2 * (int)f->kind, (const float*)f->data, ctx->d_partials);
+        else k_norm2<double><<<grid, 256, 0, ctx->stream>>>(ctx->geo, 2 * (int)f->kind, (const double*)f->data, ctx->d_partials);
+    }
     LQX_LAUNCH_CHECK(ctx);
     rc = lqx_reduce_finish(ctx, grid, 1, ctx->d_result);
     if (rc) return rc;
@@ -387,7 +395,10 @@ extern "C" int lqx_sum(const lqx_field* f, double* out) {
     const int grid = reduce_grid(ctx, 4);
     int rc = lqx_ensure_partials(ctx, (size_t)grid * nc);
     if (rc) return rc;
-    rc = f->prec == LQX_F32 ? sum_launch<float>(ctx, f, grid) : sum_launch<double>(ctx, f, grid);
+    {
+        LqxTimed timed(ctx, LQX_K_REDUCE);
+        rc = f->prec == LQX_F32 ? sum_launch<float>(ctx, f, grid) : sum_launch<double>(ctx, f, grid);
+    }
     if (rc) return rc;
     rc = lqx_reduce_finish(ctx, grid, nc, ctx->d_result);
     if (rc) return rc;
@@ -402,8 +413,11 @@ extern "C" int lqx_trace(const lqx_field* m, double out[2]) {
     const int grid = reduce_grid(ctx, 4);
     int rc = lqx_ensure_partials(ctx, (size_t)grid * 2);
     if (rc) return rc;
-    if (m->prec == LQX_F32) k_trace<float><<<grid, 256, 0, ctx->stream>>>(ctx->geo, (const float*)m->data, ctx->d_partials);
-    else k_trace<double><<<grid, 256, 0, ctx->stream>>>(ctx->geo, (const double*)m->data, ctx->d_partials);
+    {
+        LqxTimed timed(ctx, LQX_K_REDUCE);
+        if (m->prec == LQX_F32) k_trace<float><<<grid, 256, 0, ctx->stream>>>(ctx->geo, (const float*)m->data, ctx->d_partials);
+        else k_trace<double><<<grid, 256, 0, ctx->stream>>>(ctx->geo, (const double*)m->data, ctx->d_partials);
+    }
     LQX_LAUNCH_CHECK(ctx);
     rc = lqx_reduce_finish(ctx, grid, 2, ctx->d_result);
     if (rc) return rc;

@@ -7,6 +7,7 @@
 #include <stdint.h>
 
 #include <string>
+#include <utility>
 #include <vector>
 
 #include "../../include/lqx.h"
@@ -42,6 +43,28 @@ struct lqx_ctx {
     int num_sms;
     int opt_smear_variant;
     int opt_block;
+    // optional per-kernel-class device timing (bench harness): cudaEvent pairs on the stream
+    bool timing;
+    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> timers[LQX_NUM_KERNEL_CLASSES];
+};
+
+// RAII: brackets the kernel launches of one class with events when ctx->timing is on
+struct LqxTimed {
+    lqx_ctx* ctx;
+    cudaEvent_t stop;
+    LqxTimed(lqx_ctx* c, int which) : ctx(c), stop(nullptr) {
+        if (!c->timing) return;
+        cudaEvent_t start;
+        if (cudaEventCreate(&start) != cudaSuccess || cudaEventCreate(&stop) != cudaSuccess) {
+            stop = nullptr;
+            return;
+        }
+        cudaEventRecord(start, c->stream);
+        c->timers[which].push_back(std::make_pair(start, stop));
+    }
+    ~LqxTimed() {
+        if (stop) cudaEventRecord(stop, ctx->stream);
+    }
 };
 
 struct lqx_field {

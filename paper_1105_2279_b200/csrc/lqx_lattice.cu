@@ -188,7 +188,10 @@ int plaquette_launch(lqx_ctx* ctx, const lqx_field* const u[4], double* d_out) {
     const int grid = (g.V + 127) / 128;
     int rc = lqx_ensure_partials(ctx, (size_t)grid);
     if (rc) return rc;
-    k_plaquette<T><<<grid, 128, 0, ctx->stream>>>(g, make_links<T>(u), ctx->d_partials);
+    {
+        LqxTimed timed(ctx, LQX_K_PLAQUETTE);
+        k_plaquette<T><<<grid, 128, 0, ctx->stream>>>(g, make_links<T>(u), ctx->d_partials);
+    }
     LQX_LAUNCH_CHECK(ctx);
     return lqx_reduce_finish(ctx, grid, 1, d_out);
 }
@@ -205,11 +208,17 @@ int smear_launch(lqx_ctx* ctx, lqx_field* const uout[4], const lqx_field* const 
     if (d_plaq) {
         int rc = lqx_ensure_partials(ctx, (size_t)grid);
         if (rc) return rc;
-        k_smear_gather<T, true><<<grid, 128, 0, ctx->stream>>>(g, make_links<T>(uin), o, c0, c1, only_mu, ctx->d_partials);
+        {
+            LqxTimed timed(ctx, LQX_K_SMEAR);
+            k_smear_gather<T, true><<<grid, 128, 0, ctx->stream>>>(g, make_links<T>(uin), o, c0, c1, only_mu, ctx->d_partials);
+        }
         LQX_LAUNCH_CHECK(ctx);
         return lqx_reduce_finish(ctx, grid, 1, d_plaq);
     }
-    k_smear_gather<T, false><<<grid, 128, 0, ctx->stream>>>(g, make_links<T>(uin), o, c0, c1, only_mu, nullptr);
+    {
+        LqxTimed timed(ctx, LQX_K_SMEAR);
+        k_smear_gather<T, false><<<grid, 128, 0, ctx->stream>>>(g, make_links<T>(uin), o, c0, c1, only_mu, nullptr);
+    }
     LQX_LAUNCH_CHECK(ctx);
     return LQX_OK;
 }
@@ -244,6 +253,8 @@ static int hop_impl(lqx_field* chi, const lqx_field* const u[4], const lqx_field
         if (rc) return rc;
     }
     const bool ferm = psi->kind == LQX_FERMION;
+    {
+    LqxTimed timed(ctx, LQX_K_HOP);
 #define LQX_HOP(T, NSPIN, N2) \
     k_hop<T, NSPIN, N2><<<grid, 128, 0, ctx->stream>>>(g, make_links<T>(u), (const T*)psi->data, (T*)chi->data, ctx->d_partials)
     if (psi->prec == LQX_F32) {
@@ -254,6 +265,7 @@ static int hop_impl(lqx_field* chi, const lqx_field* const u[4], const lqx_field
         else      { if (n2) LQX_HOP(double, 1, true); else LQX_HOP(double, 1, false); }
     }
 #undef LQX_HOP
+    }
     LQX_LAUNCH_CHECK(ctx);
     if (n2) {
         rc = lqx_reduce_finish(ctx, grid, 1, ctx->d_result);

@@ -304,8 +304,8 @@ def test_smear_iterate_trajectory(lqx, prec, nsteps):
             assert abs(plaqs[k] - want_p[k]) < RTOL[prec], k
         for mu in range(4):
             assert site_rel_err(fu[mu].pop(), want_u[mu]) < TOL[prec] * nsteps
-        # plaquette rises monotonically towards 1 under smearing of a smooth field
-        assert all(plaqs[k + 1] > plaqs[k] for k in range(nsteps - 1)) and plaqs[-1] < 1.0
+        # no projection back to SU(3) (reading A9): the links shrink, so nothing is asserted about
+        # the direction in which the plaquette moves -- only agreement with the oracle's trajectory
 
 
 def test_smear_iterate_host_end_to_end(lqx):
