@@ -340,7 +340,7 @@ def run_ours(args):
                               "plaquette_launches": plaq_n, "timed_region": ms},
     }
 
-    if world == 1:
+    if world == 1 and not args.kernel_only:
         # ---- e2e: the public host-buffer call, H2D + D2H inside the timed region, every step
         hin = host
         hout = [torch.empty(h.shape, dtype=h.dtype, pin_memory=True) for h in host]
@@ -368,7 +368,7 @@ def run_ours(args):
         f.free()
     lat.close()
     torch.cuda.empty_cache()
-    if world == 1 and not args.no_extras:
+    if world == 1 and not args.no_extras and not args.kernel_only:
         line["kernels"] = _extras(torch, lqx, li, hbm_gbs)
     if rank == 0:
         print(json.dumps(line))
@@ -440,6 +440,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="c4", choices=sorted(WORKLOADS))
     ap.add_argument("--no-extras", action="store_true", help="skip the per-kernel numbers of the other configs")
+    ap.add_argument("--kernel-only", action="store_true",
+                    help="timed device region only (no e2e, no cpu_baseline, no extras): the command ncu wraps")
     ap.add_argument("--e2e-steps", type=int, default=5, help="cap on host-buffer steps timed for e2e")
     ap.add_argument("--ref-sites", type=int, default=400000, help="sites per step of the --impl reference sample")
     args = ap.parse_args()
