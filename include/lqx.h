@@ -19,9 +19,13 @@
  *     site(x) = x0 + L0*(x1 + L1*(x2 + L2*x3)); inside a site, outer->inner:
  *     [spin][colour row][colour column][re,im]; real index of a colour matrix element
  *     ((s*3+i)*3+j)*2+c, fermion ((s*4+a)*3+i)*2+c, colour vector (s*3+i)*2+c, complex s*2+c.
- *   * Internal device layout: site-fastest structure of arrays, one plane per real component,
- *     plane index = (QDP-order real index inside the site), plane stride = lqx_plane_stride()
- *     elements (V rounded up to 32).  Element (component r, site s) lives at r*stride + s.
+ *   * Internal device layout: blocked site-fastest structure of arrays.  Sites are grouped in
+ *     blocks of 32 consecutive lexicographic sites; inside a block the 2*kind reals of a site
+ *     object (QDP order) are cut into 128-bit chunks of W = 16/prec reals, and chunk q of the 32
+ *     sites is contiguous (a trailing half chunk of 2 reals exists for fp32 when 2*kind % 4 == 2).
+ *     Element (site s, real r), q = r / W, lies at
+ *         (s/32)*32*2*kind + q*32*W + (s%32)*w_q + (r - q*W),   w_q = W (full chunk) or 2 (half).
+ *     lqx_field_offset() evaluates this; a field occupies lqx_padded_volume()*2*kind reals.
  *   * shift(f, LQX_FORWARD, mu)(x) = f(x + mu^), shift(f, LQX_BACKWARD, mu)(x) = f(x - mu^)
  *     (fixed by Listing 1 line 25 against Eq. 2), periodic in every
  *     direction.
@@ -74,7 +78,10 @@ int lqx_init(const int dims[4], int device, void* cuda_stream, lqx_ctx** out);
 int lqx_finalize(lqx_ctx* ctx);
 int lqx_set_stream(lqx_ctx* ctx, void* cuda_stream);
 int64_t lqx_volume(const lqx_ctx* ctx);       /* V = L0*L1*L2*L3, or negative status            */
-int64_t lqx_plane_stride(const lqx_ctx* ctx); /* elements between component planes              */
+int64_t lqx_padded_volume(const lqx_ctx* ctx); /* V rounded up to whole 32-site blocks          */
+/* Element offset of (site, QDP-order real index) inside a field of this kind/precision in the
+ * internal layout, or a negative status. */
+int64_t lqx_field_offset(const lqx_ctx* ctx, lqx_kind kind, lqx_prec prec, int64_t site, int real_index);
 /* Bytes of device memory a field of this kind/precision occupies in the internal layout. */
 int64_t lqx_field_bytes(const lqx_ctx* ctx, lqx_kind kind, lqx_prec prec);
 /* Periodic neighbour table computed ON THE DEVICE by the same index arithmetic the kernels use:
@@ -94,9 +101,9 @@ int lqx_field_free(lqx_field* f);
 void* lqx_field_data(const lqx_field* f); /* device pointer of plane 0 (NULL on bad handle)     */
 int lqx_field_kind(const lqx_field* f);
 int lqx_field_prec(const lqx_field* f);
-/* host QDP order -> device SoA.  host: V*2*kind reals of the field precision.  Bit-exact. */
+/* host QDP order -> device blocked SoA.  host: V*2*kind reals of the field precision.  Bit-exact. */
 int lqx_field_push(lqx_field* f, const void* host_qdp_order);
-/* device SoA -> host QDP order.  Synchronises.  Bit-exact.  Does not free (reading A4). */
+/* device blocked SoA -> host QDP order.  Synchronises.  Bit-exact.  Does not free (reading A4). */
 int lqx_field_pop(const lqx_field* f, void* host_qdp_order);
 /* Same converters between two DEVICE buffers (dev_qdp_order: V*2*kind reals, AoS). Asynchronous. */
 int lqx_field_import_dev(lqx_field* f, const void* dev_qdp_order);
@@ -185,7 +192,9 @@ enum { LQX_K_SMEAR = 0, LQX_K_PLAQUETTE = 1, LQX_K_HOP = 2, LQX_K_CATALOGUE = 3,
 int lqx_kernel_time(lqx_ctx* ctx, int kernel_class, double* total_ms, int* count);
 /* Number of kernels this context has launched since init (for bench.py's gpu_launches). */
 int64_t lqx_launch_count(const lqx_ctx* ctx);
-/* Tuning knob for the smear kernel variant (0 = default/best). */
+/* Options: "smear_variant" 0 = best available, 1 = literal 48-product kernel, 2 = shared-corner
+ * kernel only; "tile" -1 = automatic, 0 = linear blocks, 1..3 = CTA tile shape of the
+ * nearest-neighbour kernels; "time_kernels" 0/1 (see above).  DESIGN.md sec.6. */
 int lqx_set_option(lqx_ctx* ctx, const char* key, int value);
 
 const char* lqx_strerror(int code);

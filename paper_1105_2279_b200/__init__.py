@@ -54,7 +54,8 @@ SIGNATURES = {
     "lqx_finalize": (_i, [_vp]),
     "lqx_set_stream": (_i, [_vp, _vp]),
     "lqx_volume": (_i64, [_vp]),
-    "lqx_plane_stride": (_i64, [_vp]),
+    "lqx_padded_volume": (_i64, [_vp]),
+    "lqx_field_offset": (_i64, [_vp, _i, _i, _i64, _i]),
     "lqx_field_bytes": (_i64, [_vp, _i, _i]),
     "lqx_neighbor_table": (_i, [_vp, _i, _i, _vp]),
     "lqx_field_alloc": (_i, [_vp, _i, _i, _pvp]),
@@ -149,7 +150,7 @@ class Lattice:
         _check(_lib.lqx_init((C.c_int * 4)(*self.dims), self.device, C.c_void_p(stream.cuda_stream), C.byref(out)))
         self.ctx = out
         self.volume = int(_lib.lqx_volume(self.ctx))
-        self.stride = int(_lib.lqx_plane_stride(self.ctx))
+        self.padded_volume = int(_lib.lqx_padded_volume(self.ctx))
         self._fields = []
 
     def close(self):
@@ -168,6 +169,13 @@ class Lattice:
 
     def field_bytes(self, kind, prec) -> int:
         return int(_lib.lqx_field_bytes(self.ctx, kind, prec))
+
+    def field_offset(self, kind, prec, site: int, real_index: int) -> int:
+        """Element offset of (site, QDP-order real index) in the internal blocked-SoA layout."""
+        r = int(_lib.lqx_field_offset(self.ctx, kind, prec, int(site), int(real_index)))
+        if r < 0:
+            raise LqxError(r)
+        return r
 
     def alloc(self, kind, prec, torch_memory: bool = True) -> "Field":
         """New zero field.  torch_memory=True: a torch uint8 tensor owns the bytes and the library

@@ -1,6 +1,6 @@
-// lqx core: context, geometry, device field store with QDP-order <-> SoA converters
+// lqx core: context, geometry, device field store with QDP-order <-> blocked-SoA converters
 // (SURVEY 8(a) a1, a2; PAPER.md:101-103 site tables, :195-202 push/pop/free), error handling and
-// the shared second stage of the reductions.
+// the result hand-off of the reductions.
 #include <math.h>
 #include <stdio.h>
 #include <string.h>
@@ -75,7 +75,7 @@ extern "C" int lqx_init(const int dims[4], int device, void* cuda_stream, lqx_ct
         st *= dims[d];
     }
     g.V = (int)v;
-    g.stride = (int)((v + 31) & ~(int64_t)31);
+    g.Vpad = (int)((v + 31) & ~(int64_t)31);
     g.d0 = make_fastdiv((uint32_t)dims[0]);
     g.d1 = make_fastdiv((uint32_t)dims[1]);
     g.d2 = make_fastdiv((uint32_t)dims[2]);
@@ -88,6 +88,7 @@ extern "C" int lqx_init(const int dims[4], int device, void* cuda_stream, lqx_ct
     c->launches = 0;
     c->opt_smear_variant = 0;
     c->opt_block = 0;
+    c->opt_tile = -1;
     c->timing = false;
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) {
@@ -95,9 +96,14 @@ extern "C" int lqx_init(const int dims[4], int device, void* cuda_stream, lqx_ct
         return LQX_ECUDA;
     }
     c->num_sms = prop.multiProcessorCount;
+    c->d_ticket = nullptr;
     if (cudaMalloc(&c->d_result, 64 * sizeof(double)) != cudaSuccess ||
-        cudaMallocHost(&c->h_result, 64 * sizeof(double)) != cudaSuccess) {
+        cudaMalloc(&c->d_ticket, sizeof(unsigned int)) != cudaSuccess ||
+        cudaHostAlloc(&c->h_result, 64 * sizeof(double), cudaHostAllocPortable | cudaHostAllocMapped) != cudaSuccess ||
+        cudaMemset(c->d_ticket, 0, sizeof(unsigned int)) != cudaSuccess) {
         if (c->d_result) cudaFree(c->d_result);
+        if (c->d_ticket) cudaFree(c->d_ticket);
+        cudaGetLastError();
         delete c;
         return LQX_ENOMEM;
     }
@@ -120,6 +126,7 @@ extern "C" int lqx_finalize(lqx_ctx* ctx) {
         }
     if (ctx->d_partials) cudaFree(ctx->d_partials);
     if (ctx->d_result) cudaFree(ctx->d_result);
+    if (ctx->d_ticket) cudaFree(ctx->d_ticket);
     if (ctx->h_result) cudaFreeHost(ctx->h_result);
     delete ctx;
     return LQX_OK;
@@ -131,7 +138,7 @@ extern "C" int lqx_set_stream(lqx_ctx* ctx, void* cuda_stream) {
     return LQX_OK;
 }
 extern "C" int64_t lqx_volume(const lqx_ctx* ctx) { return ctx ? ctx->geo.V : (int64_t)LQX_EINVAL; }
-extern "C" int64_t lqx_plane_stride(const lqx_ctx* ctx) { return ctx ? ctx->geo.stride : (int64_t)LQX_EINVAL; }
+extern "C" int64_t lqx_padded_volume(const lqx_ctx* ctx) { return ctx ? ctx->geo.Vpad : (int64_t)LQX_EINVAL; }
 extern "C" int64_t lqx_launch_count(const lqx_ctx* ctx) { return ctx ? ctx->launches : (int64_t)LQX_EINVAL; }
 
 static bool valid_kind(int k) { return k == LQX_COMPLEX || k == LQX_COLORVEC || k == LQX_COLORMAT || k == LQX_FERMION; }
@@ -139,13 +146,21 @@ static bool valid_prec(int p) { return p == LQX_F32 || p == LQX_F64; }
 
 extern "C" int64_t lqx_field_bytes(const lqx_ctx* ctx, lqx_kind kind, lqx_prec prec) {
     if (!ctx || !valid_kind(kind) || !valid_prec(prec)) return LQX_EINVAL;
-    return (int64_t)ctx->geo.stride * 2 * (int)kind * (int)prec;
+    return (int64_t)ctx->geo.Vpad * 2 * (int)kind * (int)prec;
+}
+
+extern "C" int64_t lqx_field_offset(const lqx_ctx* ctx, lqx_kind kind, lqx_prec prec, int64_t site, int real_index) {
+    if (!ctx || !valid_kind(kind) || !valid_prec(prec)) return LQX_EINVAL;
+    const int nreal = 2 * (int)kind;
+    if (site < 0 || site >= ctx->geo.V || real_index < 0 || real_index >= nreal) return LQX_EINVAL;
+    return (int64_t)lqx_layout_offset((int)site, real_index, nreal, 16 / (int)prec);
 }
 
 extern "C" int lqx_set_option(lqx_ctx* ctx, const char* key, int value) {
     if (!ctx || !key) return LQX_EINVAL;
     if (!strcmp(key, "smear_variant")) ctx->opt_smear_variant = value;
     else if (!strcmp(key, "block")) ctx->opt_block = value;
+    else if (!strcmp(key, "tile")) ctx->opt_tile = value;
     else if (!strcmp(key, "time_kernels")) ctx->timing = value != 0;
     else return lqx_fail(ctx, LQX_EINVAL, "unknown option");
     return LQX_OK;
@@ -224,7 +239,7 @@ extern "C" int lqx_field_alloc(lqx_ctx* ctx, lqx_kind kind, lqx_prec prec, lqx_f
         cudaGetLastError();
         return lqx_fail(ctx, LQX_ENOMEM, "cudaMalloc field");
     }
-    // the pad between V and the plane stride is never read for results, but keep it defined
+    // the pad lanes of the last 32-site block are never read for results, but keep them defined
     cudaError_t e = cudaMemsetAsync(p, 0, bytes, ctx->stream);
     if (e != cudaSuccess) {
         cudaFree(p);
@@ -263,31 +278,48 @@ extern "C" void* lqx_field_data(const lqx_field* f) { return f ? f->data : nullp
 extern "C" int lqx_field_kind(const lqx_field* f) { return f ? (int)f->kind : LQX_EINVAL; }
 extern "C" int lqx_field_prec(const lqx_field* f) { return f ? (int)f->prec : LQX_EINVAL; }
 
-// AoS (QDP order) <-> SoA.  One block handles 32 consecutive sites through shared memory so that
-// both the AoS side (32*NR contiguous reals) and the SoA side (NR runs of 32 reals) are coalesced.
+// AoS (QDP order) <-> blocked SoA.  One CUDA block handles one 32-site layout block: both sides are
+// the same 32*nreal contiguous reals, so the conversion is a permutation staged through shared
+// memory with coalesced reads and writes on both sides.
 template <typename T, bool TO_SOA>
-__global__ void k_transpose(int V, int stride, int nreal, const T* __restrict__ src, T* __restrict__ dst) {
+__global__ void k_transpose(int V, int nreal, const T* __restrict__ src, T* __restrict__ dst) {
     extern __shared__ unsigned char smem_raw[];
-    T* tile = reinterpret_cast<T*>(smem_raw);  // [32][nreal+1]
+    T* tile = reinterpret_cast<T*>(smem_raw);  // [32][nreal+1], QDP order
+    constexpr int W = 16 / (int)sizeof(T);
     const int s0 = blockIdx.x * 32;
     const int ns = min(32, V - s0);
     const int pitch = nreal + 1;
+    const int nfull = nreal / W, rem = nreal - nfull * W;
+    const size_t blk = (size_t)s0 * nreal;
+    // internal position i of the block -> (local site, real)
+    auto decode = [&](int i, int& ls, int& r) {
+        const int q = i / (32 * W);
+        if (q < nfull) {
+            const int t = i - q * 32 * W;
+            ls = t / W;
+            r = q * W + (t - ls * W);
+        } else {
+            const int t = i - nfull * 32 * W;
+            ls = t / rem;
+            r = nfull * W + (t - ls * rem);
+        }
+    };
     if (TO_SOA) {
-        const T* a = src + (size_t)s0 * nreal;
-        for (int i = threadIdx.x; i < ns * nreal; i += blockDim.x) tile[(i / nreal) * pitch + (i % nreal)] = a[i];
+        for (int i = threadIdx.x; i < ns * nreal; i += blockDim.x) tile[(i / nreal) * pitch + (i % nreal)] = src[blk + i];
         __syncthreads();
         for (int i = threadIdx.x; i < 32 * nreal; i += blockDim.x) {
-            int r = i >> 5, ls = i & 31;
-            if (ls < ns) dst[(size_t)r * stride + s0 + ls] = tile[ls * pitch + r];
+            int ls, r;
+            decode(i, ls, r);
+            dst[blk + i] = ls < ns ? tile[ls * pitch + r] : T(0);  // pad lanes of the last block stay zero
         }
     } else {
         for (int i = threadIdx.x; i < 32 * nreal; i += blockDim.x) {
-            int r = i >> 5, ls = i & 31;
-            if (ls < ns) tile[ls * pitch + r] = src[(size_t)r * stride + s0 + ls];
+            int ls, r;
+            decode(i, ls, r);
+            if (ls < ns) tile[ls * pitch + r] = src[blk + i];
         }
         __syncthreads();
-        T* a = dst + (size_t)s0 * nreal;
-        for (int i = threadIdx.x; i < ns * nreal; i += blockDim.x) a[i] = tile[(i / nreal) * pitch + (i % nreal)];
+        for (int i = threadIdx.x; i < ns * nreal; i += blockDim.x) dst[blk + i] = tile[(i / nreal) * pitch + (i % nreal)];
     }
 }
 
@@ -297,11 +329,11 @@ static int transpose_launch(lqx_ctx* ctx, const lqx_field* f, const void* src, v
     const int nblk = (g.V + 31) / 32;
     const size_t sm = (size_t)32 * (nreal + 1) * (int)f->prec;
     if (f->prec == LQX_F32) {
-        if (to_soa) k_transpose<float, true><<<nblk, 256, sm, ctx->stream>>>(g.V, g.stride, nreal, (const float*)src, (float*)dst);
-        else k_transpose<float, false><<<nblk, 256, sm, ctx->stream>>>(g.V, g.stride, nreal, (const float*)src, (float*)dst);
+        if (to_soa) k_transpose<float, true><<<nblk, 256, sm, ctx->stream>>>(g.V, nreal, (const float*)src, (float*)dst);
+        else k_transpose<float, false><<<nblk, 256, sm, ctx->stream>>>(g.V, nreal, (const float*)src, (float*)dst);
     } else {
-        if (to_soa) k_transpose<double, true><<<nblk, 256, sm, ctx->stream>>>(g.V, g.stride, nreal, (const double*)src, (double*)dst);
-        else k_transpose<double, false><<<nblk, 256, sm, ctx->stream>>>(g.V, g.stride, nreal, (const double*)src, (double*)dst);
+        if (to_soa) k_transpose<double, true><<<nblk, 256, sm, ctx->stream>>>(g.V, nreal, (const double*)src, (double*)dst);
+        else k_transpose<double, false><<<nblk, 256, sm, ctx->stream>>>(g.V, nreal, (const double*)src, (double*)dst);
     }
     LQX_LAUNCH_CHECK(ctx);
     return LQX_OK;
@@ -378,32 +410,7 @@ int lqx_ensure_partials(lqx_ctx* ctx, size_t ndoubles) {
     return LQX_OK;
 }
 
-// one block per component; fixed strided accumulation + fixed tree => deterministic
-__global__ void k_reduce_finish(const double* __restrict__ partials, int nblocks, double* __restrict__ out) {
-    __shared__ double sh[32];
-    const double* p = partials + (size_t)blockIdx.x * nblocks;
-    double t = 0.0;
-    for (int i = threadIdx.x; i < nblocks; i += blockDim.x) t += p[i];
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
-    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = t;
-    __syncthreads();
-    if (threadIdx.x < 32) {
-        t = (threadIdx.x < (blockDim.x >> 5)) ? sh[threadIdx.x] : 0.0;
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
-        if (threadIdx.x == 0) out[blockIdx.x] = t;
-    }
-}
-
-int lqx_reduce_finish(lqx_ctx* ctx, int nblocks, int ncomp, double* d_out) {
-    k_reduce_finish<<<ncomp, 1024, 0, ctx->stream>>>(ctx->d_partials, nblocks, d_out);
-    LQX_LAUNCH_CHECK(ctx);
-    return LQX_OK;
-}
-
 int lqx_fetch_result(lqx_ctx* ctx, int n, double* out) {
-    LQX_CUDA(ctx, cudaMemcpyAsync(ctx->h_result, ctx->d_result, n * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     LQX_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     for (int i = 0; i < n; ++i) out[i] = ctx->h_result[i];
     return LQX_OK;

@@ -1,20 +1,11 @@
 // lqx expression catalogue and standalone global reductions (a9).
 // Every entry point is one pass over HBM: the whole expression, shift included, is evaluated per
-// site with no temporaries (the paper's evaluate()), operands read from the
-// site-fastest SoA planes so that a warp touches 32 consecutive reals of each plane.
+// site with no temporaries (the paper's evaluate()).  One thread owns one
+// site; its operands arrive as 128-bit loads from the blocked SoA store (lqx_internal.cuh), so a
+// warp moves 512 contiguous bytes per instruction.
 #include "lqx_internal.cuh"
 
 namespace {
-
-// NS consecutive sites of one plane as one 8/16-byte access
-template <typename T, int NS>
-struct alignas(sizeof(T) * NS) Pack {
-    T v[NS];
-};
-template <typename T>
-struct VecWidth {
-    static constexpr int value = 16 / sizeof(T);  // 128-bit accesses
-};
 
 __device__ __forceinline__ float mul_rn(float a, float b) { return __fmul_rn(a, b); }
 __device__ __forceinline__ double mul_rn(double a, double b) { return __dmul_rn(a, b); }
@@ -37,34 +28,33 @@ int check_same(lqx_ctx** ctx_out, std::initializer_list<const lqx_field*> fs) {
 }
 
 // ---------------------------------------------------------------------------------------------
-// flat elementwise kernels over the whole plane array (pad included: it is never read for results)
-// mode 0: r = a ; 1: r = a + k*b ; 2: r = k*a ; 3: r = a / k
+// flat elementwise kernels over the raw storage (layout-agnostic; pad lanes included, they are
+// never read for results).  mode 0: r = a ; 1: r = a + k*b ; 2: r = k*a ; 3: r = a / k
 // ---------------------------------------------------------------------------------------------
 template <typename T, int MODE>
-__global__ void k_flat(size_t nvec, T k, const T* __restrict__ a, const T* __restrict__ b, T* __restrict__ r) {
-    constexpr int W = VecWidth<T>::value;
-    typedef Pack<T, W> P;
+__global__ void __launch_bounds__(256) k_flat(size_t nvec, T k, const T* __restrict__ a, const T* __restrict__ b, T* __restrict__ r) {
+    typedef typename Vec128<T>::type V;
+    constexpr int W = Vec128<T>::W;
     const size_t step = (size_t)gridDim.x * blockDim.x;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += step) {
-        P va = reinterpret_cast<const P*>(a)[i];
-        P vb;
-        if (MODE == 1) vb = reinterpret_cast<const P*>(b)[i];
-        P vr;
+        T va[W], vb[W], vr[W];
+        unpack(reinterpret_cast<const V*>(a)[i], va);
+        if (MODE == 1) unpack(reinterpret_cast<const V*>(b)[i], vb);
 #pragma unroll
         for (int j = 0; j < W; ++j) {
-            if (MODE == 0) vr.v[j] = va.v[j];
-            if (MODE == 1) vr.v[j] = fma(k, vb.v[j], va.v[j]);
-            if (MODE == 2) vr.v[j] = k * va.v[j];
-            if (MODE == 3) vr.v[j] = va.v[j] / k;
+            if (MODE == 0) vr[j] = va[j];
+            if (MODE == 1) vr[j] = fma(k, vb[j], va[j]);
+            if (MODE == 2) vr[j] = k * va[j];
+            if (MODE == 3) vr[j] = va[j] / k;
         }
-        reinterpret_cast<P*>(r)[i] = vr;
+        reinterpret_cast<V*>(r)[i] = pack(vr);
     }
 }
 
 template <typename T, int MODE>
 int flat_launch(lqx_ctx* ctx, lqx_field* r, const lqx_field* a, const lqx_field* b, double k) {
-    const size_t n = (size_t)ctx->geo.stride * 2 * (int)r->kind;
-    const size_t nvec = n / VecWidth<T>::value;
+    const size_t n = (size_t)ctx->geo.Vpad * 2 * (int)r->kind;
+    const size_t nvec = n / Vec128<T>::W;
     const int block = 256;
     size_t want = (nvec + block - 1) / block;
     int grid = (int)std::min<size_t>(want, (size_t)ctx->num_sms * 16);
@@ -87,58 +77,42 @@ int flat_dispatch(lqx_field* r, const lqx_field* a, const lqx_field* b, double k
 }
 
 // ---------------------------------------------------------------------------------------------
-// shift and form (iii): one thread = NS consecutive sites of one plane (blockIdx.y = plane).
-// For mu >= 1 the neighbours of NS aligned consecutive sites are NS aligned consecutive sites
-// (L0 % NS == 0), so the shifted operand is one vector access; for mu == 0 they straddle the
-// vector boundary and wrap at the row end, so they are read element-wise (L1 serves the overlap).
-// AX = false: r = shift(b);  AX = true: r = alpha*a - shift(b)
+// shift and form (iii): one thread per site; the shifted operand is the whole site object at the
+// periodic neighbour ("shift ... reads its operand through a site table" -- here the
+// index is computed).  AX = false: r = shift(b);  AX = true: r = alpha*a - shift(b)
 // ---------------------------------------------------------------------------------------------
-template <typename T, int NS, bool AX>
-__global__ void k_shift(const __grid_constant__ Geo g, int dir, int mu, T alpha, const T* __restrict__ a, const T* __restrict__ b,
-                        T* __restrict__ r) {
-    typedef Pack<T, NS> P;
-    const int s0 = (blockIdx.x * blockDim.x + threadIdx.x) * NS;
-    if (s0 >= g.V) return;
-    const size_t plane = (size_t)blockIdx.y * g.stride;
+template <typename T, int NREAL, bool AX>
+__global__ void __launch_bounds__(128) k_shift(const __grid_constant__ Geo g, int dir, int mu, T alpha, const T* __restrict__ a,
+                                               const T* __restrict__ b, T* __restrict__ r) {
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= g.V) return;
     int x[4];
-    site_coords(g, s0, x);
-    P vb;
-    if (mu == 0 && NS > 1) {
-#pragma unroll
-        for (int j = 0; j < NS; ++j) {
-            int xj = x[0] + j + dir;
-            xj = xj < 0 ? xj + g.L[0] : (xj >= g.L[0] ? xj - g.L[0] : xj);
-            vb.v[j] = __ldg(b + plane + (s0 - x[0]) + xj);
-        }
-    } else {
-        const int n0 = dir > 0 ? nbr_fwd(g, s0, x, mu) : nbr_bwd(g, s0, x, mu);
-        vb = *reinterpret_cast<const P*>(b + plane + n0);
-    }
-    P vr;
+    site_coords(g, s, x);
+    const int n = dir > 0 ? nbr_fwd(g, s, x, mu) : nbr_bwd(g, s, x, mu);
+    T vb[NREAL];
+    load_site<T, NREAL>(b, n, vb);
     if (AX) {
-        P va = *reinterpret_cast<const P*>(a + plane + s0);
+        T va[NREAL];
+        load_site<T, NREAL>(a, s, va);
 #pragma unroll
-        for (int j = 0; j < NS; ++j) vr.v[j] = mul_rn(alpha, va.v[j]) - vb.v[j];  // alpha*A rounded once, as written
-    } else {
-        vr = vb;
+        for (int j = 0; j < NREAL; ++j) vb[j] = mul_rn(alpha, va[j]) - vb[j];  // alpha*A rounded once, as written
     }
-    *reinterpret_cast<P*>(r + plane + s0) = vr;
+    store_site<T, NREAL>(r, s, vb);
 }
 
 template <typename T, bool AX>
 int shift_launch(lqx_ctx* ctx, lqx_field* r, double alpha, const lqx_field* a, const lqx_field* b, int dir, int mu) {
     const Geo& g = ctx->geo;
-    constexpr int W = VecWidth<T>::value;
-    const int nplanes = 2 * (int)r->kind;
-    const int block = 256;
+    const int block = 128, grid = (g.V + block - 1) / block;
     const T* pa = a ? (const T*)a->data : nullptr;
+    const T* pb = (const T*)b->data;
+    T* pr = (T*)r->data;
     LqxTimed timed(ctx, LQX_K_CATALOGUE);
-    if (g.L[0] % W == 0) {
-        dim3 grid((g.V / W + block - 1) / block, nplanes);
-        k_shift<T, W, AX><<<grid, block, 0, ctx->stream>>>(g, dir, mu, (T)alpha, pa, (const T*)b->data, (T*)r->data);
-    } else {
-        dim3 grid((g.V + block - 1) / block, nplanes);
-        k_shift<T, 1, AX><<<grid, block, 0, ctx->stream>>>(g, dir, mu, (T)alpha, pa, (const T*)b->data, (T*)r->data);
+    switch ((int)r->kind) {
+        case LQX_COMPLEX: k_shift<T, 2, AX><<<grid, block, 0, ctx->stream>>>(g, dir, mu, (T)alpha, pa, pb, pr); break;
+        case LQX_COLORVEC: k_shift<T, 6, AX><<<grid, block, 0, ctx->stream>>>(g, dir, mu, (T)alpha, pa, pb, pr); break;
+        case LQX_COLORMAT: k_shift<T, 18, AX><<<grid, block, 0, ctx->stream>>>(g, dir, mu, (T)alpha, pa, pb, pr); break;
+        default: k_shift<T, 24, AX><<<grid, block, 0, ctx->stream>>>(g, dir, mu, (T)alpha, pa, pb, pr); break;
     }
     LQX_LAUNCH_CHECK(ctx);
     return LQX_OK;
@@ -149,24 +123,22 @@ int shift_launch(lqx_ctx* ctx, lqx_field* r, double alpha, const lqx_field* a, c
 // ---------------------------------------------------------------------------------------------
 // form (i) R = A*B + C*adj(D)
 template <typename T>
-__global__ void __launch_bounds__(128) k_mm_plus_madj(const __grid_constant__ Geo g, const T* __restrict__ a, const T* __restrict__ b,
-                                                      const T* __restrict__ c, const T* __restrict__ d,
-                                                      T* __restrict__ r) {
+__global__ void __launch_bounds__(128) k_mm_plus_madj(int V, const T* __restrict__ a, const T* __restrict__ b, const T* __restrict__ c,
+                                                      const T* __restrict__ d, T* __restrict__ r) {
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= g.V) return;
-    Mat3<T> ma = load_mat(a, g.stride, s), mb = load_mat(b, g.stride, s);
-    Mat3<T> mc = load_mat(c, g.stride, s), md = load_mat(d, g.stride, s);
+    if (s >= V) return;
+    const Mat3<T> ma = load_mat(a, s), mb = load_mat(b, s);
+    const Mat3<T> mc = load_mat(c, s), md = load_mat(d, s);
     Mat3<T> acc = mul_nn(ma, mb);
     mac_na(acc, mc, md);
-    store_mat(r, g.stride, s, acc);
+    store_mat(r, s, acc);
 }
 // form (ii) c = trace(A*B) = sum_ik A_ik B_ki
 template <typename T>
-__global__ void __launch_bounds__(128) k_trace_mm(const __grid_constant__ Geo g, const T* __restrict__ a, const T* __restrict__ b,
-                                                  T* __restrict__ c) {
+__global__ void __launch_bounds__(128) k_trace_mm(int V, const T* __restrict__ a, const T* __restrict__ b, T* __restrict__ c) {
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= g.V) return;
-    Mat3<T> ma = load_mat(a, g.stride, s), mb = load_mat(b, g.stride, s);
+    if (s >= V) return;
+    const Mat3<T> ma = load_mat(a, s), mb = load_mat(b, s);
     T re = T(0), im = T(0);
 #pragma unroll
     for (int i = 0; i < 3; ++i)
@@ -177,99 +149,110 @@ __global__ void __launch_bounds__(128) k_trace_mm(const __grid_constant__ Geo g,
             im = fma(ma.re[i][k], mb.im[k][i], im);
             im = fma(ma.im[i][k], mb.re[k][i], im);
         }
-    c[s] = re;
-    c[(size_t)g.stride + s] = im;
+    const T out[2] = {re, im};
+    store_site<T, 2>(c, s, out);
 }
 // form (iv) w = M*v per spin component
 template <typename T, int NSPIN>
-__global__ void __launch_bounds__(128) k_mat_vec(const __grid_constant__ Geo g, const T* __restrict__ m, const T* __restrict__ v,
-                                                 T* __restrict__ w) {
+__global__ void __launch_bounds__(128) k_mat_vec(int V, const T* __restrict__ m, const T* __restrict__ v, T* __restrict__ w) {
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= g.V) return;
-    Mat3<T> mm = load_mat(m, g.stride, s);
+    if (s >= V) return;
+    const Mat3<T> mm = load_mat(m, s);
+    Vec3<T> vv[NSPIN], ww[NSPIN];
+    load_vecs<T, NSPIN>(v, s, vv);
 #pragma unroll
     for (int a = 0; a < NSPIN; ++a) {
-        Vec3<T> vv = load_vec(v, g.stride, s, a);
-        Vec3<T> ww;
 #pragma unroll
-        for (int i = 0; i < 3; ++i) ww.re[i] = ww.im[i] = T(0);
-        mac_mv(ww, mm, vv);
-        store_vec(w, g.stride, s, a, ww);
+        for (int i = 0; i < 3; ++i) ww[a].re[i] = ww[a].im[i] = T(0);
+        mac_mv(ww[a], mm, vv[a]);
     }
+    store_vecs<T, NSPIN>(w, s, ww);
 }
 
 // ---------------------------------------------------------------------------------------------
-// standalone reductions: fp64 accumulation per thread over a grid-stride loop with a FIXED grid,
-// then the deterministic block tree (lqx_internal.cuh) and the second stage (lqx_core.cu).
+// standalone reductions: one launch.  Each thread accumulates in fp64 over a grid-stride loop of
+// sites with a FIXED grid, then the deterministic block tree + last-block finish
+// (lqx_internal.cuh) writes the result straight into pinned host memory.
 // ---------------------------------------------------------------------------------------------
-template <typename T>
-__global__ void k_norm2(const __grid_constant__ Geo g, int nplanes, const T* __restrict__ f, double* __restrict__ partials) {
-    constexpr int W = VecWidth<T>::value;
-    typedef Pack<T, W> P;
+template <typename T, int NREAL>
+__global__ void __launch_bounds__(256) k_norm2(int V, const T* __restrict__ f, double* __restrict__ partials, unsigned int* ticket,
+                                               double* __restrict__ out) {
     double acc[1] = {0.0};
-    const int nv = g.V / W;  // full vectors per plane
     const int step = gridDim.x * blockDim.x;
-    for (int p = 0; p < nplanes; ++p) {
-        const T* base = f + (size_t)p * g.stride;
-        for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < nv; i += step) {
-            P v = reinterpret_cast<const P*>(base)[i];
+    for (int s = blockIdx.x * blockDim.x + threadIdx.x; s < V; s += step) {
+        T r[NREAL];
+        load_site<T, NREAL>(f, s, r);
+        double t0 = 0.0, t1 = 0.0;  // two chains per site object
 #pragma unroll
-            for (int j = 0; j < W; ++j) acc[0] = fma((double)v.v[j], (double)v.v[j], acc[0]);
+        for (int j = 0; j < NREAL; j += 2) {
+            t0 = fma((double)r[j], (double)r[j], t0);
+            t1 = fma((double)r[j + 1], (double)r[j + 1], t1);
         }
-        for (int i = nv * W + blockIdx.x * blockDim.x + threadIdx.x; i < g.V; i += step) {
-            double t = (double)base[i];
-            acc[0] = fma(t, t, acc[0]);
-        }
+        acc[0] += t0 + t1;
     }
-    block_reduce_store<1>(acc, partials, gridDim.x, blockIdx.x);
+    block_reduce_finish<1>(acc, partials, ticket, out);
 }
-// sum over sites of every plane -> NC = nplanes doubles
-template <typename T, int NC>
-__global__ void k_sum(const __grid_constant__ Geo g, const T* __restrict__ f, double* __restrict__ partials) {
-    double acc[NC];
+// sum over sites of the site object -> NREAL doubles in QDP order
+template <typename T, int NREAL>
+__global__ void __launch_bounds__(256) k_sum(int V, const T* __restrict__ f, double* __restrict__ partials, unsigned int* ticket,
+                                             double* __restrict__ out) {
+    double acc[NREAL];
 #pragma unroll
-    for (int c = 0; c < NC; ++c) acc[c] = 0.0;
+    for (int c = 0; c < NREAL; ++c) acc[c] = 0.0;
     const int step = gridDim.x * blockDim.x;
-    for (int s = blockIdx.x * blockDim.x + threadIdx.x; s < g.V; s += step) {
+    for (int s = blockIdx.x * blockDim.x + threadIdx.x; s < V; s += step) {
+        T r[NREAL];
+        load_site<T, NREAL>(f, s, r);
 #pragma unroll
-        for (int c = 0; c < NC; ++c) acc[c] += (double)__ldg(f + (size_t)c * g.stride + s);
+        for (int c = 0; c < NREAL; ++c) acc[c] += (double)r[c];
     }
-    block_reduce_store<NC>(acc, partials, gridDim.x, blockIdx.x);
+    block_reduce_finish<NREAL>(acc, partials, ticket, out);
 }
-// sum_x tr M(x): planes of the diagonal elements (0,0),(1,1),(2,2)
+// sum_x tr M(x): diagonal elements (0,0),(1,1),(2,2) = QDP reals 0,1 / 8,9 / 16,17
 template <typename T>
-__global__ void k_trace(const __grid_constant__ Geo g, const T* __restrict__ m, double* __restrict__ partials) {
+__global__ void __launch_bounds__(256) k_trace(int V, const T* __restrict__ m, double* __restrict__ partials, unsigned int* ticket,
+                                               double* __restrict__ out) {
+    typedef typename Vec128<T>::type V128;
+    constexpr int W = Vec128<T>::W;
     double acc[2] = {0.0, 0.0};
     const int step = gridDim.x * blockDim.x;
-    for (int s = blockIdx.x * blockDim.x + threadIdx.x; s < g.V; s += step) {
-#pragma unroll
-        for (int i = 0; i < 3; ++i) {
-            acc[0] += (double)__ldg(m + (size_t)(2 * (4 * i)) * g.stride + s);
-            acc[1] += (double)__ldg(m + (size_t)(2 * (4 * i) + 1) * g.stride + s);
+    for (int s = blockIdx.x * blockDim.x + threadIdx.x; s < V; s += step) {
+        // only the chunks that hold diagonal elements are touched: fp32 chunks 0, 2, 4; fp64 chunks 0, 4, 8
+        const T* blk = m + (size_t)(s >> 5) * (32 * 18);
+        const int lane = s & 31;
+        if (W == 4) {
+            T c0[W], c2[W];
+            unpack(__ldg(reinterpret_cast<const V128*>(blk) + lane), c0);
+            unpack(__ldg(reinterpret_cast<const V128*>(blk) + 2 * 32 + lane), c2);
+            const float2 c4 = __ldg(reinterpret_cast<const float2*>(blk + 4 * 32 * 4) + lane);
+            acc[0] += (double)c0[0] + (double)c2[0] + (double)c4.x;
+            acc[1] += (double)c0[1] + (double)c2[1] + (double)c4.y;
+        } else {
+            T d0[W], d1[W], d2[W];
+            unpack(__ldg(reinterpret_cast<const V128*>(blk) + lane), d0);
+            unpack(__ldg(reinterpret_cast<const V128*>(blk) + 4 * 32 + lane), d1);
+            unpack(__ldg(reinterpret_cast<const V128*>(blk) + 8 * 32 + lane), d2);
+            acc[0] += (double)d0[0] + (double)d1[0] + (double)d2[0];
+            acc[1] += (double)d0[1] + (double)d1[1] + (double)d2[1];
         }
     }
-    block_reduce_store<2>(acc, partials, gridDim.x, blockIdx.x);
+    block_reduce_finish<2>(acc, partials, ticket, out);
 }
 
-int reduce_grid(const lqx_ctx* ctx, int per_thread_items) {
+int reduce_grid(const lqx_ctx* ctx, int sites_per_thread) {
     // fixed function of V only => deterministic summation tree
-    long want = ((long)ctx->geo.V / per_thread_items + 255) / 256;
+    long want = ((long)ctx->geo.V / sites_per_thread + 255) / 256;
     long cap = (long)ctx->num_sms * 8;
     return (int)std::max<long>(1, std::min(want, cap));
 }
 
-template <typename T>
-int sum_launch(lqx_ctx* ctx, const lqx_field* f, int grid) {
-    const T* p = (const T*)f->data;
-    switch ((int)f->kind) {
-        case LQX_COMPLEX: k_sum<T, 2><<<grid, 256, 0, ctx->stream>>>(ctx->geo, p, ctx->d_partials); break;
-        case LQX_COLORVEC: k_sum<T, 6><<<grid, 256, 0, ctx->stream>>>(ctx->geo, p, ctx->d_partials); break;
-        case LQX_COLORMAT: k_sum<T, 18><<<grid, 256, 0, ctx->stream>>>(ctx->geo, p, ctx->d_partials); break;
-        default: k_sum<T, 24><<<grid, 256, 0, ctx->stream>>>(ctx->geo, p, ctx->d_partials); break;
+#define LQX_BY_KIND(KERNEL, T, kind, ...)                                                       \
+    switch ((int)(kind)) {                                                                      \
+        case LQX_COMPLEX: KERNEL<T, 2><<<grid, 256, 0, ctx->stream>>>(__VA_ARGS__); break;      \
+        case LQX_COLORVEC: KERNEL<T, 6><<<grid, 256, 0, ctx->stream>>>(__VA_ARGS__); break;     \
+        case LQX_COLORMAT: KERNEL<T, 18><<<grid, 256, 0, ctx->stream>>>(__VA_ARGS__); break;    \
+        default: KERNEL<T, 24><<<grid, 256, 0, ctx->stream>>>(__VA_ARGS__); break;              \
     }
-    LQX_LAUNCH_CHECK(ctx);
-    return LQX_OK;
-}
 
 }  // namespace
 
@@ -316,14 +299,13 @@ extern "C" int lqx_mm_plus_madj(lqx_field* r, const lqx_field* a, const lqx_fiel
     for (const lqx_field* f : {(const lqx_field*)r, a, b, c, d})
         if (f->kind != LQX_COLORMAT) return lqx_fail(ctx, LQX_ETYPE, "mm_plus_madj wants colour matrices");
     LQX_CUDA(ctx, cudaSetDevice(ctx->device));
-    const Geo& g = ctx->geo;
-    const int grid = (g.V + 127) / 128;
+    const int V = ctx->geo.V, grid = (V + 127) / 128;
     LqxTimed timed(ctx, LQX_K_CATALOGUE);
     if (r->prec == LQX_F32)
-        k_mm_plus_madj<float><<<grid, 128, 0, ctx->stream>>>(g, (const float*)a->data, (const float*)b->data,
+        k_mm_plus_madj<float><<<grid, 128, 0, ctx->stream>>>(V, (const float*)a->data, (const float*)b->data,
                                                             (const float*)c->data, (const float*)d->data, (float*)r->data);
     else
-        k_mm_plus_madj<double><<<grid, 128, 0, ctx->stream>>>(g, (const double*)a->data, (const double*)b->data,
+        k_mm_plus_madj<double><<<grid, 128, 0, ctx->stream>>>(V, (const double*)a->data, (const double*)b->data,
                                                              (const double*)c->data, (const double*)d->data, (double*)r->data);
     LQX_LAUNCH_CHECK(ctx);
     return LQX_OK;
@@ -336,13 +318,12 @@ extern "C" int lqx_trace_mm(lqx_field* c, const lqx_field* a, const lqx_field* b
     if (c->kind != LQX_COMPLEX || a->kind != LQX_COLORMAT || b->kind != LQX_COLORMAT)
         return lqx_fail(ctx, LQX_ETYPE, "trace_mm: complex = trace(matrix*matrix)");
     LQX_CUDA(ctx, cudaSetDevice(ctx->device));
-    const Geo& g = ctx->geo;
-    const int grid = (g.V + 127) / 128;
+    const int V = ctx->geo.V, grid = (V + 127) / 128;
     LqxTimed timed(ctx, LQX_K_CATALOGUE);
     if (c->prec == LQX_F32)
-        k_trace_mm<float><<<grid, 128, 0, ctx->stream>>>(g, (const float*)a->data, (const float*)b->data, (float*)c->data);
+        k_trace_mm<float><<<grid, 128, 0, ctx->stream>>>(V, (const float*)a->data, (const float*)b->data, (float*)c->data);
     else
-        k_trace_mm<double><<<grid, 128, 0, ctx->stream>>>(g, (const double*)a->data, (const double*)b->data, (double*)c->data);
+        k_trace_mm<double><<<grid, 128, 0, ctx->stream>>>(V, (const double*)a->data, (const double*)b->data, (double*)c->data);
     LQX_LAUNCH_CHECK(ctx);
     return LQX_OK;
 }
@@ -354,16 +335,15 @@ extern "C" int lqx_mat_vec(lqx_field* w, const lqx_field* m, const lqx_field* v)
     if (m->kind != LQX_COLORMAT || w->kind != v->kind || (v->kind != LQX_COLORVEC && v->kind != LQX_FERMION))
         return lqx_fail(ctx, LQX_ETYPE, "mat_vec: matrix * (colour vector | fermion)");
     LQX_CUDA(ctx, cudaSetDevice(ctx->device));
-    const Geo& g = ctx->geo;
-    const int grid = (g.V + 127) / 128;
+    const int V = ctx->geo.V, grid = (V + 127) / 128;
     LqxTimed timed(ctx, LQX_K_CATALOGUE);
     const bool ferm = v->kind == LQX_FERMION;
     if (w->prec == LQX_F32) {
-        if (ferm) k_mat_vec<float, 4><<<grid, 128, 0, ctx->stream>>>(g, (const float*)m->data, (const float*)v->data, (float*)w->data);
-        else k_mat_vec<float, 1><<<grid, 128, 0, ctx->stream>>>(g, (const float*)m->data, (const float*)v->data, (float*)w->data);
+        if (ferm) k_mat_vec<float, 4><<<grid, 128, 0, ctx->stream>>>(V, (const float*)m->data, (const float*)v->data, (float*)w->data);
+        else k_mat_vec<float, 1><<<grid, 128, 0, ctx->stream>>>(V, (const float*)m->data, (const float*)v->data, (float*)w->data);
     } else {
-        if (ferm) k_mat_vec<double, 4><<<grid, 128, 0, ctx->stream>>>(g, (const double*)m->data, (const double*)v->data, (double*)w->data);
-        else k_mat_vec<double, 1><<<grid, 128, 0, ctx->stream>>>(g, (const double*)m->data, (const double*)v->data, (double*)w->data);
+        if (ferm) k_mat_vec<double, 4><<<grid, 128, 0, ctx->stream>>>(V, (const double*)m->data, (const double*)v->data, (double*)w->data);
+        else k_mat_vec<double, 1><<<grid, 128, 0, ctx->stream>>>(V, (const double*)m->data, (const double*)v->data, (double*)w->data);
     }
     LQX_LAUNCH_CHECK(ctx);
     return LQX_OK;
@@ -373,17 +353,19 @@ extern "C" int lqx_norm2(const lqx_field* f, double* out) {
     if (!f || !out) return LQX_EINVAL;
     lqx_ctx* ctx = f->ctx;
     LQX_CUDA(ctx, cudaSetDevice(ctx->device));
-    const int grid = reduce_grid(ctx, 8);
+    const int grid = reduce_grid(ctx, 2);
     int rc = lqx_ensure_partials(ctx, (size_t)grid);
     if (rc) return rc;
+    const int V = ctx->geo.V;
     {
         LqxTimed timed(ctx, LQX_K_REDUCE);
-        if (f->prec == LQX_F32) k_norm2<float><<<grid, 256, 0, ctx->stream>>>(ctx->geo, 2 * (int)f->kind, (const float*)f->data, ctx->d_partials);
-        else k_norm2<double><<<grid, 256, 0, ctx->stream>>>(ctx->geo, 2 * (int)f->kind, (const double*)f->data, ctx->d_partials);
+        if (f->prec == LQX_F32) {
+            LQX_BY_KIND(k_norm2, float, f->kind, V, (const float*)f->data, ctx->d_partials, ctx->d_ticket, ctx->h_result)
+        } else {
+            LQX_BY_KIND(k_norm2, double, f->kind, V, (const double*)f->data, ctx->d_partials, ctx->d_ticket, ctx->h_result)
+        }
     }
     LQX_LAUNCH_CHECK(ctx);
-    rc = lqx_reduce_finish(ctx, grid, 1, ctx->d_result);
-    if (rc) return rc;
     return lqx_fetch_result(ctx, 1, out);
 }
 
@@ -392,16 +374,19 @@ extern "C" int lqx_sum(const lqx_field* f, double* out) {
     lqx_ctx* ctx = f->ctx;
     LQX_CUDA(ctx, cudaSetDevice(ctx->device));
     const int nc = 2 * (int)f->kind;
-    const int grid = reduce_grid(ctx, 4);
+    const int grid = reduce_grid(ctx, 2);
     int rc = lqx_ensure_partials(ctx, (size_t)grid * nc);
     if (rc) return rc;
+    const int V = ctx->geo.V;
     {
         LqxTimed timed(ctx, LQX_K_REDUCE);
-        rc = f->prec == LQX_F32 ? sum_launch<float>(ctx, f, grid) : sum_launch<double>(ctx, f, grid);
+        if (f->prec == LQX_F32) {
+            LQX_BY_KIND(k_sum, float, f->kind, V, (const float*)f->data, ctx->d_partials, ctx->d_ticket, ctx->h_result)
+        } else {
+            LQX_BY_KIND(k_sum, double, f->kind, V, (const double*)f->data, ctx->d_partials, ctx->d_ticket, ctx->h_result)
+        }
     }
-    if (rc) return rc;
-    rc = lqx_reduce_finish(ctx, grid, nc, ctx->d_result);
-    if (rc) return rc;
+    LQX_LAUNCH_CHECK(ctx);
     return lqx_fetch_result(ctx, nc, out);
 }
 
@@ -410,16 +395,15 @@ extern "C" int lqx_trace(const lqx_field* m, double out[2]) {
     lqx_ctx* ctx = m->ctx;
     if (m->kind != LQX_COLORMAT) return lqx_fail(ctx, LQX_ETYPE, "trace wants a colour matrix");
     LQX_CUDA(ctx, cudaSetDevice(ctx->device));
-    const int grid = reduce_grid(ctx, 4);
+    const int grid = reduce_grid(ctx, 2);
     int rc = lqx_ensure_partials(ctx, (size_t)grid * 2);
     if (rc) return rc;
+    const int V = ctx->geo.V;
     {
         LqxTimed timed(ctx, LQX_K_REDUCE);
-        if (m->prec == LQX_F32) k_trace<float><<<grid, 256, 0, ctx->stream>>>(ctx->geo, (const float*)m->data, ctx->d_partials);
-        else k_trace<double><<<grid, 256, 0, ctx->stream>>>(ctx->geo, (const double*)m->data, ctx->d_partials);
+        if (m->prec == LQX_F32) k_trace<float><<<grid, 256, 0, ctx->stream>>>(V, (const float*)m->data, ctx->d_partials, ctx->d_ticket, ctx->h_result);
+        else k_trace<double><<<grid, 256, 0, ctx->stream>>>(V, (const double*)m->data, ctx->d_partials, ctx->d_ticket, ctx->h_result);
     }
     LQX_LAUNCH_CHECK(ctx);
-    rc = lqx_reduce_finish(ctx, grid, 2, ctx->d_result);
-    if (rc) return rc;
     return lqx_fetch_result(ctx, 2, out);
 }

@@ -1,11 +1,12 @@
 // lqx internal declarations: context / field handles, lattice geometry with in-kernel periodic
-// neighbour arithmetic, SoA addressing (a2) and the site algebra used by every
+// neighbour arithmetic, blocked-SoA addressing (a2) and the site algebra used by every
 // kernel (sec.4 types; operators of Listing 1).
 // Shares nothing with oracle/.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <algorithm>
 #include <string>
 #include <utility>
 #include <vector>
@@ -25,7 +26,7 @@ struct Geo {  // passed by value to kernels
     int L[4];
     int stride_site[4];  // 1, L0, L0*L1, L0*L1*L2
     int V;
-    int stride;  // plane stride in elements (V rounded up to 32)
+    int Vpad;    // V rounded up to a whole number of 32-site blocks
     FastDiv d0, d1, d2;
 };
 
@@ -37,12 +38,14 @@ struct lqx_ctx {
     std::vector<lqx_field*> fields;
     double* d_partials;  // reduction scratch
     size_t partials_cap; // in doubles
-    double* d_result;    // 64 doubles
-    double* h_result;    // pinned, 64 doubles
+    double* d_result;    // 64 doubles (device scratch results)
+    double* h_result;    // pinned + mapped, 64 doubles: kernels write results straight to the host
+    unsigned int* d_ticket;  // last-block ticket of the one-launch reductions (zero between launches)
     int64_t launches;
     int num_sms;
     int opt_smear_variant;
     int opt_block;
+    int opt_tile;  // -1 = automatic, 0 = Linear, 1..3 = TileA..TileC (lqx_smear.cuh)
     // optional per-kernel-class device timing (bench harness): cudaEvent pairs on the stream
     bool timing;
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> timers[LQX_NUM_KERNEL_CLASSES];
@@ -78,10 +81,7 @@ struct lqx_field {
 int lqx_fail(lqx_ctx* ctx, int code, const char* what);
 int lqx_cuda_fail(lqx_ctx* ctx, cudaError_t e, const char* where);
 int lqx_ensure_partials(lqx_ctx* ctx, size_t ndoubles);
-// second stage of every reduction: sums nblocks partials of ncomp doubles (layout
-// partials[comp*nblocks + b]) into d_out[0 .. ncomp) (device memory, e.g. ctx->d_result)
-int lqx_reduce_finish(lqx_ctx* ctx, int nblocks, int ncomp, double* d_out);
-// copies ctx->d_result[0..n) to host `out` and synchronises the stream
+// synchronises the stream and copies ctx->h_result[0..n) (written by a reduction kernel) to `out`
 int lqx_fetch_result(lqx_ctx* ctx, int n, double* out);
 
 #define LQX_CUDA(ctx, call)                                              \
@@ -129,8 +129,78 @@ __device__ __forceinline__ int nbr_bwd(const Geo& g, int s, const int x[4], int 
 }
 
 // --------------------------------------------------------------------------------------------
-// device side: site algebra on SoA planes.  T = float or double.
-// Colour matrix element (i,j): planes 2*(3*i+j) (re) and 2*(3*i+j)+1 (im).
+// device side: the field store's internal layout -- blocked site-fastest SoA.
+//
+// Sites are grouped in blocks of 32 consecutive lexicographic sites (one warp).  Inside a block
+// the NREAL reals of a site object (QDP order, lqx.h) are cut into 128-bit chunks of
+// W = 16/sizeof(T) reals (4 floats / 2 doubles); chunk q of all 32 sites is contiguous:
+//
+//     offset(site s, real r) = (s>>5)*32*NREAL + q*32*W + (s&31)*w_q + (r - q*W),   q = r / W,
+//     w_q = W for the NREAL/W full chunks, and 2 for the trailing half chunk (fp32, NREAL%4 == 2).
+//
+// So a warp reading one chunk of 32 consecutive sites issues ONE 128-bit load per lane over 512
+// contiguous bytes, a whole colour matrix is 5 (fp32) / 9 (fp64) loads from ONE computed address
+// plus immediates, and a field is exactly as large as in plain SoA (Vpad*NREAL reals).
+// --------------------------------------------------------------------------------------------
+template <typename T>
+struct Vec128;
+template <>
+struct Vec128<float> {
+    typedef float4 type;
+    static constexpr int W = 4;
+};
+template <>
+struct Vec128<double> {
+    typedef double2 type;
+    static constexpr int W = 2;
+};
+
+__device__ __forceinline__ void unpack(const float4& v, float* r) { r[0] = v.x; r[1] = v.y; r[2] = v.z; r[3] = v.w; }
+__device__ __forceinline__ void unpack(const double2& v, double* r) { r[0] = v.x; r[1] = v.y; }
+__device__ __forceinline__ float4 pack(const float* r) { return make_float4(r[0], r[1], r[2], r[3]); }
+__device__ __forceinline__ double2 pack(const double* r) { return make_double2(r[0], r[1]); }
+
+// element offset of (site s, real r) for a field of nreal reals per site, W reals per 128 bits
+__host__ __device__ __forceinline__ size_t lqx_layout_offset(int s, int r, int nreal, int W) {
+    const int nfull = nreal / W;
+    const int q = r / W < nfull ? r / W : nfull;
+    const int wq = q < nfull ? W : nreal - nfull * W;
+    return (size_t)(s >> 5) * 32 * nreal + (size_t)q * 32 * W + (size_t)(s & 31) * wq + (r - q * W);
+}
+
+// all NREAL reals of site s (read-only path)
+template <typename T, int NREAL>
+__device__ __forceinline__ void load_site(const T* __restrict__ base, int s, T (&r)[NREAL]) {
+    typedef typename Vec128<T>::type V;
+    constexpr int W = Vec128<T>::W, NFULL = NREAL / W;
+    const T* blk = base + (size_t)(s >> 5) * (32 * NREAL);
+    const int lane = s & 31;
+    const V* p = reinterpret_cast<const V*>(blk) + lane;
+#pragma unroll
+    for (int q = 0; q < NFULL; ++q) unpack(__ldg(p + q * 32), &r[q * W]);
+    if (NREAL % W != 0) {  // fp32 only: trailing (re,im) pair
+        const float2 t = __ldg(reinterpret_cast<const float2*>(blk + NFULL * 32 * W) + lane);
+        r[NFULL * W] = (T)t.x;
+        r[NFULL * W + 1] = (T)t.y;
+    }
+}
+template <typename T, int NREAL>
+__device__ __forceinline__ void store_site(T* __restrict__ base, int s, const T (&r)[NREAL]) {
+    typedef typename Vec128<T>::type V;
+    constexpr int W = Vec128<T>::W, NFULL = NREAL / W;
+    T* blk = base + (size_t)(s >> 5) * (32 * NREAL);
+    const int lane = s & 31;
+    V* p = reinterpret_cast<V*>(blk) + lane;
+#pragma unroll
+    for (int q = 0; q < NFULL; ++q) p[q * 32] = pack(&r[q * W]);
+    if (NREAL % W != 0) {
+        reinterpret_cast<float2*>(blk + NFULL * 32 * W)[lane] = make_float2((float)r[NFULL * W], (float)r[NFULL * W + 1]);
+    }
+}
+
+// --------------------------------------------------------------------------------------------
+// device side: site algebra.  T = float or double.
+// Colour matrix element (i,j): QDP-order reals 2*(3*i+j) (re) and 2*(3*i+j)+1 (im).
 // --------------------------------------------------------------------------------------------
 template <typename T>
 struct Mat3 {
@@ -142,45 +212,55 @@ struct Vec3 {
 };
 
 template <typename T>
-__device__ __forceinline__ Mat3<T> load_mat(const T* __restrict__ p, int stride, int s) {
+__device__ __forceinline__ Mat3<T> load_mat(const T* __restrict__ p, int s) {
+    T r[18];
+    load_site<T, 18>(p, s, r);
     Mat3<T> m;
 #pragma unroll
     for (int i = 0; i < 3; ++i)
 #pragma unroll
         for (int j = 0; j < 3; ++j) {
-            m.re[i][j] = __ldg(p + (size_t)(2 * (3 * i + j)) * stride + s);
-            m.im[i][j] = __ldg(p + (size_t)(2 * (3 * i + j) + 1) * stride + s);
+            m.re[i][j] = r[2 * (3 * i + j)];
+            m.im[i][j] = r[2 * (3 * i + j) + 1];
         }
     return m;
 }
 template <typename T>
-__device__ __forceinline__ void store_mat(T* __restrict__ p, int stride, int s, const Mat3<T>& m) {
+__device__ __forceinline__ void store_mat(T* __restrict__ p, int s, const Mat3<T>& m) {
+    T r[18];
 #pragma unroll
     for (int i = 0; i < 3; ++i)
 #pragma unroll
         for (int j = 0; j < 3; ++j) {
-            p[(size_t)(2 * (3 * i + j)) * stride + s] = m.re[i][j];
-            p[(size_t)(2 * (3 * i + j) + 1) * stride + s] = m.im[i][j];
+            r[2 * (3 * i + j)] = m.re[i][j];
+            r[2 * (3 * i + j) + 1] = m.im[i][j];
+        }
+    store_site<T, 18>(p, s, r);
+}
+// NSPIN colour vectors of one site (NSPIN = 1: LatticeColorVector, 4: LatticeFermion)
+template <typename T, int NSPIN>
+__device__ __forceinline__ void load_vecs(const T* __restrict__ p, int s, Vec3<T> (&v)[NSPIN]) {
+    T r[6 * NSPIN];
+    load_site<T, 6 * NSPIN>(p, s, r);
+#pragma unroll
+    for (int a = 0; a < NSPIN; ++a)
+#pragma unroll
+        for (int i = 0; i < 3; ++i) {
+            v[a].re[i] = r[2 * (3 * a + i)];
+            v[a].im[i] = r[2 * (3 * a + i) + 1];
         }
 }
-// vector `a` of nspin-component field: planes 2*(3*a+i)+c
-template <typename T>
-__device__ __forceinline__ Vec3<T> load_vec(const T* __restrict__ p, int stride, int s, int a) {
-    Vec3<T> v;
+template <typename T, int NSPIN>
+__device__ __forceinline__ void store_vecs(T* __restrict__ p, int s, const Vec3<T> (&v)[NSPIN]) {
+    T r[6 * NSPIN];
 #pragma unroll
-    for (int i = 0; i < 3; ++i) {
-        v.re[i] = __ldg(p + (size_t)(2 * (3 * a + i)) * stride + s);
-        v.im[i] = __ldg(p + (size_t)(2 * (3 * a + i) + 1) * stride + s);
-    }
-    return v;
-}
-template <typename T>
-__device__ __forceinline__ void store_vec(T* __restrict__ p, int stride, int s, int a, const Vec3<T>& v) {
+    for (int a = 0; a < NSPIN; ++a)
 #pragma unroll
-    for (int i = 0; i < 3; ++i) {
-        p[(size_t)(2 * (3 * a + i)) * stride + s] = v.re[i];
-        p[(size_t)(2 * (3 * a + i) + 1) * stride + s] = v.im[i];
-    }
+        for (int i = 0; i < 3; ++i) {
+            r[2 * (3 * a + i)] = v[a].re[i];
+            r[2 * (3 * a + i) + 1] = v[a].im[i];
+        }
+    store_site<T, 6 * NSPIN>(p, s, r);
 }
 
 // C = A*B        (AB)_ij = sum_k A_ik B_kj
@@ -336,16 +416,24 @@ __device__ __forceinline__ void mac_adj_mv(Vec3<T>& w, const Mat3<T>& m, const V
 }
 
 // --------------------------------------------------------------------------------------------
-// device side: deterministic block reduction of NC doubles per thread.
-// warp shuffle tree -> shared memory across warps -> thread 0 writes partials[c*nblocks + block].
+// device side: deterministic reduction of NC doubles per thread in ONE launch.
+// warp shuffle tree -> shared memory across warps -> partials[c*nblocks + block]; the block that
+// takes the last ticket sums the partials in a fixed order and writes out[0..NC).  The grid is a
+// fixed function of the lattice, so the summation tree (and the result) is the same run to run.
+// `out` may be device memory or pinned host memory (UVA).
 // --------------------------------------------------------------------------------------------
 template <int NC>
-__device__ __forceinline__ void block_reduce_store(double (&v)[NC], double* __restrict__ partials,
-                                                   int nblocks, int block) {
+__device__ __forceinline__ void block_reduce_finish(double (&v)[NC], double* __restrict__ partials,
+                                                    unsigned int* __restrict__ ticket, double* __restrict__ out) {
     __shared__ double sh[32][NC + (NC % 2 == 0 ? 1 : 0)];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int nwarps = (blockDim.x + 31) >> 5;
-    __syncthreads();  // the buffer may be reused by a second call in the same kernel
+    __shared__ bool last;
+    const int tid = threadIdx.x + blockDim.x * (threadIdx.y + blockDim.y * threadIdx.z);
+    const int nthreads = blockDim.x * blockDim.y * blockDim.z;
+    const int lane = tid & 31, warp = tid >> 5;
+    const int nwarps = (nthreads + 31) >> 5;
+    const int nblocks = gridDim.x * gridDim.y * gridDim.z;
+    const int block = blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z);
+    __syncthreads();
 #pragma unroll
     for (int c = 0; c < NC; ++c) {
         double t = v[c];
@@ -362,5 +450,98 @@ __device__ __forceinline__ void block_reduce_store(double (&v)[NC], double* __re
             for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
             if (lane == 0) partials[(size_t)c * nblocks + block] = t;
         }
+        if (lane == 0) {
+            __threadfence();
+            last = (atomicAdd(ticket, 1u) == (unsigned)(nblocks - 1));
+        }
     }
+    __syncthreads();
+    if (!last) return;
+    __threadfence();
+    for (int c = 0; c < NC; ++c) {
+        double t = 0.0;
+        for (int i = tid; i < nblocks; i += nthreads) t += __ldcg(partials + (size_t)c * nblocks + i);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+        __syncthreads();
+        if (lane == 0) sh[warp][0] = t;
+        __syncthreads();
+        if (warp == 0) {
+            t = (lane < nwarps) ? sh[lane][0] : 0.0;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+            if (lane == 0) out[c] = t;
+        }
+    }
+    if (tid == 0) *ticket = 0u;  // ready for the next launch on this stream
 }
+
+// --------------------------------------------------------------------------------------------
+// device side: CTA -> sites maps of the nearest-neighbour kernels (hop, plaquette, smear).
+//
+// Tiled<TX,TY,TZ,TT>: a CTA owns a compact 4-d tile (one thread per site, x fastest inside the
+//   tile) so that the neighbour operands its threads share are served by L1.  Tiles are visited
+//   x, y, z fastest inside a slab of `zs` z-tiles, then t, then the next slab: the +-t neighbour
+//   slices of a slab (a few MB) are still in L2 when they are needed again, and only the two
+//   z-faces of a slab are re-read from HBM.
+// Linear: generic fallback for extents no tile shape divides: 128 consecutive lexicographic sites.
+// --------------------------------------------------------------------------------------------
+struct TileMap {
+    int nt[4];  // tiles per direction
+    int zs;     // z-tiles per slab
+};
+
+template <int TX, int TY, int TZ, int TT>
+struct Tiled {
+    static constexpr int THREADS = TX * TY * TZ * TT;
+    static constexpr int T0 = TX, T1 = TY, T2 = TZ, T3 = TT;
+    __device__ static __forceinline__ bool site(const Geo& g, const TileMap& m, int x[4], int& s) {
+        const int id = blockIdx.x;
+        const int n01 = m.nt[0] * m.nt[1];
+        const int per_slab = n01 * m.zs * m.nt[3];
+        const int k = id / per_slab;
+        int rem = id - k * per_slab;
+        const int zsk = min(m.zs, m.nt[2] - k * m.zs);
+        const int slice = n01 * zsk;
+        const int tt = rem / slice;
+        rem -= tt * slice;
+        const int tz = rem / n01;
+        rem -= tz * n01;
+        const int ty = rem / m.nt[0];
+        const int tx = rem - ty * m.nt[0];
+        const int l = threadIdx.x;
+        x[0] = tx * TX + (l % TX);
+        x[1] = ty * TY + (l / TX) % TY;
+        x[2] = (tz + k * m.zs) * TZ + (l / (TX * TY)) % TZ;
+        x[3] = tt * TT + l / (TX * TY * TZ);
+        s = x[0] + g.L[0] * (x[1] + g.L[1] * (x[2] + g.L[2] * x[3]));
+        return true;
+    }
+    static bool fits(const Geo& g) { return g.L[0] % TX == 0 && g.L[1] % TY == 0 && g.L[2] % TZ == 0 && g.L[3] % TT == 0; }
+    static int grid(const Geo& g) { return (g.L[0] / TX) * (g.L[1] / TY) * (g.L[2] / TZ) * (g.L[3] / TT); }
+    static TileMap map(const Geo& g, int slab_sites_z) {
+        TileMap m;
+        m.nt[0] = g.L[0] / TX;
+        m.nt[1] = g.L[1] / TY;
+        m.nt[2] = g.L[2] / TZ;
+        m.nt[3] = g.L[3] / TT;
+        m.zs = std::max(1, std::min(m.nt[2], slab_sites_z / TZ));
+        return m;
+    }
+};
+
+struct Linear {
+    static constexpr int THREADS = 128;
+    __device__ static __forceinline__ bool site(const Geo& g, const TileMap&, int x[4], int& s) {
+        s = blockIdx.x * THREADS + threadIdx.x;
+        if (s >= g.V) return false;
+        site_coords(g, s, x);
+        return true;
+    }
+    static bool fits(const Geo&) { return true; }
+    static int grid(const Geo& g) { return (g.V + THREADS - 1) / THREADS; }
+    static TileMap map(const Geo&, int) {
+        TileMap m = {{0, 0, 0, 0}, 1};
+        return m;
+    }
+};

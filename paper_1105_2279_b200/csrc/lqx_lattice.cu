@@ -1,32 +1,24 @@
-// lqx nearest-neighbour kernels: hop, plaquette (a8), staple sum + smear step (a7)
-// and the iterated smearing driver (a10).  Each is a single pass in which one thread evaluates the
-// whole expression of its site, reading shifted operands at the periodic
-// neighbour computed in-kernel (the role of the paper's site tables).
+// lqx nearest-neighbour kernels: hop, plaquette (a8), literal staple sum + smear
+// step (a7) and the iterated smearing driver (a10).  Each is a single pass in which one thread
+// evaluates the whole expression of its site, reading shifted operands at
+// the periodic neighbour computed in-kernel (the role of the paper's site tables).
+// CTAs own compact 4-d tiles (lqx_internal.cuh, Tiled<>) so that shared neighbours are L1 hits.
 #include "lqx_internal.cuh"
+#include "lqx_smear.cuh"
 
 namespace {
-
-template <typename T>
-struct Links {
-    const T* u[4];
-};
-template <typename T>
-struct LinksOut {
-    T* u[4];
-};
 
 // ---------------------------------------------------------------------------------------------
 // hop: chi(x) = sum_mu U_mu(x) psi(x+mu^) + adj(U_mu(x-mu^)) psi(x-mu^)
 // (Listing 1 lines 25/27 summed over mu; Eq. 2; BASELINE configs[1])
 // ---------------------------------------------------------------------------------------------
-template <typename T, int NSPIN, bool NORM2>
-__global__ void __launch_bounds__(128) k_hop(const __grid_constant__ Geo g, const __grid_constant__ Links<T> u, const T* __restrict__ psi, T* __restrict__ chi,
-                                             double* __restrict__ partials) {
-    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+template <typename T, int NSPIN, bool NORM2, typename MAP>
+__global__ void __launch_bounds__(MAP::THREADS) k_hop(const __grid_constant__ Geo g, const __grid_constant__ TileMap tm,
+                                                      const __grid_constant__ Links<T> u, const T* __restrict__ psi, T* __restrict__ chi,
+                                                      double* __restrict__ partials, unsigned int* ticket, double* __restrict__ out) {
+    int x[4], s;
     double n2[1] = {0.0};
-    if (s < g.V) {
-        int x[4];
-        site_coords(g, s, x);
+    if (MAP::site(g, tm, x, s)) {
         Vec3<T> acc[NSPIN];
 #pragma unroll
         for (int a = 0; a < NSPIN; ++a)
@@ -36,83 +28,86 @@ __global__ void __launch_bounds__(128) k_hop(const __grid_constant__ Geo g, cons
         for (int mu = 0; mu < 4; ++mu) {
             const int f = nbr_fwd(g, s, x, mu), b = nbr_bwd(g, s, x, mu);
             {
-                Mat3<T> m = load_mat(u.u[mu], g.stride, s);
+                const Mat3<T> m = load_mat(u.u[mu], s);
+                Vec3<T> v[NSPIN];
+                load_vecs<T, NSPIN>(psi, f, v);
 #pragma unroll
-                for (int a = 0; a < NSPIN; ++a) mac_mv(acc[a], m, load_vec(psi, g.stride, f, a));
+                for (int a = 0; a < NSPIN; ++a) mac_mv(acc[a], m, v[a]);
             }
             {
-                Mat3<T> m = load_mat(u.u[mu], g.stride, b);
+                const Mat3<T> m = load_mat(u.u[mu], b);
+                Vec3<T> v[NSPIN];
+                load_vecs<T, NSPIN>(psi, b, v);
 #pragma unroll
-                for (int a = 0; a < NSPIN; ++a) mac_adj_mv(acc[a], m, load_vec(psi, g.stride, b, a));
+                for (int a = 0; a < NSPIN; ++a) mac_adj_mv(acc[a], m, v[a]);
             }
         }
+        store_vecs<T, NSPIN>(chi, s, acc);
+        if (NORM2) {
 #pragma unroll
-        for (int a = 0; a < NSPIN; ++a) {
-            store_vec(chi, g.stride, s, a, acc[a]);
-            if (NORM2) {
+            for (int a = 0; a < NSPIN; ++a)
 #pragma unroll
                 for (int i = 0; i < 3; ++i) {
                     n2[0] = fma((double)acc[a].re[i], (double)acc[a].re[i], n2[0]);
                     n2[0] = fma((double)acc[a].im[i], (double)acc[a].im[i], n2[0]);
                 }
-            }
         }
     }
-    if (NORM2) block_reduce_store<1>(n2, partials, gridDim.x, blockIdx.x);
+    if (NORM2) block_reduce_finish<1>(n2, partials, ticket, out);
 }
 
 // ---------------------------------------------------------------------------------------------
 // plaquette: sum_{mu<nu} Re tr[U_mu(x) U_nu(x+mu^) adj(U_mu(x+nu^)) adj(U_nu(x))]
 //          = sum_{mu<nu} Re tr[Q_munu(x) adj(Q_numu(x))],  Q_ab(x) = U_a(x) U_b(x+a^)
 // ---------------------------------------------------------------------------------------------
-template <typename T>
-__global__ void __launch_bounds__(128) k_plaquette(const __grid_constant__ Geo g, const __grid_constant__ Links<T> u, double* __restrict__ partials) {
-    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+template <typename T, typename MAP>
+__global__ void __launch_bounds__(MAP::THREADS) k_plaquette(const __grid_constant__ Geo g, const __grid_constant__ TileMap tm,
+                                                            const __grid_constant__ Links<T> u, double* __restrict__ partials,
+                                                            unsigned int* ticket, double* __restrict__ out) {
+    int x[4], s;
     double p[1] = {0.0};
-    if (s < g.V) {
-        int x[4];
-        site_coords(g, s, x);
+    if (MAP::site(g, tm, x, s)) {
         T acc = T(0);
 #pragma unroll 1
         for (int mu = 0; mu < 3; ++mu) {
-            const Mat3<T> a = load_mat(u.u[mu], g.stride, s);
+            const Mat3<T> a = load_mat(u.u[mu], s);
             const int xpmu = nbr_fwd(g, s, x, mu);
 #pragma unroll 1
             for (int nu = mu + 1; nu < 4; ++nu) {
                 const int xpnu = nbr_fwd(g, s, x, nu);
-                Mat3<T> q1 = mul_nn(a, load_mat(u.u[nu], g.stride, xpmu));
-                Mat3<T> q2 = mul_nn(load_mat(u.u[nu], g.stride, s), load_mat(u.u[mu], g.stride, xpnu));
+                const Mat3<T> q1 = mul_nn(a, load_mat(u.u[nu], xpmu));
+                const Mat3<T> q2 = mul_nn(load_mat(u.u[nu], s), load_mat(u.u[mu], xpnu));
                 acc += re_tr_na(q1, q2);
             }
         }
         p[0] = (double)acc;
     }
-    block_reduce_store<1>(p, partials, gridDim.x, blockIdx.x);
+    block_reduce_finish<1>(p, partials, ticket, out);
 }
 
 // ---------------------------------------------------------------------------------------------
-// staple sum + smear step, literal gather form (variant 1): one thread per site, mu and nu loops
-// inside; every staple is a chain of two products kept in registers.
+// staple sum + smear step, literal gather form: one thread per site, mu and nu loops inside;
+// every staple is a chain of two products kept in registers (48 products per site).
 //   S_mu(x) = sum_{nu!=mu} U_nu(x) U_mu(x+nu^) adj(U_nu(x+mu^)) + adj(U_nu(x-nu^)) U_mu(x-nu^) U_nu(x-nu^+mu^)
 //   U'_mu(x) = c0 U_mu(x) + c1 S_mu(x)
 // PLAQ: the plaquette of the INPUT field is accumulated on the way:
 //   Re tr[U_mu U_nu(x+mu) adj(U_mu(x+nu)) adj(U_nu)] = Re tr[U_mu(x) adj(upper staple_{mu,nu}(x))], mu<nu.
-// ONLY_MU >= 0: write the bare staple sum of that direction into out.u[0] (diagnostic entry).
+// only_mu >= 0: write the bare staple sum of that direction into out.u[0] (diagnostic entry).
 // ---------------------------------------------------------------------------------------------
-template <typename T, bool PLAQ>
-__global__ void __launch_bounds__(128) k_smear_gather(const __grid_constant__ Geo g, const __grid_constant__ Links<T> u, const __grid_constant__ LinksOut<T> out, T c0, T c1, int only_mu,
-                                                      double* __restrict__ partials) {
-    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+template <typename T, bool PLAQ, typename MAP>
+__global__ void __launch_bounds__(MAP::THREADS) k_smear_gather(const __grid_constant__ Geo g, const __grid_constant__ TileMap tm,
+                                                               const __grid_constant__ Links<T> u, const __grid_constant__ LinksOut<T> out,
+                                                               T c0, T c1, int only_mu, double* __restrict__ partials,
+                                                               unsigned int* ticket, double* __restrict__ red_out) {
+    int x[4], s;
     double p[1] = {0.0};
-    if (s < g.V) {
-        int x[4];
-        site_coords(g, s, x);
+    if (MAP::site(g, tm, x, s)) {
         T pl = T(0);
         const int mu_lo = only_mu >= 0 ? only_mu : 0, mu_hi = only_mu >= 0 ? only_mu + 1 : 4;
 #pragma unroll 1
         for (int mu = mu_lo; mu < mu_hi; ++mu) {
             const int xpmu = nbr_fwd(g, s, x, mu);
-            const Mat3<T> umu = load_mat(u.u[mu], g.stride, s);
+            const Mat3<T> umu = load_mat(u.u[mu], s);
             Mat3<T> acc = zero_mat<T>();
 #pragma unroll 1
             for (int nu = 0; nu < 4; ++nu) {
@@ -122,9 +117,9 @@ __global__ void __launch_bounds__(128) k_smear_gather(const __grid_constant__ Ge
                 // x - nu^ + mu^ : step forward in mu from xmnu (coordinates differ from x only in nu)
                 const int xmnupmu = xmnu + (xpmu - s);
                 {
-                    Mat3<T> t = mul_nn(load_mat(u.u[nu], g.stride, s), load_mat(u.u[mu], g.stride, xpnu));
+                    const Mat3<T> t = mul_nn(load_mat(u.u[nu], s), load_mat(u.u[mu], xpnu));
                     if (PLAQ && mu < nu) {
-                        Mat3<T> up = mul_na(t, load_mat(u.u[nu], g.stride, xpmu));
+                        const Mat3<T> up = mul_na(t, load_mat(u.u[nu], xpmu));
                         pl += re_tr_na(umu, up);
 #pragma unroll
                         for (int i = 0; i < 3; ++i)
@@ -134,16 +129,16 @@ __global__ void __launch_bounds__(128) k_smear_gather(const __grid_constant__ Ge
                                 acc.im[i][j] += up.im[i][j];
                             }
                     } else {
-                        mac_na(acc, t, load_mat(u.u[nu], g.stride, xpmu));
+                        mac_na(acc, t, load_mat(u.u[nu], xpmu));
                     }
                 }
                 {
-                    Mat3<T> t = mul_an(load_mat(u.u[nu], g.stride, xmnu), load_mat(u.u[mu], g.stride, xmnu));
-                    mac_nn(acc, t, load_mat(u.u[nu], g.stride, xmnupmu));
+                    const Mat3<T> t = mul_an(load_mat(u.u[nu], xmnu), load_mat(u.u[mu], xmnu));
+                    mac_nn(acc, t, load_mat(u.u[nu], xmnupmu));
                 }
             }
             if (only_mu >= 0) {
-                store_mat(out.u[0], g.stride, s, acc);
+                store_mat(out.u[0], s, acc);
             } else {
                 Mat3<T> r;
 #pragma unroll
@@ -153,12 +148,12 @@ __global__ void __launch_bounds__(128) k_smear_gather(const __grid_constant__ Ge
                         r.re[i][j] = fma(c1, acc.re[i][j], c0 * umu.re[i][j]);
                         r.im[i][j] = fma(c1, acc.im[i][j], c0 * umu.im[i][j]);
                     }
-                store_mat(out.u[mu], g.stride, s, r);
+                store_mat(out.u[mu], s, r);
             }
         }
         p[0] = (double)pl;
     }
-    if (PLAQ) block_reduce_store<1>(p, partials, gridDim.x, blockIdx.x);
+    if (PLAQ) block_reduce_finish<1>(p, partials, ticket, red_out);
 }
 
 int check_links(lqx_ctx** ctx_out, const lqx_field* const u[4]) {
@@ -175,61 +170,79 @@ int check_links(lqx_ctx** ctx_out, const lqx_field* const u[4]) {
     return LQX_OK;
 }
 
-template <typename T>
-Links<T> make_links(const lqx_field* const u[4]) {
-    Links<T> l;
-    for (int mu = 0; mu < 4; ++mu) l.u[mu] = (const T*)u[mu]->data;
-    return l;
-}
+// z-extent (sites) of a slab of the tile visiting order: thick enough that the two re-read z-faces
+// are a small fraction, thin enough that three t-slices of a slab stay in L2
+const int kSlabZ = 16;
 
 template <typename T>
-int plaquette_launch(lqx_ctx* ctx, const lqx_field* const u[4], double* d_out) {
+int plaquette_launch(lqx_ctx* ctx, const lqx_field* const u[4], double* out) {
     const Geo& g = ctx->geo;
-    const int grid = (g.V + 127) / 128;
-    int rc = lqx_ensure_partials(ctx, (size_t)grid);
-    if (rc) return rc;
-    {
-        LqxTimed timed(ctx, LQX_K_PLAQUETTE);
-        k_plaquette<T><<<grid, 128, 0, ctx->stream>>>(g, make_links<T>(u), ctx->d_partials);
-    }
-    LQX_LAUNCH_CHECK(ctx);
-    return lqx_reduce_finish(ctx, grid, 1, d_out);
-}
-
-// one smear step on the stream; if d_plaq != nullptr the input plaquette sum lands there
-template <typename T>
-int smear_launch(lqx_ctx* ctx, lqx_field* const uout[4], const lqx_field* const uin[4], double alpha, int only_mu,
-                 double* d_plaq) {
-    const Geo& g = ctx->geo;
-    const int grid = (g.V + 127) / 128;
-    LinksOut<T> o;
-    for (int mu = 0; mu < 4; ++mu) o.u[mu] = uout[mu] ? (T*)uout[mu]->data : nullptr;
-    const T c0 = (T)(1.0 - alpha), c1 = (T)(alpha / 6.0);
-    if (d_plaq) {
+    const int choice = lqx_pick_tile(ctx, 1);
+    LQX_WITH_MAP(choice, {
+        const int grid = MAP::grid(g);
         int rc = lqx_ensure_partials(ctx, (size_t)grid);
         if (rc) return rc;
-        {
-            LqxTimed timed(ctx, LQX_K_SMEAR);
-            k_smear_gather<T, true><<<grid, 128, 0, ctx->stream>>>(g, make_links<T>(uin), o, c0, c1, only_mu, ctx->d_partials);
-        }
-        LQX_LAUNCH_CHECK(ctx);
-        return lqx_reduce_finish(ctx, grid, 1, d_plaq);
-    }
-    {
-        LqxTimed timed(ctx, LQX_K_SMEAR);
-        k_smear_gather<T, false><<<grid, 128, 0, ctx->stream>>>(g, make_links<T>(uin), o, c0, c1, only_mu, nullptr);
-    }
+        LqxTimed timed(ctx, LQX_K_PLAQUETTE);
+        k_plaquette<T, MAP><<<grid, MAP::THREADS, 0, ctx->stream>>>(g, MAP::map(g, kSlabZ), make_links<T>(u), ctx->d_partials,
+                                                                  ctx->d_ticket, out);
+    })
     LQX_LAUNCH_CHECK(ctx);
     return LQX_OK;
 }
 
+// one literal smear step on the stream; if plaq != nullptr the input plaquette sum lands there
+template <typename T>
+int smear_gather_launch(lqx_ctx* ctx, lqx_field* const uout[4], const lqx_field* const uin[4], double alpha, int only_mu,
+                        double* plaq) {
+    const Geo& g = ctx->geo;
+    LinksOut<T> o;
+    for (int mu = 0; mu < 4; ++mu) o.u[mu] = uout[mu] ? (T*)uout[mu]->data : nullptr;
+    const T c0 = (T)(1.0 - alpha), c1 = (T)(alpha / 6.0);
+    const int choice = lqx_pick_tile(ctx, sizeof(T) == 4 ? 1 : 2);
+    LQX_WITH_MAP(choice, {
+        const int grid = MAP::grid(g);
+        if (plaq) {
+            int rc = lqx_ensure_partials(ctx, (size_t)grid);
+            if (rc) return rc;
+        }
+        LqxTimed timed(ctx, LQX_K_SMEAR);
+        if (plaq)
+            k_smear_gather<T, true, MAP><<<grid, MAP::THREADS, 0, ctx->stream>>>(g, MAP::map(g, kSlabZ), make_links<T>(uin), o, c0, c1, only_mu,
+                                                                               ctx->d_partials, ctx->d_ticket, plaq);
+        else
+            k_smear_gather<T, false, MAP><<<grid, MAP::THREADS, 0, ctx->stream>>>(g, MAP::map(g, kSlabZ), make_links<T>(uin), o, c0, c1, only_mu,
+                                                                                nullptr, nullptr, nullptr);
+    })
+    LQX_LAUNCH_CHECK(ctx);
+    return LQX_OK;
+}
+
+// smear step dispatch: option "smear_variant" 0 = best available (shared-corner kernel where it
+// covers the lattice, else literal), 1 = literal gather, 2 = shared-corner or fail
 int smear_dispatch(lqx_ctx* ctx, lqx_field* const uout[4], const lqx_field* const uin[4], double alpha, int only_mu,
-                   double* d_plaq) {
-    return uin[0]->prec == LQX_F32 ? smear_launch<float>(ctx, uout, uin, alpha, only_mu, d_plaq)
-                                   : smear_launch<double>(ctx, uout, uin, alpha, only_mu, d_plaq);
+                   double* plaq) {
+    if (only_mu < 0 && ctx->opt_smear_variant != 1) {
+        int rc = lqx_smear_shared_launch(ctx, uout, uin, alpha, plaq);
+        if (rc <= 0) return rc;
+        if (ctx->opt_smear_variant == 2) return lqx_fail(ctx, LQX_EGEOM, "shared-corner smear kernel does not cover this lattice");
+    }
+    return uin[0]->prec == LQX_F32 ? smear_gather_launch<float>(ctx, uout, uin, alpha, only_mu, plaq)
+                                   : smear_gather_launch<double>(ctx, uout, uin, alpha, only_mu, plaq);
 }
 
 }  // namespace
+
+int lqx_pick_tile(const lqx_ctx* ctx, int first_choice) {
+    const Geo& g = ctx->geo;
+    auto fits = [&](int c) {
+        return c == 1 ? TileA::fits(g) : c == 2 ? TileB::fits(g) : c == 3 ? TileC::fits(g) : c == 0;
+    };
+    if (ctx->opt_tile >= 0 && fits(ctx->opt_tile)) return ctx->opt_tile;
+    if (fits(first_choice)) return first_choice;
+    for (int c = 1; c <= 3; ++c)
+        if (fits(c)) return c;
+    return 0;
+}
 
 // =============================================================================================
 // C entry points
@@ -246,32 +259,31 @@ static int hop_impl(lqx_field* chi, const lqx_field* const u[4], const lqx_field
     if (lqx_same(chi, psi)) return lqx_fail(ctx, LQX_EALIAS, "hop: chi aliases psi");
     LQX_CUDA(ctx, cudaSetDevice(ctx->device));
     const Geo& g = ctx->geo;
-    const int grid = (g.V + 127) / 128;
     const bool n2 = norm2_out != nullptr;
-    if (n2) {
-        rc = lqx_ensure_partials(ctx, (size_t)grid);
-        if (rc) return rc;
-    }
     const bool ferm = psi->kind == LQX_FERMION;
-    {
-    LqxTimed timed(ctx, LQX_K_HOP);
-#define LQX_HOP(T, NSPIN, N2) \
-    k_hop<T, NSPIN, N2><<<grid, 128, 0, ctx->stream>>>(g, make_links<T>(u), (const T*)psi->data, (T*)chi->data, ctx->d_partials)
-    if (psi->prec == LQX_F32) {
-        if (ferm) { if (n2) LQX_HOP(float, 4, true); else LQX_HOP(float, 4, false); }
-        else      { if (n2) LQX_HOP(float, 1, true); else LQX_HOP(float, 1, false); }
-    } else {
-        if (ferm) { if (n2) LQX_HOP(double, 4, true); else LQX_HOP(double, 4, false); }
-        else      { if (n2) LQX_HOP(double, 1, true); else LQX_HOP(double, 1, false); }
-    }
+    const int choice = lqx_pick_tile(ctx, 2);
+#define LQX_HOP(T, NSPIN, N2)                                                                                      \
+    k_hop<T, NSPIN, N2, MAP><<<grid, MAP::THREADS, 0, ctx->stream>>>(g, tm, make_links<T>(u), (const T*)psi->data, \
+                                                                    (T*)chi->data, ctx->d_partials, ctx->d_ticket, ctx->h_result)
+    LQX_WITH_MAP(choice, {
+        const int grid = MAP::grid(g);
+        if (n2) {
+            rc = lqx_ensure_partials(ctx, (size_t)grid);
+            if (rc) return rc;
+        }
+        const TileMap tm = MAP::map(g, kSlabZ);
+        LqxTimed timed(ctx, LQX_K_HOP);
+        if (psi->prec == LQX_F32) {
+            if (ferm) { if (n2) LQX_HOP(float, 4, true); else LQX_HOP(float, 4, false); }
+            else      { if (n2) LQX_HOP(float, 1, true); else LQX_HOP(float, 1, false); }
+        } else {
+            if (ferm) { if (n2) LQX_HOP(double, 4, true); else LQX_HOP(double, 4, false); }
+            else      { if (n2) LQX_HOP(double, 1, true); else LQX_HOP(double, 1, false); }
+        }
+    })
 #undef LQX_HOP
-    }
     LQX_LAUNCH_CHECK(ctx);
-    if (n2) {
-        rc = lqx_reduce_finish(ctx, grid, 1, ctx->d_result);
-        if (rc) return rc;
-        return lqx_fetch_result(ctx, 1, norm2_out);
-    }
+    if (n2) return lqx_fetch_result(ctx, 1, norm2_out);
     return LQX_OK;
 }
 
@@ -288,7 +300,7 @@ extern "C" int lqx_plaquette(const lqx_field* const u[4], double* plaq_sum, doub
     int rc = check_links(&ctx, u);
     if (rc) return rc;
     LQX_CUDA(ctx, cudaSetDevice(ctx->device));
-    rc = u[0]->prec == LQX_F32 ? plaquette_launch<float>(ctx, u, ctx->d_result) : plaquette_launch<double>(ctx, u, ctx->d_result);
+    rc = u[0]->prec == LQX_F32 ? plaquette_launch<float>(ctx, u, ctx->h_result) : plaquette_launch<double>(ctx, u, ctx->h_result);
     if (rc) return rc;
     double p;
     rc = lqx_fetch_result(ctx, 1, &p);
@@ -337,7 +349,7 @@ extern "C" int lqx_smear_step(lqx_field* const uout[4], const lqx_field* const u
     int rc = check_smear_args(&ctx, uout, uin);
     if (rc) return rc;
     LQX_CUDA(ctx, cudaSetDevice(ctx->device));
-    rc = smear_dispatch(ctx, uout, uin, alpha, -1, plaq_in_or_null ? ctx->d_result : nullptr);
+    rc = smear_dispatch(ctx, uout, uin, alpha, -1, plaq_in_or_null ? ctx->h_result : nullptr);
     if (rc) return rc;
     if (plaq_in_or_null) return lqx_fetch_result(ctx, 1, plaq_in_or_null);
     return LQX_OK;
@@ -352,12 +364,19 @@ extern "C" int lqx_smear_iterate(lqx_field* const u[4], lqx_field* const tmp[4],
     if (nsteps < 0) return lqx_fail(ctx, LQX_EINVAL, "nsteps < 0");
     if (nsteps == 0) return LQX_OK;
     LQX_CUDA(ctx, cudaSetDevice(ctx->device));
-    double* d_plaq = nullptr;
+    // per-step plaquette sums: the kernels write them straight into pinned host memory
     const bool want = plaq_avg_after_each != nullptr;
+    double* res = nullptr;
+    bool res_owned = false;
     if (want) {
-        if (cudaMalloc(&d_plaq, (size_t)nsteps * sizeof(double)) != cudaSuccess) {
-            cudaGetLastError();
-            return lqx_fail(ctx, LQX_ENOMEM, "plaquette results");
+        if (nsteps <= 64) {
+            res = ctx->h_result;
+        } else {
+            if (cudaHostAlloc(&res, (size_t)nsteps * sizeof(double), cudaHostAllocPortable | cudaHostAllocMapped) != cudaSuccess) {
+                cudaGetLastError();
+                return lqx_fail(ctx, LQX_ENOMEM, "plaquette results");
+            }
+            res_owned = true;
         }
     }
     // Ping-pong u -> tmp -> u ...  The plaquette of the field after step k is the plaquette of the
@@ -366,7 +385,7 @@ extern "C" int lqx_smear_iterate(lqx_field* const u[4], lqx_field* const tmp[4],
     lqx_field* const* src = u;
     lqx_field* const* dst = tmp;
     for (int k = 0; k < nsteps && rc == LQX_OK; ++k) {
-        double* dp = (want && k > 0) ? d_plaq + (k - 1) : nullptr;
+        double* dp = (want && k > 0) ? res + (k - 1) : nullptr;
         rc = smear_dispatch(ctx, dst, (const lqx_field* const*)src, alpha, -1, dp);
         std::swap(src, dst);
     }
@@ -375,21 +394,18 @@ extern "C" int lqx_smear_iterate(lqx_field* const u[4], lqx_field* const tmp[4],
         for (int mu = 0; mu < 4 && rc == LQX_OK; ++mu) rc = lqx_copy(u[mu], tmp[mu]);
     }
     if (rc == LQX_OK && want) {
-        rc = u[0]->prec == LQX_F32 ? plaquette_launch<float>(ctx, (const lqx_field* const*)u, d_plaq + (nsteps - 1))
-                                   : plaquette_launch<double>(ctx, (const lqx_field* const*)u, d_plaq + (nsteps - 1));
+        rc = u[0]->prec == LQX_F32 ? plaquette_launch<float>(ctx, (const lqx_field* const*)u, res + (nsteps - 1))
+                                   : plaquette_launch<double>(ctx, (const lqx_field* const*)u, res + (nsteps - 1));
     }
-    if (rc == LQX_OK && want) {
-        std::vector<double> h((size_t)nsteps);
-        cudaError_t e = cudaMemcpyAsync(h.data(), d_plaq, (size_t)nsteps * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream);
-        if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
-        if (e != cudaSuccess) rc = lqx_cuda_fail(ctx, e, "smear_iterate results");
-        const double norm = 18.0 * (double)ctx->geo.V;
-        for (int k = 0; k < nsteps && rc == LQX_OK; ++k) plaq_avg_after_each[k] = h[k] / norm;
-    } else if (rc == LQX_OK) {
+    if (rc == LQX_OK) {
         cudaError_t e = cudaStreamSynchronize(ctx->stream);
         if (e != cudaSuccess) rc = lqx_cuda_fail(ctx, e, "smear_iterate sync");
     }
-    if (d_plaq) cudaFree(d_plaq);
+    if (rc == LQX_OK && want) {
+        const double norm = 18.0 * (double)ctx->geo.V;
+        for (int k = 0; k < nsteps; ++k) plaq_avg_after_each[k] = res[k] / norm;
+    }
+    if (res_owned) cudaFreeHost(res);
     return rc;
 }
 

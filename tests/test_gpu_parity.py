@@ -74,17 +74,35 @@ def test_push_pop_round_trip_bit_exact(lqx, dims, prec, kind):
         assert np.array_equal(g.pop(), a)
 
 
-def test_internal_layout_is_site_fastest_soa(lqx):
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+@pytest.mark.parametrize("kind", ["c", "cv", "cm", "f"])
+def test_internal_layout_is_blocked_site_fastest_soa(lqx, prec, kind):
+    """include/lqx.h: blocks of 32 sites, 128-bit chunks of the site object, chunk q of the 32 sites
+    contiguous.  The expected offsets are recomputed here from that sentence, not from the library."""
     import torch
 
-    dims = (4, 2, 2, 2)
-    a = _gauss(5, 0, dims, "cm", "f32")
+    dims = (6, 2, 3, 2)  # V = 72: two full blocks and a ragged one
+    a = _gauss(5, 0, dims, kind, prec)
+    v = a.shape[0]
+    nreal = a.reshape(v, -1).shape[1]
+    w = 4 if prec == "f32" else 2
+    nfull = nreal // w
     with lqx.Lattice(dims) as lat:
         f = lat.from_host(a)
         torch.cuda.synchronize()
-        raw = f._mem.view(torch.float32).cpu().numpy().reshape(18, lat.stride)
-        assert lat.stride % 32 == 0 and lat.stride >= lat.volume
-        assert np.array_equal(raw[:, : lat.volume], a.reshape(lat.volume, 18).T)
+        assert lat.padded_volume % 32 == 0 and lat.volume <= lat.padded_volume < lat.volume + 32
+        assert lat.field_bytes(f.kind, f.prec) == lat.padded_volume * nreal * (4 if prec == "f32" else 8)
+        raw = f._mem.view(torch.float32 if prec == "f32" else torch.float64).cpu().numpy()
+        flat = a.reshape(v, nreal)
+        expect = np.zeros(lat.padded_volume * nreal, dtype=flat.dtype)
+        for s in range(v):
+            for r in range(nreal):
+                q = min(r // w, nfull)
+                wq = w if q < nfull else nreal - nfull * w
+                off = (s // 32) * 32 * nreal + q * 32 * w + (s % 32) * wq + (r - q * w)
+                expect[off] = flat[s, r]
+                assert lat.field_offset(f.kind, f.prec, s, r) == off
+        assert np.array_equal(raw, expect)  # pad lanes of the last block are zero
 
 
 # ------------------------------------------------------------------------------------------------
