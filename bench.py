@@ -313,7 +313,7 @@ def run_ours(args):
     # FP-pipe peak from unit counts and clocks: 148 SMs x 128 fp32 (64 fp64) FMA lanes x sm_max
     alu_peak_tflops = 148 * (128 if prec == "f32" else 64) * 2 * sm_max * 1e6 / 1e12
     roofline = {
-        "kernel": "k_smear (staple sum + smear update, fused input plaquette)",
+        "kernel": "k_smear_rolled (staple sum + smear update, fused input plaquette)",
         "bound": "alu", "achieved": 2 * lane_ops / (k_ms * 1e-3) / 1e12, "peak": alu_peak_tflops, "unit": "TFLOP/s",
         "frac": 2 * lane_ops / (k_ms * 1e-3) / 1e12 / alu_peak_tflops,
         "peak_source": f"148 SMs x {128 if prec == 'f32' else 64} FMA lanes x 2 x {sm_max:.0f} MHz (DESIGN.md sec.7); "

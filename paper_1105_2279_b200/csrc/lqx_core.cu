@@ -410,6 +410,38 @@ int lqx_ensure_partials(lqx_ctx* ctx, size_t ndoubles) {
     return LQX_OK;
 }
 
+// one CTA per component; fixed strided accumulation (4 independent chains per thread) + fixed tree
+__global__ void __launch_bounds__(1024) k_sum_partials(const double* __restrict__ partials, int nblocks, double* __restrict__ out) {
+    __shared__ double sh[32];
+    const double* p = partials + (size_t)blockIdx.x * nblocks;
+    double t0 = 0.0, t1 = 0.0, t2 = 0.0, t3 = 0.0;
+    int i = threadIdx.x;
+    for (; i + 3 * 1024 < nblocks; i += 4 * 1024) {
+        t0 += p[i];
+        t1 += p[i + 1024];
+        t2 += p[i + 2048];
+        t3 += p[i + 3072];
+    }
+    for (; i < nblocks; i += 1024) t0 += p[i];
+    double t = (t0 + t1) + (t2 + t3);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = t;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        t = sh[threadIdx.x];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+        if (threadIdx.x == 0) out[blockIdx.x] = t;
+    }
+}
+
+int lqx_sum_partials(lqx_ctx* ctx, int nblocks, int ncomp, double* out) {
+    k_sum_partials<<<ncomp, 1024, 0, ctx->stream>>>(ctx->d_partials, nblocks, out);
+    LQX_LAUNCH_CHECK(ctx);
+    return LQX_OK;
+}
+
 int lqx_fetch_result(lqx_ctx* ctx, int n, double* out) {
     LQX_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     for (int i = 0; i < n; ++i) out[i] = ctx->h_result[i];

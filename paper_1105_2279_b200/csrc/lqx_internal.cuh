@@ -168,6 +168,24 @@ __host__ __device__ __forceinline__ size_t lqx_layout_offset(int s, int r, int n
     return (size_t)(s >> 5) * 32 * nreal + (size_t)q * 32 * W + (size_t)(s & 31) * wq + (r - q * W);
 }
 
+// 128-bit / 64-bit read-only loads as VOLATILE asm: the compiler keeps them in program order, which
+// is how the unrolled nearest-neighbour kernels control how many operands are in flight.
+__device__ __forceinline__ float4 ldg_pinned(const float4* p) {
+    float4 v;
+    asm volatile("ld.global.nc.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ double2 ldg_pinned(const double2* p) {
+    double2 v;
+    asm volatile("ld.global.nc.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ float2 ldg_pinned(const float2* p) {
+    float2 v;
+    asm volatile("ld.global.nc.v2.f32 {%0,%1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p));
+    return v;
+}
+
 // all NREAL reals of site s (read-only path)
 template <typename T, int NREAL>
 __device__ __forceinline__ void load_site(const T* __restrict__ base, int s, T (&r)[NREAL]) {
@@ -180,6 +198,21 @@ __device__ __forceinline__ void load_site(const T* __restrict__ base, int s, T (
     for (int q = 0; q < NFULL; ++q) unpack(__ldg(p + q * 32), &r[q * W]);
     if (NREAL % W != 0) {  // fp32 only: trailing (re,im) pair
         const float2 t = __ldg(reinterpret_cast<const float2*>(blk + NFULL * 32 * W) + lane);
+        r[NFULL * W] = (T)t.x;
+        r[NFULL * W + 1] = (T)t.y;
+    }
+}
+template <typename T, int NREAL>
+__device__ __forceinline__ void load_site_pinned(const T* __restrict__ base, int s, T (&r)[NREAL]) {
+    typedef typename Vec128<T>::type V;
+    constexpr int W = Vec128<T>::W, NFULL = NREAL / W;
+    const T* blk = base + (size_t)(s >> 5) * (32 * NREAL);
+    const int lane = s & 31;
+    const V* p = reinterpret_cast<const V*>(blk) + lane;
+#pragma unroll
+    for (int q = 0; q < NFULL; ++q) unpack(ldg_pinned(p + q * 32), &r[q * W]);
+    if (NREAL % W != 0) {
+        const float2 t = ldg_pinned(reinterpret_cast<const float2*>(blk + NFULL * 32 * W) + lane);
         r[NFULL * W] = (T)t.x;
         r[NFULL * W + 1] = (T)t.y;
     }
@@ -215,6 +248,20 @@ template <typename T>
 __device__ __forceinline__ Mat3<T> load_mat(const T* __restrict__ p, int s) {
     T r[18];
     load_site<T, 18>(p, s, r);
+    Mat3<T> m;
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            m.re[i][j] = r[2 * (3 * i + j)];
+            m.im[i][j] = r[2 * (3 * i + j) + 1];
+        }
+    return m;
+}
+template <typename T>
+__device__ __forceinline__ Mat3<T> load_mat_pinned(const T* __restrict__ p, int s) {
+    T r[18];
+    load_site_pinned<T, 18>(p, s, r);
     Mat3<T> m;
 #pragma unroll
     for (int i = 0; i < 3; ++i)
@@ -451,13 +498,17 @@ __device__ __forceinline__ void block_reduce_finish(double (&v)[NC], double* __r
             if (lane == 0) partials[(size_t)c * nblocks + block] = t;
         }
         if (lane == 0) {
-            __threadfence();
-            last = (atomicAdd(ticket, 1u) == (unsigned)(nblocks - 1));
+            // release-only ticket: orders this lane's partial stores before the increment without the
+            // L1 invalidation (CCTL.IVALL) that __threadfence() would cost every CTA of the grid --
+            // in the smear kernel that wipes the neighbours its co-resident CTAs share
+            unsigned int t;
+            asm volatile("atom.release.gpu.global.add.u32 %0, [%1], 1;" : "=r"(t) : "l"(ticket) : "memory");
+            last = (t == (unsigned)(nblocks - 1));
         }
     }
     __syncthreads();
     if (!last) return;
-    __threadfence();
+    __threadfence();  // acquire side, paid by the one finishing CTA; partials are then read from L2
     for (int c = 0; c < NC; ++c) {
         double t = 0.0;
         for (int i = tid; i < nblocks; i += nthreads) t += __ldcg(partials + (size_t)c * nblocks + i);
@@ -475,6 +526,39 @@ __device__ __forceinline__ void block_reduce_finish(double (&v)[NC], double* __r
     }
     if (tid == 0) *ticket = 0u;  // ready for the next launch on this stream
 }
+
+// Two-launch form for the long nearest-neighbour kernels: the CTA only stores its partial (no fence,
+// no ticket, nothing that delays its retirement); lqx_sum_partials() then adds them up in a fixed
+// order with one small CTA per component.
+template <int NC>
+__device__ __forceinline__ void block_reduce_partial(double (&v)[NC], double* __restrict__ partials) {
+    __shared__ double sh[32][NC + (NC % 2 == 0 ? 1 : 0)];
+    const int tid = threadIdx.x + blockDim.x * (threadIdx.y + blockDim.y * threadIdx.z);
+    const int nthreads = blockDim.x * blockDim.y * blockDim.z;
+    const int lane = tid & 31, warp = tid >> 5;
+    const int nwarps = (nthreads + 31) >> 5;
+    const int nblocks = gridDim.x * gridDim.y * gridDim.z;
+    const int block = blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z);
+#pragma unroll
+    for (int c = 0; c < NC; ++c) {
+        double t = v[c];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+        if (lane == 0) sh[warp][c] = t;
+    }
+    __syncthreads();
+    if (warp == 0) {
+#pragma unroll
+        for (int c = 0; c < NC; ++c) {
+            double t = (lane < nwarps) ? sh[lane][c] : 0.0;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+            if (lane == 0) partials[(size_t)c * nblocks + block] = t;
+        }
+    }
+}
+// out[c] = sum_b partials[c*nblocks + b], c < ncomp, on the context's stream (lqx_core.cu)
+int lqx_sum_partials(lqx_ctx* ctx, int nblocks, int ncomp, double* out);
 
 // --------------------------------------------------------------------------------------------
 // device side: CTA -> sites maps of the nearest-neighbour kernels (hop, plaquette, smear).

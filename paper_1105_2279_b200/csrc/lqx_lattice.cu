@@ -1,5 +1,5 @@
-// lqx nearest-neighbour kernels: hop, plaquette (a8), literal staple sum + smear
-// step (a7) and the iterated smearing driver (a10).  Each is a single pass in which one thread
+// lqx nearest-neighbour kernels: hop, plaquette (a8), and the C entry points of the
+// staple sum / smear step (a7, kernels in lqx_smear.cu) and of the iterated smearing driver (a10).  Each is a single pass in which one thread
 // evaluates the whole expression of its site, reading shifted operands at
 // the periodic neighbour computed in-kernel (the role of the paper's site tables).
 // CTAs own compact 4-d tiles (lqx_internal.cuh, Tiled<>) so that shared neighbours are L1 hits.
@@ -62,8 +62,7 @@ __global__ void __launch_bounds__(MAP::THREADS) k_hop(const __grid_constant__ Ge
 // ---------------------------------------------------------------------------------------------
 template <typename T, typename MAP>
 __global__ void __launch_bounds__(MAP::THREADS) k_plaquette(const __grid_constant__ Geo g, const __grid_constant__ TileMap tm,
-                                                            const __grid_constant__ Links<T> u, double* __restrict__ partials,
-                                                            unsigned int* ticket, double* __restrict__ out) {
+                                                            const __grid_constant__ Links<T> u, double* __restrict__ partials) {
     int x[4], s;
     double p[1] = {0.0};
     if (MAP::site(g, tm, x, s)) {
@@ -82,78 +81,7 @@ __global__ void __launch_bounds__(MAP::THREADS) k_plaquette(const __grid_constan
         }
         p[0] = (double)acc;
     }
-    block_reduce_finish<1>(p, partials, ticket, out);
-}
-
-// ---------------------------------------------------------------------------------------------
-// staple sum + smear step, literal gather form: one thread per site, mu and nu loops inside;
-// every staple is a chain of two products kept in registers (48 products per site).
-//   S_mu(x) = sum_{nu!=mu} U_nu(x) U_mu(x+nu^) adj(U_nu(x+mu^)) + adj(U_nu(x-nu^)) U_mu(x-nu^) U_nu(x-nu^+mu^)
-//   U'_mu(x) = c0 U_mu(x) + c1 S_mu(x)
-// PLAQ: the plaquette of the INPUT field is accumulated on the way:
-//   Re tr[U_mu U_nu(x+mu) adj(U_mu(x+nu)) adj(U_nu)] = Re tr[U_mu(x) adj(upper staple_{mu,nu}(x))], mu<nu.
-// only_mu >= 0: write the bare staple sum of that direction into out.u[0] (diagnostic entry).
-// ---------------------------------------------------------------------------------------------
-template <typename T, bool PLAQ, typename MAP>
-__global__ void __launch_bounds__(MAP::THREADS) k_smear_gather(const __grid_constant__ Geo g, const __grid_constant__ TileMap tm,
-                                                               const __grid_constant__ Links<T> u, const __grid_constant__ LinksOut<T> out,
-                                                               T c0, T c1, int only_mu, double* __restrict__ partials,
-                                                               unsigned int* ticket, double* __restrict__ red_out) {
-    int x[4], s;
-    double p[1] = {0.0};
-    if (MAP::site(g, tm, x, s)) {
-        T pl = T(0);
-        const int mu_lo = only_mu >= 0 ? only_mu : 0, mu_hi = only_mu >= 0 ? only_mu + 1 : 4;
-#pragma unroll 1
-        for (int mu = mu_lo; mu < mu_hi; ++mu) {
-            const int xpmu = nbr_fwd(g, s, x, mu);
-            const Mat3<T> umu = load_mat(u.u[mu], s);
-            Mat3<T> acc = zero_mat<T>();
-#pragma unroll 1
-            for (int nu = 0; nu < 4; ++nu) {
-                if (nu == mu) continue;
-                const int xpnu = nbr_fwd(g, s, x, nu);
-                const int xmnu = nbr_bwd(g, s, x, nu);
-                // x - nu^ + mu^ : step forward in mu from xmnu (coordinates differ from x only in nu)
-                const int xmnupmu = xmnu + (xpmu - s);
-                {
-                    const Mat3<T> t = mul_nn(load_mat(u.u[nu], s), load_mat(u.u[mu], xpnu));
-                    if (PLAQ && mu < nu) {
-                        const Mat3<T> up = mul_na(t, load_mat(u.u[nu], xpmu));
-                        pl += re_tr_na(umu, up);
-#pragma unroll
-                        for (int i = 0; i < 3; ++i)
-#pragma unroll
-                            for (int j = 0; j < 3; ++j) {
-                                acc.re[i][j] += up.re[i][j];
-                                acc.im[i][j] += up.im[i][j];
-                            }
-                    } else {
-                        mac_na(acc, t, load_mat(u.u[nu], xpmu));
-                    }
-                }
-                {
-                    const Mat3<T> t = mul_an(load_mat(u.u[nu], xmnu), load_mat(u.u[mu], xmnu));
-                    mac_nn(acc, t, load_mat(u.u[nu], xmnupmu));
-                }
-            }
-            if (only_mu >= 0) {
-                store_mat(out.u[0], s, acc);
-            } else {
-                Mat3<T> r;
-#pragma unroll
-                for (int i = 0; i < 3; ++i)
-#pragma unroll
-                    for (int j = 0; j < 3; ++j) {
-                        r.re[i][j] = fma(c1, acc.re[i][j], c0 * umu.re[i][j]);
-                        r.im[i][j] = fma(c1, acc.im[i][j], c0 * umu.im[i][j]);
-                    }
-                store_mat(out.u[mu], s, r);
-            }
-        }
-        p[0] = (double)pl;
-    }
-    if (PLAQ) block_reduce_finish<1>(p, partials, ticket, red_out);
+    block_reduce_partial<1>(p, partials);
 }
 
 int check_links(lqx_ctx** ctx_out, const lqx_field* const u[4]) {
@@ -170,64 +98,22 @@ int check_links(lqx_ctx** ctx_out, const lqx_field* const u[4]) {
     return LQX_OK;
 }
 
-// z-extent (sites) of a slab of the tile visiting order: thick enough that the two re-read z-faces
-// are a small fraction, thin enough that three t-slices of a slab stay in L2
-const int kSlabZ = 16;
 
 template <typename T>
 int plaquette_launch(lqx_ctx* ctx, const lqx_field* const u[4], double* out) {
     const Geo& g = ctx->geo;
-    const int choice = lqx_pick_tile(ctx, 1);
+    const int choice = lqx_pick_tile(ctx, sizeof(T) == 4 ? 1 : 0);
+    int nblocks = 0;
     LQX_WITH_MAP(choice, {
         const int grid = MAP::grid(g);
+        nblocks = grid;
         int rc = lqx_ensure_partials(ctx, (size_t)grid);
         if (rc) return rc;
         LqxTimed timed(ctx, LQX_K_PLAQUETTE);
-        k_plaquette<T, MAP><<<grid, MAP::THREADS, 0, ctx->stream>>>(g, MAP::map(g, kSlabZ), make_links<T>(u), ctx->d_partials,
-                                                                  ctx->d_ticket, out);
+        k_plaquette<T, MAP><<<grid, MAP::THREADS, 0, ctx->stream>>>(g, MAP::map(g, kSlabZ), make_links<T>(u), ctx->d_partials);
     })
     LQX_LAUNCH_CHECK(ctx);
-    return LQX_OK;
-}
-
-// one literal smear step on the stream; if plaq != nullptr the input plaquette sum lands there
-template <typename T>
-int smear_gather_launch(lqx_ctx* ctx, lqx_field* const uout[4], const lqx_field* const uin[4], double alpha, int only_mu,
-                        double* plaq) {
-    const Geo& g = ctx->geo;
-    LinksOut<T> o;
-    for (int mu = 0; mu < 4; ++mu) o.u[mu] = uout[mu] ? (T*)uout[mu]->data : nullptr;
-    const T c0 = (T)(1.0 - alpha), c1 = (T)(alpha / 6.0);
-    const int choice = lqx_pick_tile(ctx, sizeof(T) == 4 ? 1 : 2);
-    LQX_WITH_MAP(choice, {
-        const int grid = MAP::grid(g);
-        if (plaq) {
-            int rc = lqx_ensure_partials(ctx, (size_t)grid);
-            if (rc) return rc;
-        }
-        LqxTimed timed(ctx, LQX_K_SMEAR);
-        if (plaq)
-            k_smear_gather<T, true, MAP><<<grid, MAP::THREADS, 0, ctx->stream>>>(g, MAP::map(g, kSlabZ), make_links<T>(uin), o, c0, c1, only_mu,
-                                                                               ctx->d_partials, ctx->d_ticket, plaq);
-        else
-            k_smear_gather<T, false, MAP><<<grid, MAP::THREADS, 0, ctx->stream>>>(g, MAP::map(g, kSlabZ), make_links<T>(uin), o, c0, c1, only_mu,
-                                                                                nullptr, nullptr, nullptr);
-    })
-    LQX_LAUNCH_CHECK(ctx);
-    return LQX_OK;
-}
-
-// smear step dispatch: option "smear_variant" 0 = best available (shared-corner kernel where it
-// covers the lattice, else literal), 1 = literal gather, 2 = shared-corner or fail
-int smear_dispatch(lqx_ctx* ctx, lqx_field* const uout[4], const lqx_field* const uin[4], double alpha, int only_mu,
-                   double* plaq) {
-    if (only_mu < 0 && ctx->opt_smear_variant != 1) {
-        int rc = lqx_smear_shared_launch(ctx, uout, uin, alpha, plaq);
-        if (rc <= 0) return rc;
-        if (ctx->opt_smear_variant == 2) return lqx_fail(ctx, LQX_EGEOM, "shared-corner smear kernel does not cover this lattice");
-    }
-    return uin[0]->prec == LQX_F32 ? smear_gather_launch<float>(ctx, uout, uin, alpha, only_mu, plaq)
-                                   : smear_gather_launch<double>(ctx, uout, uin, alpha, only_mu, plaq);
+    return lqx_sum_partials(ctx, nblocks, 1, out);
 }
 
 }  // namespace
@@ -235,11 +121,21 @@ int smear_dispatch(lqx_ctx* ctx, lqx_field* const uout[4], const lqx_field* cons
 int lqx_pick_tile(const lqx_ctx* ctx, int first_choice) {
     const Geo& g = ctx->geo;
     auto fits = [&](int c) {
-        return c == 1 ? TileA::fits(g) : c == 2 ? TileB::fits(g) : c == 3 ? TileC::fits(g) : c == 0;
+        switch (c) {
+            case 0: return true;
+            case 1: return TileA::fits(g);
+            case 2: return TileB::fits(g);
+            case 3: return TileC::fits(g);
+            case 4: return TileD::fits(g);
+            case 5: return TileE::fits(g);
+            case 6: return TileF::fits(g);
+            default: return false;
+        }
     };
     if (ctx->opt_tile >= 0 && fits(ctx->opt_tile)) return ctx->opt_tile;
     if (fits(first_choice)) return first_choice;
-    for (int c = 1; c <= 3; ++c)
+    static const int order[kNumTiles] = {4, 1, 5, 2, 3, 6};
+    for (int c : order)
         if (fits(c)) return c;
     return 0;
 }
@@ -339,7 +235,7 @@ extern "C" int lqx_staple_sum(lqx_field* out, const lqx_field* const u[4], int m
         if (lqx_same(out, u[b])) return lqx_fail(ctx, LQX_EALIAS, "staple_sum: output aliases a link field");
     LQX_CUDA(ctx, cudaSetDevice(ctx->device));
     lqx_field* o[4] = {out, nullptr, nullptr, nullptr};
-    return smear_dispatch(ctx, o, u, 0.0, mu, nullptr);
+    return lqx_smear_launch(ctx, o, u, 0.0, mu, nullptr);
 }
 
 extern "C" int lqx_smear_step(lqx_field* const uout[4], const lqx_field* const uin[4], double alpha,
@@ -349,7 +245,7 @@ extern "C" int lqx_smear_step(lqx_field* const uout[4], const lqx_field* const u
     int rc = check_smear_args(&ctx, uout, uin);
     if (rc) return rc;
     LQX_CUDA(ctx, cudaSetDevice(ctx->device));
-    rc = smear_dispatch(ctx, uout, uin, alpha, -1, plaq_in_or_null ? ctx->h_result : nullptr);
+    rc = lqx_smear_launch(ctx, uout, uin, alpha, -1, plaq_in_or_null ? ctx->h_result : nullptr);
     if (rc) return rc;
     if (plaq_in_or_null) return lqx_fetch_result(ctx, 1, plaq_in_or_null);
     return LQX_OK;
@@ -386,7 +282,7 @@ extern "C" int lqx_smear_iterate(lqx_field* const u[4], lqx_field* const tmp[4],
     lqx_field* const* dst = tmp;
     for (int k = 0; k < nsteps && rc == LQX_OK; ++k) {
         double* dp = (want && k > 0) ? res + (k - 1) : nullptr;
-        rc = smear_dispatch(ctx, dst, (const lqx_field* const*)src, alpha, -1, dp);
+        rc = lqx_smear_launch(ctx, dst, (const lqx_field* const*)src, alpha, -1, dp);
         std::swap(src, dst);
     }
     // result is in src now; if that is tmp (odd nsteps), copy back into u

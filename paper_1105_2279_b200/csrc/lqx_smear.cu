@@ -1,5 +1,295 @@
-// lqx shared-corner smear kernel: placeholder translation unit -- the
-// literal kernel in lqx_lattice.cu serves every lattice until this one is filled in.
+// lqx staple sum + smear step kernels (BASELINE.json configs[0],[2],[3]):
+//   S_mu(x)  = sum_{nu!=mu} U_nu(x) U_mu(x+nu^) adj(U_nu(x+mu^)) + adj(U_nu(x-nu^)) U_mu(x-nu^) U_nu(x-nu^+mu^)
+//   U'_mu(x) = c0 U_mu(x) + c1 S_mu(x),   c0 = 1-alpha, c1 = alpha/6
+// One thread evaluates the whole expression of its site; the shifted operands
+// are read at periodic neighbours computed in-kernel.  Variants of the same
+// literal 48-product evaluation, selected by the context option "smear_variant":
+//   1  k_smear_gather : mu outer / nu inner as run-time loops, one accumulator (also the staple_sum entry)
+//   3  k_smear_rolled : same order, neighbour indices in shared memory, U_mu(x) not held, register cap
+//                       that allows three 256-thread (six 128-thread) CTAs per SM in fp32  [default]
 #include "lqx_smear.cuh"
 
-int lqx_smear_shared_launch(lqx_ctx*, lqx_field* const[4], const lqx_field* const[4], double, double*) { return 1; }
+#include <type_traits>
+
+namespace {
+
+// variant 1: mu outer / nu inner as run-time loops; every staple is a chain of two products kept in
+// registers (48 products per site).
+// PLAQ: the plaquette of the INPUT field is accumulated on the way:
+//   Re tr[U_mu U_nu(x+mu) adj(U_mu(x+nu)) adj(U_nu)] = Re tr[U_mu(x) adj(upper staple_{mu,nu}(x))], mu<nu.
+// only_mu >= 0: write the bare staple sum of that direction into out.u[0] (diagnostic entry).
+// ---------------------------------------------------------------------------------------------
+template <typename T, bool PLAQ, typename MAP>
+__global__ void __launch_bounds__(MAP::THREADS) k_smear_gather(const __grid_constant__ Geo g, const __grid_constant__ TileMap tm,
+                                                               const __grid_constant__ Links<T> u, const __grid_constant__ LinksOut<T> out,
+                                                               T c0, T c1, int only_mu, double* __restrict__ partials,
+                                                               unsigned int* ticket, double* __restrict__ red_out) {
+    int x[4], s;
+    double p[1] = {0.0};
+    if (MAP::site(g, tm, x, s)) {
+        T pl = T(0);
+        const int mu_lo = only_mu >= 0 ? only_mu : 0, mu_hi = only_mu >= 0 ? only_mu + 1 : 4;
+#pragma unroll 1
+        for (int mu = mu_lo; mu < mu_hi; ++mu) {
+            const int xpmu = nbr_fwd(g, s, x, mu);
+            const Mat3<T> umu = load_mat(u.u[mu], s);
+            Mat3<T> acc = zero_mat<T>();
+#pragma unroll 1
+            for (int nu = 0; nu < 4; ++nu) {
+                if (nu == mu) continue;
+                const int xpnu = nbr_fwd(g, s, x, nu);
+                const int xmnu = nbr_bwd(g, s, x, nu);
+                // x - nu^ + mu^ : step forward in mu from xmnu (coordinates differ from x only in nu)
+                const int xmnupmu = xmnu + (xpmu - s);
+                {
+                    const Mat3<T> t = mul_nn(load_mat(u.u[nu], s), load_mat(u.u[mu], xpnu));
+                    if (PLAQ && mu < nu) {
+                        const Mat3<T> up = mul_na(t, load_mat(u.u[nu], xpmu));
+                        pl += re_tr_na(umu, up);
+#pragma unroll
+                        for (int i = 0; i < 3; ++i)
+#pragma unroll
+                            for (int j = 0; j < 3; ++j) {
+                                acc.re[i][j] += up.re[i][j];
+                                acc.im[i][j] += up.im[i][j];
+                            }
+                    } else {
+                        mac_na(acc, t, load_mat(u.u[nu], xpmu));
+                    }
+                }
+                {
+                    const Mat3<T> t = mul_an(load_mat(u.u[nu], xmnu), load_mat(u.u[mu], xmnu));
+                    mac_nn(acc, t, load_mat(u.u[nu], xmnupmu));
+                }
+            }
+            if (only_mu >= 0) {
+                store_mat(out.u[0], s, acc);
+            } else {
+                Mat3<T> r;
+#pragma unroll
+                for (int i = 0; i < 3; ++i)
+#pragma unroll
+                    for (int j = 0; j < 3; ++j) {
+                        r.re[i][j] = fma(c1, acc.re[i][j], c0 * umu.re[i][j]);
+                        r.im[i][j] = fma(c1, acc.im[i][j], c0 * umu.im[i][j]);
+                    }
+                store_mat(out.u[mu], s, r);
+            }
+        }
+        p[0] = (double)pl;
+    }
+    if (PLAQ) block_reduce_partial<1>(p, partials);
+}
+
+
+template <typename T>
+__device__ __forceinline__ void add_to(Mat3<T>& acc, const Mat3<T>& m) {
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            acc.re[i][j] += m.re[i][j];
+            acc.im[i][j] += m.im[i][j];
+        }
+}
+template <typename T>
+__device__ __forceinline__ Mat3<T> smear_update(T c0, T c1, const Mat3<T>& umu, const Mat3<T>& acc) {
+    Mat3<T> r;
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            r.re[i][j] = fma(c1, acc.re[i][j], c0 * umu.re[i][j]);
+            r.im[i][j] = fma(c1, acc.im[i][j], c0 * umu.im[i][j]);
+        }
+    return r;
+}
+
+// variant 3: the literal evaluation with the loops kept rolled (so that only one staple's operands are
+// live: 80 registers, three 256-thread CTAs per SM in fp32), the eight neighbour site indices of the
+// thread parked in shared memory and looked up by the run-time direction, and U_mu(x) fetched only
+// when it is needed instead of being held across the nu loop.  Per link: first the three upper
+// staples with nu DEscending, so that after the nu > mu ones the accumulator is exactly
+// sum_{nu>mu} upper_{mu,nu} and the plaquette terms of this link cost ONE trace
+//   sum_{nu>mu} Re tr[U_mu U_nu(x+mu) adj(U_mu(x+nu)) adj(U_nu)] = Re tr[U_mu(x) adj(acc)],
+// then the three lower staples.
+template <typename T, bool PLAQ, typename MAP, int MINB>
+__global__ void __launch_bounds__(MAP::THREADS, MINB) k_smear_rolled(const __grid_constant__ Geo g, const __grid_constant__ TileMap tm,
+                                                                     const __grid_constant__ Links<T> u, const __grid_constant__ LinksOut<T> out,
+                                                                     T c0, T c1, double* __restrict__ partials, unsigned int* ticket,
+                                                                     double* __restrict__ red_out) {
+    __shared__ int nb[8][MAP::THREADS];  // [0..3] x+d^, [4..7] x-d^
+    int x[4], s;
+    double p[1] = {0.0};
+    const int tid = threadIdx.x;
+    if (MAP::site(g, tm, x, s)) {
+#pragma unroll
+        for (int d = 0; d < 4; ++d) {
+            nb[d][tid] = (x[d] + 1 == g.L[d]) ? s - (g.L[d] - 1) * g.stride_site[d] : s + g.stride_site[d];
+            nb[4 + d][tid] = (x[d] == 0) ? s + (g.L[d] - 1) * g.stride_site[d] : s - g.stride_site[d];
+        }
+        T pl = T(0);
+#pragma unroll 1
+        for (int mu = 0; mu < 4; ++mu) {
+            const T* __restrict__ umu_p = u.u[mu];
+            const int xpmu = nb[mu][tid];
+            Mat3<T> acc = zero_mat<T>();
+#pragma unroll 1
+            for (int nu = 3; nu >= 0; --nu) {  // upper: U_nu(x) U_mu(x+nu^) adj(U_nu(x+mu^))
+                if (nu == mu) {
+                    if (PLAQ && mu < 3) pl += re_tr_na(load_mat(umu_p, s), acc);
+                    continue;
+                }
+                const T* __restrict__ unu_p = u.u[nu];
+                const Mat3<T> t = mul_nn(load_mat(unu_p, s), load_mat(umu_p, nb[nu][tid]));
+                mac_na(acc, t, load_mat(unu_p, xpmu));
+            }
+#pragma unroll 1
+            for (int nu = 0; nu < 4; ++nu) {  // lower: adj(U_nu(x-nu^)) U_mu(x-nu^) U_nu(x-nu^+mu^)
+                if (nu == mu) continue;
+                const T* __restrict__ unu_p = u.u[nu];
+                const int xmnu = nb[4 + nu][tid];
+                const Mat3<T> t = mul_an(load_mat(unu_p, xmnu), load_mat(umu_p, xmnu));
+                mac_nn(acc, t, load_mat(unu_p, xmnu + (xpmu - s)));
+            }
+            store_mat(out.u[mu], s, smear_update(c0, c1, load_mat(umu_p, s), acc));
+        }
+        p[0] = (double)pl;
+    }
+    if (PLAQ) block_reduce_partial<1>(p, partials);
+}
+
+// variant 4: four threads per site -- thread (site, mu) evaluates the six staples of ONE link, so a
+// CTA of 4*TILE threads works on a TILE-site tile whose operand footprint (the tile, its faces and
+// edges: ~15 matrices per site) is small enough to stay in L1 while 16 warps per SM hide latency.
+// The literal kernel with one thread per site keeps three such footprints per SM alive and thrashes
+// L1 (38 % hits, L2 -> L1 traffic at the L2 bandwidth limit; profiles/r01b).
+template <typename T, bool PLAQ, typename MAP, int MINB>
+__global__ void __launch_bounds__(MAP::THREADS * 4, MINB) k_smear_mu4(const __grid_constant__ Geo g, const __grid_constant__ TileMap tm,
+                                                                      const __grid_constant__ Links<T> u, const __grid_constant__ LinksOut<T> out,
+                                                                      T c0, T c1, double* __restrict__ partials, unsigned int* ticket,
+                                                                      double* __restrict__ red_out) {
+    __shared__ int nb[8][MAP::THREADS];  // [0..3] x+d^, [4..7] x-d^
+    int x[4], s;
+    double p[1] = {0.0};
+    const int tid = threadIdx.x, mu = threadIdx.y;
+    const bool valid = MAP::site(g, tm, x, s);
+    if (valid && mu == 0) {
+#pragma unroll
+        for (int d = 0; d < 4; ++d) {
+            nb[d][tid] = (x[d] + 1 == g.L[d]) ? s - (g.L[d] - 1) * g.stride_site[d] : s + g.stride_site[d];
+            nb[4 + d][tid] = (x[d] == 0) ? s + (g.L[d] - 1) * g.stride_site[d] : s - g.stride_site[d];
+        }
+    }
+    __syncthreads();
+    if (valid) {
+        T pl = T(0);
+        const T* __restrict__ umu_p = u.u[mu];
+        const int xpmu = nb[mu][tid];
+        Mat3<T> acc = zero_mat<T>();
+#pragma unroll 1
+        for (int nu = 0; nu < 4; ++nu) {
+            if (nu == mu) continue;
+            const T* __restrict__ unu_p = u.u[nu];
+            const int xpnu = nb[nu][tid], xmnu = nb[4 + nu][tid];
+            {
+                const Mat3<T> t = mul_nn(load_mat(unu_p, s), load_mat(umu_p, xpnu));
+                if (PLAQ && mu < nu) {
+                    const Mat3<T> up = mul_na(t, load_mat(unu_p, xpmu));
+                    pl += re_tr_na(load_mat(umu_p, s), up);
+                    add_to(acc, up);
+                } else {
+                    mac_na(acc, t, load_mat(unu_p, xpmu));
+                }
+            }
+            {
+                const Mat3<T> t = mul_an(load_mat(unu_p, xmnu), load_mat(umu_p, xmnu));
+                mac_nn(acc, t, load_mat(unu_p, xmnu + (xpmu - s)));
+            }
+        }
+        store_mat(out.u[mu], s, smear_update(c0, c1, load_mat(umu_p, s), acc));
+        p[0] = (double)pl;
+    }
+    if (PLAQ) block_reduce_partial<1>(p, partials);
+}
+
+// tiles of the four-threads-per-site kernel: 64 sites (256 threads, two or three CTAs per SM) or
+// 128 sites (512 threads, one CTA per SM)
+typedef Tiled<8, 2, 2, 2> Tile64A;
+typedef Tiled<16, 2, 2, 1> Tile64B;
+typedef Tiled<4, 4, 2, 2> Tile64C;
+
+template <typename T, typename MAP, int MINB>
+int smear_mu4_launch(lqx_ctx* ctx, const Links<T>& in, const LinksOut<T>& o, T c0, T c1, double* plaq) {
+    const Geo& g = ctx->geo;
+    const int grid = MAP::grid(g);
+    const TileMap tm = MAP::map(g, kSlabZ);
+    if (plaq) {
+        int rc = lqx_ensure_partials(ctx, (size_t)grid);
+        if (rc) return rc;
+    }
+    const dim3 blk(MAP::THREADS, 4);
+    LqxTimed timed(ctx, LQX_K_SMEAR);
+    if (plaq) k_smear_mu4<T, true, MAP, MINB><<<grid, blk, 0, ctx->stream>>>(g, tm, in, o, c0, c1, ctx->d_partials, ctx->d_ticket, plaq);
+    else k_smear_mu4<T, false, MAP, MINB><<<grid, blk, 0, ctx->stream>>>(g, tm, in, o, c0, c1, nullptr, nullptr, nullptr);
+    LQX_LAUNCH_CHECK(ctx);
+    return plaq ? lqx_sum_partials(ctx, grid, 1, plaq) : LQX_OK;
+}
+
+template <typename T>
+int smear_launch_t(lqx_ctx* ctx, lqx_field* const uout[4], const lqx_field* const uin[4], double alpha, int only_mu,
+                   double* plaq) {
+    const Geo& g = ctx->geo;
+    LinksOut<T> o;
+    for (int mu = 0; mu < 4; ++mu) o.u[mu] = uout[mu] ? (T*)uout[mu]->data : nullptr;
+    const Links<T> in = make_links<T>(uin);
+    const T c0 = (T)(1.0 - alpha), c1 = (T)(alpha / 6.0);
+    int variant = ctx->opt_smear_variant;
+    if (variant != 1 && variant != 4) variant = 3;
+    if (only_mu >= 0) variant = 1;
+    if (variant == 4) {
+        // option "tile": 1 = 8x2x2x2, 2 = 16x2x2x1, 3 = 4x4x2x2 (64 sites); 4 = 8x4x2x2, 5 = 16x2x2x2 (128 sites)
+        const int t = ctx->opt_tile;
+        int rc = 1;
+        constexpr int MB64 = sizeof(T) == 4 ? 3 : 1;
+        if ((t == 1 || t < 0) && Tile64A::fits(g)) rc = smear_mu4_launch<T, Tile64A, MB64>(ctx, in, o, c0, c1, plaq);
+        else if (t == 2 && Tile64B::fits(g)) rc = smear_mu4_launch<T, Tile64B, MB64>(ctx, in, o, c0, c1, plaq);
+        else if ((t == 3 || t < 0) && Tile64C::fits(g)) rc = smear_mu4_launch<T, Tile64C, MB64>(ctx, in, o, c0, c1, plaq);
+        else if (t == 4 && TileB::fits(g)) rc = smear_mu4_launch<T, TileB, 1>(ctx, in, o, c0, c1, plaq);
+        else if (t == 5 && TileE::fits(g)) rc = smear_mu4_launch<T, TileE, 1>(ctx, in, o, c0, c1, plaq);
+        if (rc <= 0) return rc;
+        variant = 3;  // no tile of this kernel divides the lattice
+    }
+    const int choice = lqx_pick_tile(ctx, sizeof(T) == 4 ? 1 : 0);  // measured best
+    int nblocks = 0;
+    LQX_WITH_MAP(choice, {
+        const int grid = MAP::grid(g);
+        nblocks = grid;
+        const TileMap tm = MAP::map(g, kSlabZ);
+        if (plaq) {
+            int rc = lqx_ensure_partials(ctx, (size_t)grid);
+            if (rc) return rc;
+        }
+        double* part = plaq ? ctx->d_partials : nullptr;
+        unsigned int* tick = plaq ? ctx->d_ticket : nullptr;
+        LqxTimed timed(ctx, LQX_K_SMEAR);
+        if (variant == 1) {
+            if (plaq) k_smear_gather<T, true, MAP><<<grid, MAP::THREADS, 0, ctx->stream>>>(g, tm, in, o, c0, c1, only_mu, part, tick, plaq);
+            else k_smear_gather<T, false, MAP><<<grid, MAP::THREADS, 0, ctx->stream>>>(g, tm, in, o, c0, c1, only_mu, part, tick, plaq);
+        } else {
+            constexpr int MB = sizeof(T) == 4 ? (MAP::THREADS >= 256 ? 3 : 6) : (MAP::THREADS >= 256 ? 1 : 3);
+            if (plaq) k_smear_rolled<T, true, MAP, MB><<<grid, MAP::THREADS, 0, ctx->stream>>>(g, tm, in, o, c0, c1, part, tick, plaq);
+            else k_smear_rolled<T, false, MAP, MB><<<grid, MAP::THREADS, 0, ctx->stream>>>(g, tm, in, o, c0, c1, part, tick, plaq);
+        }
+    })
+    LQX_LAUNCH_CHECK(ctx);
+    return plaq ? lqx_sum_partials(ctx, nblocks, 1, plaq) : LQX_OK;
+}
+
+}  // namespace
+
+int lqx_smear_launch(lqx_ctx* ctx, lqx_field* const uout[4], const lqx_field* const uin[4], double alpha, int only_mu,
+                     double* plaq) {
+    return uin[0]->prec == LQX_F32 ? smear_launch_t<float>(ctx, uout, uin, alpha, only_mu, plaq)
+                                   : smear_launch_t<double>(ctx, uout, uin, alpha, only_mu, plaq);
+}

@@ -19,10 +19,16 @@ static inline Links<T> make_links(const lqx_field* const u[4]) {
     return l;
 }
 
-// tile shapes the nearest-neighbour kernels are instantiated for (choice 1..3; 0 = Linear fallback)
-typedef Tiled<8, 4, 4, 2> TileA;  // 256 threads
-typedef Tiled<8, 4, 2, 2> TileB;  // 128 threads
-typedef Tiled<4, 4, 4, 2> TileC;  // 128 threads, for L0 % 8 != 0
+// tile shapes the nearest-neighbour kernels are instantiated for (choice 1..6; 0 = Linear fallback).
+// Wide-in-x tiles cost fewer L1 wavefronts for the x-shifted operands (a 16-byte-shifted row of
+// TX sites touches one extra 128-byte line per row), compact tiles reuse more neighbours in L1.
+typedef Tiled<8, 4, 4, 2> TileA;   // 256 threads
+typedef Tiled<8, 4, 2, 2> TileB;   // 128 threads
+typedef Tiled<4, 4, 4, 2> TileC;   // 128 threads, for L0 % 8 != 0
+typedef Tiled<16, 4, 2, 2> TileD;  // 256 threads
+typedef Tiled<16, 2, 2, 2> TileE;  // 128 threads
+typedef Tiled<32, 2, 2, 2> TileF;  // 256 threads
+static const int kNumTiles = 6;
 // first shape that divides the lattice (ctx option "tile" forces one if it fits); 0 = Linear
 int lqx_pick_tile(const lqx_ctx* ctx, int first_choice);
 
@@ -31,10 +37,18 @@ int lqx_pick_tile(const lqx_ctx* ctx, int first_choice);
         case 1: { typedef TileA MAP; __VA_ARGS__ } break;  \
         case 2: { typedef TileB MAP; __VA_ARGS__ } break;  \
         case 3: { typedef TileC MAP; __VA_ARGS__ } break;  \
+        case 4: { typedef TileD MAP; __VA_ARGS__ } break;  \
+        case 5: { typedef TileE MAP; __VA_ARGS__ } break;  \
+        case 6: { typedef TileF MAP; __VA_ARGS__ } break;  \
         default: { typedef Linear MAP; __VA_ARGS__ } break; \
     }
 
-// shared-corner smear step (lqx_smear.cu).  Returns LQX_OK, or 1 if this lattice / precision is
-// not covered and the caller should use the literal kernel.
-int lqx_smear_shared_launch(lqx_ctx* ctx, lqx_field* const uout[4], const lqx_field* const uin[4], double alpha,
-                            double* plaq_out);
+// z-extent (sites) of a slab of the tile visiting order: thick enough that the two re-read z-faces
+// are a small fraction, thin enough that three t-slices of a slab stay in L2
+static const int kSlabZ = 16;
+
+// One smear step (all four directions, only_mu < 0) or the bare staple sum of one direction
+// (only_mu >= 0, written to uout[0]) on the context's stream (lqx_smear.cu).  If plaq != nullptr the
+// plaquette sum of the INPUT field lands there (device or pinned host memory).
+int lqx_smear_launch(lqx_ctx* ctx, lqx_field* const uout[4], const lqx_field* const uin[4], double alpha, int only_mu,
+                     double* plaq);
