@@ -46,6 +46,29 @@ def _peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)", 1965.0
 
 
+def _ncu_traffic():
+    """DRAM bytes per launch of the dominant kernel from the newest committed ncu capture
+    (profiles/rNN?_smear*.md, rows dram__bytes_read.sum / dram__bytes_write.sum, last launch column).
+    bench.py never runs under ncu; this is the recorded figure, or (None, reason)."""
+    import glob
+    import re
+
+    files = sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_smear*.md")))
+    if not files:
+        return None, "no ncu capture under profiles/"
+    vals = {}
+    for line in open(files[-1]):
+        m = re.match(r"\|\s*dram__bytes_(read|write)\.sum\s*\|\s*(\w+)\s*\|(.*)\|\s*$", line)
+        if m:
+            scale = {"Gbyte": 1e9, "Mbyte": 1e6, "Kbyte": 1e3, "byte": 1.0}.get(m.group(2))
+            cols = [c.strip() for c in m.group(3).split("|")]
+            if scale and cols:
+                vals[m.group(1)] = float(cols[-1]) * scale
+    if len(vals) != 2:
+        return None, "dram__bytes rows not found in " + os.path.basename(files[-1])
+    return vals["read"] + vals["write"], "profiles/" + os.path.basename(files[-1])
+
+
 class ClockSampler(threading.Thread):
     """Polls SM clock and throttle reasons through NVML while the timed region runs."""
 
@@ -196,16 +219,29 @@ def _extras(torch, lqx, li, hbm_gbs):
     out = []
     flush = torch.zeros(64 * 1024 * 1024, dtype=torch.float32, device="cuda")  # 256 MB > L2
 
-    def add(name, prec, sites, reals_per_site, flops_per_site, fn, reps=10, cold=False):
+    def add(name, prec, sites, reals_per_site, flops_per_site, fn, reps=10, cold=False, lat=None, kclass=None):
+        """`ms` = the whole C-ABI call (for the synchronising entry points that includes the host sync);
+        with lat/kclass also `kernel_ms` = device time of that call's kernels (CUDA event pairs the
+        library records around its launches)."""
         for _ in range(3):
             fn()
         torch.cuda.synchronize()
+        if kclass is not None:
+            lat.set_option("time_kernels", 1)
+            lat.kernel_time(kclass)
         med, best = _time_kernel(torch, fn, reps, flush if cold else None)
         nbytes = sites * reals_per_site * (4 if prec == "f32" else 8)
-        out.append({"kernel": name, "dtype": prec, "ms": round(med, 5), "ms_best": round(best, 5),
-                    "site_evals_per_s": sites / (med * 1e-3), "alg_gbs": nbytes / (med * 1e-3) / 1e9,
-                    "hbm_frac": nbytes / (med * 1e-3) / 1e9 / hbm_gbs, "gflops": sites * flops_per_site / (med * 1e-3) / 1e9,
-                    "l2": "flushed between launches" if cold else "inputs larger than L2"})
+        row = {"kernel": name, "dtype": prec, "ms": round(med, 5), "ms_best": round(best, 5),
+               "site_evals_per_s": sites / (med * 1e-3), "alg_gbs": nbytes / (med * 1e-3) / 1e9,
+               "hbm_frac": nbytes / (med * 1e-3) / 1e9 / hbm_gbs, "gflops": sites * flops_per_site / (med * 1e-3) / 1e9,
+               "l2": "flushed between launches" if cold else "inputs larger than L2"}
+        if kclass is not None:
+            kms, n = lat.kernel_time(kclass)
+            lat.set_option("time_kernels", 0)
+            if n:
+                row["kernel_ms"] = round(kms / n, 5)
+                row["kernel_hbm_frac"] = nbytes / (kms / n * 1e-3) / 1e9 / hbm_gbs
+        out.append(row)
 
     # ---- C2: hop, 16^3x32 fp32 (working set 63 MB < L2: cold and warm)
     dims = li.CONFIGS["c2"]["dims"]
@@ -218,7 +254,21 @@ def _extras(torch, lqx, li, hbm_gbs):
         out[-1]["l2"] = "flushed between launches"
         add("hop c2 (L2-warm)", "f32", v, 120, 2280, lambda: lqx.hop(chi, u, psi), reps=20)
         out[-1]["l2"] = "warm: 63 MB working set fits the 126 MB L2"
-        add("hop+norm2 fused c2 (L2-cold, incl. sync)", "f32", v, 120, 2328, lambda: lqx.hop_norm2(chi, u, psi), reps=20, cold=True)
+        add("hop+norm2 fused c2 (L2-cold, incl. sync)", "f32", v, 120, 2328, lambda: lqx.hop_norm2(chi, u, psi), reps=20, cold=True,
+            lat=lat, kclass=lqx.K_HOP)
+    # ---- the same hop kernel on a lattice 16x larger (32^3x64: 1 GB moved), where launch ramp-up and
+    # drain no longer dominate: the kernel's own HBM fraction
+    dims = li.CONFIGS["c5"]["dims"]
+    for prec, pcode in (("f32", lqx.F32), ("f64", lqx.F64)):
+        with lqx.Lattice(dims) as lat:
+            u = []
+            for mu in range(4):
+                a = li._as_real(li.haar_su3_complex(2, mu, lat.volume, "cuda"), prec)
+                u.append(lat.alloc(lqx.COLORMAT, pcode).import_dev(a))
+                del a
+            psi = lat.alloc(lqx.FERMION, pcode).import_dev(li.gaussian_field(2, 10, dims, "f", prec, device="cuda"))
+            chi = lat.alloc(lqx.FERMION, pcode)
+            add("hop 32^3x64 (not a BASELINE config; size check)", prec, lat.volume, 120, 2280, lambda: lqx.hop(chi, u, psi), reps=10)
     # ---- C3: smear + plaquette, 32^3x64 fp64
     dims = li.CONFIGS["c3"]["dims"]
     with lqx.Lattice(dims) as lat:
@@ -227,8 +277,8 @@ def _extras(torch, lqx, li, hbm_gbs):
         v = lat.volume
         add("smear_step c3", "f64", v, 144, SMEAR_CANONICAL_FLOPS, lambda: lqx.smear_step(o, u, ALPHA), reps=6)
         add("smear_step+plaquette(in) fused c3 (incl. sync)", "f64", v, 144, SMEAR_CANONICAL_FLOPS + 108,
-            lambda: lqx.smear_step(o, u, ALPHA, want_plaq_in=True), reps=6)
-        add("plaquette c3 (incl. sync)", "f64", v, 72, 2591, lambda: lqx.plaquette(u), reps=6)
+            lambda: lqx.smear_step(o, u, ALPHA, want_plaq_in=True), reps=6, lat=lat, kclass=lqx.K_SMEAR)
+        add("plaquette c3 (incl. sync)", "f64", v, 72, 2591, lambda: lqx.plaquette(u), reps=6, lat=lat, kclass=lqx.K_PLAQUETTE)
     # ---- C5: catalogue sweep, 32^3x64, both precisions
     dims = li.CONFIGS["c5"]["dims"]
     for prec, pcode in (("f32", lqx.F32), ("f64", lqx.F64)):
@@ -246,9 +296,9 @@ def _extras(torch, lqx, li, hbm_gbs):
             add("form iii' 2.5*A-shift(B,FORWARD,0) c5", prec, v, 54, 36, lambda: lqx.ax_minus_shift(r, 2.5, cm[0], cm[1], lqx.FORWARD, 0))
             add("form iv M*v c5", prec, v, 30, 66, lambda: lqx.mat_vec(w, cm[0], vec))
             add("shift(A,FORWARD,3) c5", prec, v, 36, 0, lambda: lqx.shift(r, cm[0], lqx.FORWARD, 3))
-            add("norm2(colour matrix) c5 (incl. sync)", prec, v, 18, 36, lambda: lqx.norm2(cm[0]))
-            add("sum(colour matrix) c5 (incl. sync)", prec, v, 18, 18, lambda: lqx.sum(cm[0]))
-            add("trace(colour matrix) c5 (incl. sync)", prec, v, 6, 6, lambda: lqx.trace(cm[0]))
+            add("norm2(colour matrix) c5 (incl. sync)", prec, v, 18, 36, lambda: lqx.norm2(cm[0]), lat=lat, kclass=lqx.K_REDUCE)
+            add("sum(colour matrix) c5 (incl. sync)", prec, v, 18, 18, lambda: lqx.sum(cm[0]), lat=lat, kclass=lqx.K_REDUCE)
+            add("trace(colour matrix) c5 (incl. sync)", prec, v, 6, 6, lambda: lqx.trace(cm[0]), lat=lat, kclass=lqx.K_REDUCE)
     del flush
     torch.cuda.empty_cache()
     return out
@@ -312,6 +362,7 @@ def run_ours(args):
     lane_ops = V * SMEAR_LANE_OPS[variant]
     # FP-pipe peak from unit counts and clocks: 148 SMs x 128 fp32 (64 fp64) FMA lanes x sm_max
     alu_peak_tflops = 148 * (128 if prec == "f32" else 64) * 2 * sm_max * 1e6 / 1e12
+    traffic, traffic_src = _ncu_traffic() if (args.workload == "c4") else (None, "no capture for this workload")
     roofline = {
         "kernel": "k_smear_rolled (staple sum + smear update, fused input plaquette)",
         "bound": "alu", "achieved": 2 * lane_ops / (k_ms * 1e-3) / 1e12, "peak": alu_peak_tflops, "unit": "TFLOP/s",
@@ -320,7 +371,8 @@ def run_ours(args):
                        f"FMA-chain micro-benchmark in this run: {2 * fma_peak / 1e12:.1f} TFLOP/s"
                        + (f", packed f32x2: {2 * fma2_peak / 1e12:.1f}" if fma2_peak else ""),
         "flops_counted": f"executed FMA lane-ops x 2 ({SMEAR_LANE_OPS[variant]} lane-ops/site, {variant} evaluation)",
-        "traffic": None, "ms_per_launch": k_ms, "launches": smear_n,
+        "traffic": traffic, "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum)",
+        "traffic_source": traffic_src, "ms_per_launch": k_ms, "launches": smear_n,
         "hbm": {"bound": "hbm", "achieved": alg_bytes / (k_ms * 1e-3) / 1e9, "peak": hbm_gbs, "unit": "GB/s",
                 "frac": alg_bytes / (k_ms * 1e-3) / 1e9 / hbm_gbs, "peak_source": hbm_src,
                 "copy_kernel_this_run_gbs": copy_peak / 1e9, "alg_bytes_per_launch": alg_bytes},

@@ -231,6 +231,26 @@ __device__ __forceinline__ void store_site(T* __restrict__ base, int s, const T 
     }
 }
 
+// reals [R0, R0+NR) of site s of a field with NREAL reals per site (whole 128-bit chunks only)
+template <typename T, int NREAL, int R0, int NR>
+__device__ __forceinline__ void load_site_part(const T* __restrict__ base, int s, T (&r)[NR]) {
+    typedef typename Vec128<T>::type V;
+    constexpr int W = Vec128<T>::W;
+    static_assert(R0 % W == 0 && NR % W == 0 && R0 + NR <= (NREAL / W) * W, "whole chunks only");
+    const V* p = reinterpret_cast<const V*>(base + (size_t)(s >> 5) * (32 * NREAL)) + (s & 31);
+#pragma unroll
+    for (int q = 0; q < NR / W; ++q) unpack(__ldg(p + (R0 / W + q) * 32), &r[q * W]);
+}
+template <typename T, int NREAL, int R0, int NR>
+__device__ __forceinline__ void store_site_part(T* __restrict__ base, int s, const T (&r)[NR]) {
+    typedef typename Vec128<T>::type V;
+    constexpr int W = Vec128<T>::W;
+    static_assert(R0 % W == 0 && NR % W == 0 && R0 + NR <= (NREAL / W) * W, "whole chunks only");
+    V* p = reinterpret_cast<V*>(base + (size_t)(s >> 5) * (32 * NREAL)) + (s & 31);
+#pragma unroll
+    for (int q = 0; q < NR / W; ++q) p[(R0 / W + q) * 32] = pack(&r[q * W]);
+}
+
 // --------------------------------------------------------------------------------------------
 // device side: site algebra.  T = float or double.
 // Colour matrix element (i,j): QDP-order reals 2*(3*i+j) (re) and 2*(3*i+j)+1 (im).
@@ -509,20 +529,40 @@ __device__ __forceinline__ void block_reduce_finish(double (&v)[NC], double* __r
     __syncthreads();
     if (!last) return;
     __threadfence();  // acquire side, paid by the one finishing CTA; partials are then read from L2
-    for (int c = 0; c < NC; ++c) {
-        double t = 0.0;
-        for (int i = tid; i < nblocks; i += nthreads) t += __ldcg(partials + (size_t)c * nblocks + i);
+    if (NC <= 2) {  // few components: the whole CTA sums each one
+        for (int c = 0; c < NC; ++c) {
+            double t = 0.0;
+            for (int i = tid; i < nblocks; i += nthreads) t += __ldcg(partials + (size_t)c * nblocks + i);
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
-        __syncthreads();
-        if (lane == 0) sh[warp][0] = t;
-        __syncthreads();
-        if (warp == 0) {
-            t = (lane < nwarps) ? sh[lane][0] : 0.0;
+            for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+            __syncthreads();
+            if (lane == 0) sh[warp][0] = t;
+            __syncthreads();
+            if (warp == 0) {
+                t = (lane < nwarps) ? sh[lane][0] : 0.0;
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+                if (lane == 0) out[c] = t;
+            }
+        }
+    } else {  // many components (sum of a site object): one warp per component, all in parallel
+        for (int c = warp; c < NC; c += nwarps) {
+            const double* pc = partials + (size_t)c * nblocks;
+            double t0 = 0.0, t1 = 0.0, t2 = 0.0, t3 = 0.0;
+            int i = lane;
+            for (; i + 96 < nblocks; i += 128) {
+                t0 += __ldcg(pc + i);
+                t1 += __ldcg(pc + i + 32);
+                t2 += __ldcg(pc + i + 64);
+                t3 += __ldcg(pc + i + 96);
+            }
+            for (; i < nblocks; i += 32) t0 += __ldcg(pc + i);
+            double t = (t0 + t1) + (t2 + t3);
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
             if (lane == 0) out[c] = t;
         }
+        __syncthreads();
     }
     if (tid == 0) *ticket = 0u;  // ready for the next launch on this stream
 }

@@ -13,7 +13,7 @@ namespace {
 // (Listing 1 lines 25/27 summed over mu; Eq. 2; BASELINE configs[1])
 // ---------------------------------------------------------------------------------------------
 template <typename T, int NSPIN, bool NORM2, typename MAP>
-__global__ void __launch_bounds__(MAP::THREADS) k_hop(const __grid_constant__ Geo g, const __grid_constant__ TileMap tm,
+__global__ void __launch_bounds__(MAP::THREADS, sizeof(T) == 4 ? 1 : 512 / MAP::THREADS) k_hop(const __grid_constant__ Geo g, const __grid_constant__ TileMap tm,
                                                       const __grid_constant__ Links<T> u, const T* __restrict__ psi, T* __restrict__ chi,
                                                       double* __restrict__ partials, unsigned int* ticket, double* __restrict__ out) {
     int x[4], s;
@@ -102,7 +102,7 @@ int check_links(lqx_ctx** ctx_out, const lqx_field* const u[4]) {
 template <typename T>
 int plaquette_launch(lqx_ctx* ctx, const lqx_field* const u[4], double* out) {
     const Geo& g = ctx->geo;
-    const int choice = lqx_pick_tile(ctx, sizeof(T) == 4 ? 1 : 0);
+    const int choice = lqx_pick_tile(ctx, 0);  // measured: linear 128-site blocks beat every tile shape here
     int nblocks = 0;
     LQX_WITH_MAP(choice, {
         const int grid = MAP::grid(g);
@@ -157,7 +157,7 @@ static int hop_impl(lqx_field* chi, const lqx_field* const u[4], const lqx_field
     const Geo& g = ctx->geo;
     const bool n2 = norm2_out != nullptr;
     const bool ferm = psi->kind == LQX_FERMION;
-    const int choice = lqx_pick_tile(ctx, 2);
+    const int choice = lqx_pick_tile(ctx, 0);  // measured: linear blocks beat every tile shape for the hop
 #define LQX_HOP(T, NSPIN, N2)                                                                                      \
     k_hop<T, NSPIN, N2, MAP><<<grid, MAP::THREADS, 0, ctx->stream>>>(g, tm, make_links<T>(u), (const T*)psi->data, \
                                                                     (T*)chi->data, ctx->d_partials, ctx->d_ticket, ctx->h_result)

@@ -7,6 +7,10 @@
 //   1  k_smear_gather : mu outer / nu inner as run-time loops, one accumulator (also the staple_sum entry)
 //   3  k_smear_rolled : same order, neighbour indices in shared memory, U_mu(x) not held, register cap
 //                       that allows three 256-thread (six 128-thread) CTAs per SM in fp32  [default]
+//   4  k_smear_mu4    : four threads per site (one per link) on 64/128-site tiles whose operands fit L1
+// Tried and dropped: full unrolling of mu, nu (255 registers + spills), L1 prefetch
+// of the next staple's operands (4.3 ms: the L1 request path is the busy unit), nu-outer with four
+// accumulators (60 instead of 76 operand fetches, but 168 registers: 3.5 ms).
 #include "lqx_smear.cuh"
 
 #include <type_traits>
