@@ -192,9 +192,12 @@ enum { LQX_K_SMEAR = 0, LQX_K_PLAQUETTE = 1, LQX_K_HOP = 2, LQX_K_CATALOGUE = 3,
 int lqx_kernel_time(lqx_ctx* ctx, int kernel_class, double* total_ms, int* count);
 /* Number of kernels this context has launched since init (for bench.py's gpu_launches). */
 int64_t lqx_launch_count(const lqx_ctx* ctx);
-/* Options: "smear_variant" 0 = best available, 1 = literal 48-product kernel, 2 = shared-corner
- * kernel only; "tile" -1 = automatic, 0 = linear blocks, 1..3 = CTA tile shape of the
- * nearest-neighbour kernels; "time_kernels" 0/1 (see above).  DESIGN.md sec.6. */
+/* Options: "smear_variant" 0 or 3 = default (rolled literal kernel), 1 = first-cut literal kernel,
+ * 2 = shared-corner kernel (36 products, lower staples exchanged through shared memory), 4 = four
+ * threads per site; variants fall back to 3 where none of their tile shapes divides the lattice.
+ * "tile" -1 = automatic, 0 = linear 128-site blocks, 1..6 = CTA tile shape (8x4x4x2, 8x4x2x2,
+ * 4x4x4x2, 16x4x2x2, 16x2x2x2, 32x2x2x2) of the nearest-neighbour kernels, used if it divides the
+ * lattice.  "time_kernels" 0/1 (see above).  All variants agree within rounding; DESIGN.md sec.6. */
 int lqx_set_option(lqx_ctx* ctx, const char* key, int value);
 
 const char* lqx_strerror(int code);

@@ -163,6 +163,190 @@ __global__ void __launch_bounds__(MAP::THREADS, MINB) k_smear_rolled(const __gri
     if (PLAQ) block_reduce_partial<1>(p, partials);
 }
 
+// variant 2: shared-corner evaluation.  With Q = U_nu(x) U_mu(x+nu^) the thread of site x
+// gets, for the ordered pair (mu, nu), the upper staple of ITS link mu, Q adj(U_nu(x+mu^)), and the lower
+// staple of link nu at the neighbour x+mu^, adj(U_mu(x)) Q -- 36 products per site instead of 48 and 16
+// distinct operand matrices instead of 44.  The lower staples travel one site in direction mu through
+// shared memory: slot[site][link] (one 3x3 matrix each, laid out [link][chunk][site] so that neighbouring
+// sites are neighbouring 16-byte words: conflict-free even for the x-shifted site).  Phase mu = 0..3:
+//   (a) every thread: its three pairs (mu, nu != mu): upper staples into a register accumulator, lower
+//       staples added into slot[x+mu^][nu] if x+mu^ is inside the CTA's tile;
+//   (b) the lower staples that ENTER the tile through its low-mu face come from sites of the neighbouring
+//       tile: 3*THREADS/T_mu work items (face site, nu), spread evenly over the CTA's threads, each the
+//       literal two products adj(U_mu(y)) U_nu(y) U_mu(y+nu^), y = x-mu^, added into slot[x][nu];
+//   (c) the thread adds its accumulator into slot[x][mu];  __syncthreads().
+// In one phase every slot[.][link != mu] receives exactly one lower staple "from direction mu" (from the
+// in-tile neighbour or from a halo item) and slot[.][mu] only its owner's uppers, so the read-modify-
+// writes never collide and the summation order is fixed: results are bit-reproducible.
+// After the four phases U'_mu(x) = c0 U_mu(x) + c1 slot[x][mu].
+template <typename T, int NT>
+struct Slots {
+    typedef typename Vec128<T>::type V;
+    static constexpr int W = Vec128<T>::W, NFULL = 18 / W;
+    T* base;
+    __device__ __forceinline__ T* link(int l) const { return base + l * (18 * NT); }
+    __device__ __forceinline__ void zero(int site, int l) const {
+        T* b = link(l);
+        const T z[4] = {T(0), T(0), T(0), T(0)};
+#pragma unroll
+        for (int q = 0; q < NFULL; ++q) reinterpret_cast<V*>(b + q * W * NT)[site] = pack(z);
+        if (18 % W != 0) reinterpret_cast<float2*>(b + NFULL * W * NT)[site] = make_float2(0.f, 0.f);
+    }
+    __device__ __forceinline__ void add(int site, int l, const Mat3<T>& m) const {
+        T r[18];
+#pragma unroll
+        for (int i = 0; i < 3; ++i)
+#pragma unroll
+            for (int j = 0; j < 3; ++j) {
+                r[2 * (3 * i + j)] = m.re[i][j];
+                r[2 * (3 * i + j) + 1] = m.im[i][j];
+            }
+        T* b = link(l);
+#pragma unroll
+        for (int q = 0; q < NFULL; ++q) {
+            V* p = reinterpret_cast<V*>(b + q * W * NT) + site;
+            T o[W];
+            unpack(*p, o);
+#pragma unroll
+            for (int k = 0; k < W; ++k) o[k] += r[q * W + k];
+            *p = pack(o);
+        }
+        if (18 % W != 0) {
+            float2* p = reinterpret_cast<float2*>(b + NFULL * W * NT) + site;
+            float2 o = *p;
+            o.x += (float)r[NFULL * W];
+            o.y += (float)r[NFULL * W + 1];
+            *p = o;
+        }
+    }
+    __device__ __forceinline__ Mat3<T> get(int site, int l) const {
+        T r[18];
+        const T* b = link(l);
+#pragma unroll
+        for (int q = 0; q < NFULL; ++q) unpack(reinterpret_cast<const V*>(b + q * W * NT)[site], &r[q * W]);
+        if (18 % W != 0) {
+            const float2 o = reinterpret_cast<const float2*>(b + NFULL * W * NT)[site];
+            r[NFULL * W] = (T)o.x;
+            r[NFULL * W + 1] = (T)o.y;
+        }
+        Mat3<T> m;
+#pragma unroll
+        for (int i = 0; i < 3; ++i)
+#pragma unroll
+            for (int j = 0; j < 3; ++j) {
+                m.re[i][j] = r[2 * (3 * i + j)];
+                m.im[i][j] = r[2 * (3 * i + j) + 1];
+            }
+        return m;
+    }
+};
+
+template <typename T, bool PLAQ, typename MAP, int MINB>
+__global__ void __launch_bounds__(MAP::THREADS, MINB) k_smear_shared(const __grid_constant__ Geo g, const __grid_constant__ TileMap tm,
+                                                                     const __grid_constant__ Links<T> u, const __grid_constant__ LinksOut<T> out,
+                                                                     T c0, T c1, double* __restrict__ partials) {
+    constexpr int NT = MAP::THREADS;
+    constexpr int T0 = MAP::T0, T1 = MAP::T1, T2 = MAP::T2, T3 = MAP::T3;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    Slots<T, NT> slots;
+    slots.base = reinterpret_cast<T*>(smem_raw);
+    int(*nb)[NT] = reinterpret_cast<int(*)[NT]>(smem_raw + sizeof(T) * 4 * 18 * NT);  // [0..3] x+d^
+    int x[4], s;
+    MAP::site(g, tm, x, s);  // tiles always cover whole sites
+    const int tid = threadIdx.x;
+    const int l[4] = {tid % T0, (tid / T0) % T1, (tid / (T0 * T1)) % T2, tid / (T0 * T1 * T2)};
+    const int org[4] = {x[0] - l[0], x[1] - l[1], x[2] - l[2], x[3] - l[3]};
+#pragma unroll
+    for (int d = 0; d < 4; ++d) {
+        nb[d][tid] = (x[d] + 1 == g.L[d]) ? s - (g.L[d] - 1) * g.stride_site[d] : s + g.stride_site[d];
+        slots.zero(tid, d);
+    }
+    __syncthreads();
+    T pl = T(0);
+#pragma unroll 1
+    for (int mu = 0; mu < 4; ++mu) {
+        const T* __restrict__ umu_p = u.u[mu];
+        const int tmu = mu == 0 ? T0 : (mu == 1 ? T1 : (mu == 2 ? T2 : T3));
+        const int lsmu = mu == 0 ? 1 : (mu == 1 ? T0 : (mu == 2 ? T0 * T1 : T0 * T1 * T2));
+        {  // (a) the thread's own three pairs
+            const int xpmu = nb[mu][tid];
+            const bool inside = coord_of(l, mu) + 1 < tmu;
+            const Mat3<T> a = load_mat(umu_p, s);
+            Mat3<T> acc = zero_mat<T>();
+#pragma unroll 1
+            for (int nu = 3; nu >= 0; --nu) {
+                if (nu == mu) {
+                    if (PLAQ && mu < 3) pl += re_tr_na(a, acc);  // acc = sum_{nu>mu} upper_{mu,nu}
+                    continue;
+                }
+                const T* __restrict__ unu_p = u.u[nu];
+                const Mat3<T> q = mul_nn(load_mat(unu_p, s), load_mat(umu_p, nb[nu][tid]));
+                mac_na(acc, q, load_mat(unu_p, xpmu));
+                if (inside) slots.add(tid + lsmu, nu, mul_an(a, q));
+            }
+            // (c) needs no barrier before it: slot[.][mu] has no other writer in this phase
+            slots.add(tid, mu, acc);
+        }
+        {  // (b) lower staples entering through the low-mu face
+            const int nface = NT / tmu;
+#pragma unroll 1
+            for (int i = tid; i < 3 * nface; i += NT) {
+                const int k = i / nface;
+                int j = i - k * nface;
+                const int nu = k + (k >= mu ? 1 : 0);
+                int lc[4];
+                lc[0] = mu == 0 ? 0 : j % T0;
+                if (mu != 0) j /= T0;
+                lc[1] = mu == 1 ? 0 : j % T1;
+                if (mu != 1) j /= T1;
+                lc[2] = mu == 2 ? 0 : j % T2;
+                if (mu != 2) j /= T2;
+                lc[3] = mu == 3 ? 0 : j;
+                const int li = lc[0] + T0 * (lc[1] + T1 * (lc[2] + T2 * lc[3]));
+                const int gx[4] = {org[0] + lc[0], org[1] + lc[1], org[2] + lc[2], org[3] + lc[3]};
+                const int sx = gx[0] + g.L[0] * (gx[1] + g.L[1] * (gx[2] + g.L[2] * gx[3]));
+                const int sy = coord_of(gx, mu) == 0 ? sx + (g.L[mu] - 1) * g.stride_site[mu] : sx - g.stride_site[mu];
+                const int syn = coord_of(gx, nu) + 1 == g.L[nu] ? sy - (g.L[nu] - 1) * g.stride_site[nu] : sy + g.stride_site[nu];
+                const T* __restrict__ unu_p = u.u[nu];
+                const Mat3<T> t = mul_an(load_mat(umu_p, sy), load_mat(unu_p, sy));
+                slots.add(li, nu, mul_nn(t, load_mat(umu_p, syn)));
+            }
+        }
+        __syncthreads();
+    }
+#pragma unroll 1
+    for (int mu = 0; mu < 4; ++mu) store_mat(out.u[mu], s, smear_update(c0, c1, load_mat(u.u[mu], s), slots.get(tid, mu)));
+    if (PLAQ) {
+        double p[1] = {(double)pl};
+        block_reduce_partial<1>(p, partials);
+    }
+}
+
+template <typename T, typename MAP, int MINB>
+int smear_shared_launch(lqx_ctx* ctx, const Links<T>& in, const LinksOut<T>& o, T c0, T c1, double* plaq) {
+    const Geo& g = ctx->geo;
+    const int grid = MAP::grid(g);
+    const TileMap tm = MAP::map(g, kSlabZ);
+    const size_t smem = sizeof(T) * 4 * 18 * MAP::THREADS + sizeof(int) * 4 * MAP::THREADS;
+    static bool configured = false;  // per instantiation
+    if (!configured) {
+        LQX_CUDA(ctx, cudaFuncSetAttribute(k_smear_shared<T, true, MAP, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        LQX_CUDA(ctx, cudaFuncSetAttribute(k_smear_shared<T, false, MAP, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        configured = true;
+    }
+    if (plaq) {
+        int rc = lqx_ensure_partials(ctx, (size_t)grid);
+        if (rc) return rc;
+    }
+    {
+        LqxTimed timed(ctx, LQX_K_SMEAR);
+        if (plaq) k_smear_shared<T, true, MAP, MINB><<<grid, MAP::THREADS, smem, ctx->stream>>>(g, tm, in, o, c0, c1, ctx->d_partials);
+        else k_smear_shared<T, false, MAP, MINB><<<grid, MAP::THREADS, smem, ctx->stream>>>(g, tm, in, o, c0, c1, nullptr);
+    }
+    LQX_LAUNCH_CHECK(ctx);
+    return plaq ? lqx_sum_partials(ctx, grid, 1, plaq) : LQX_OK;
+}
+
 // variant 4: four threads per site -- thread (site, mu) evaluates the six staples of ONE link, so a
 // CTA of 4*TILE threads works on a TILE-site tile whose operand footprint (the tile, its faces and
 // edges: ~15 matrices per site) is small enough to stay in L1 while 16 warps per SM hide latency.
@@ -249,8 +433,21 @@ int smear_launch_t(lqx_ctx* ctx, lqx_field* const uout[4], const lqx_field* cons
     const Links<T> in = make_links<T>(uin);
     const T c0 = (T)(1.0 - alpha), c1 = (T)(alpha / 6.0);
     int variant = ctx->opt_smear_variant;
-    if (variant != 1 && variant != 4) variant = 3;
+    if (variant != 1 && variant != 2 && variant != 4) variant = 3;
     if (only_mu >= 0) variant = 1;
+    if (variant == 2) {
+        // option "tile": 1 = 8x4x4x2 (256 threads), 2 = 8x4x2x2, 3 = 4x4x4x2, 4 = 16x4x2x2 (256), 5 = 16x2x2x2
+        const int t = ctx->opt_tile;
+        int rc = 1;
+        constexpr int MB256 = sizeof(T) == 4 ? 2 : 1, MB128 = sizeof(T) == 4 ? 4 : 2;
+        if (sizeof(T) == 4 && (t == 1 || t < 0) && TileA::fits(g)) rc = smear_shared_launch<T, TileA, MB256>(ctx, in, o, c0, c1, plaq);
+        else if (sizeof(T) == 4 && t == 4 && TileD::fits(g)) rc = smear_shared_launch<T, TileD, MB256>(ctx, in, o, c0, c1, plaq);
+        else if ((t == 2 || t < 0) && TileB::fits(g)) rc = smear_shared_launch<T, TileB, MB128>(ctx, in, o, c0, c1, plaq);
+        else if (t == 5 && TileE::fits(g)) rc = smear_shared_launch<T, TileE, MB128>(ctx, in, o, c0, c1, plaq);
+        else if ((t == 3 || t < 0) && TileC::fits(g)) rc = smear_shared_launch<T, TileC, MB128>(ctx, in, o, c0, c1, plaq);
+        if (rc <= 0) return rc;
+        variant = 3;  // no tile of this kernel divides the lattice
+    }
     if (variant == 4) {
         // option "tile": 1 = 8x2x2x2, 2 = 16x2x2x1, 3 = 4x4x2x2 (64 sites); 4 = 8x4x2x2, 5 = 16x2x2x2 (128 sites)
         const int t = ctx->opt_tile;

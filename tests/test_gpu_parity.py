@@ -290,6 +290,44 @@ def test_staple_smear_plaquette(lqx, dims, prec):
         assert abs(ps2 - w2) / max(abs(w2), scale) < RTOL[prec]
 
 
+# every smear kernel variant (option "smear_variant": 1 literal gather, 2 shared-corner with the lower
+# staples exchanged through shared memory, 3 rolled literal = default, 4 four threads per site) and every
+# CTA tile shape that divides the lattice, against the truth oracle; 16x8x4x4 spans several tiles in every
+# direction for all shapes, 8x4x4x2 is exactly one 8x4x4x2 tile (every neighbour wraps into the same tile)
+@pytest.mark.parametrize("dims", [(16, 8, 4, 4), (8, 4, 4, 2), (4, 4, 4, 4)])
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+@pytest.mark.parametrize("variant", [1, 2, 3, 4])
+def test_smear_variants_and_tiles(lqx, dims, prec, variant):
+    tv = orc.truth_variant(prec)
+    u = _links(5, dims, prec)
+    want = orc.smear_step(dims, u, 0.5, tv)
+    psum_want = orc.plaquette_sum(dims, u, tv)
+    with lqx.Lattice(dims) as lat:
+        fu = [lat.from_host(t) for t in u]
+        out = [lat.alloc(lqx.COLORMAT, fu[0].prec) for _ in range(4)]
+        scale = np.sqrt(18.0 * lat.volume)
+        lat.set_option("smear_variant", variant)
+        first = None
+        for tile in (-1, 0, 1, 2, 3, 4, 5, 6):
+            lat.set_option("tile", tile)
+            for o in out:
+                lqx.scale(o, 0.0, o)
+            p = lqx.smear_step(out, fu, 0.5, want_plaq_in=True)
+            got = [o.pop() for o in out]
+            for mu in range(4):
+                assert site_rel_err(got[mu], want[mu]) < TOL[prec], (variant, tile, mu)
+            assert abs(p - psum_want) / max(abs(psum_want), scale) < RTOL[prec], (variant, tile)
+            # run to run, and whatever the tile shape of a given variant, the per-site arithmetic is fixed
+            lqx.smear_step(out, fu, 0.5, want_plaq_in=True)
+            for mu in range(4):
+                assert np.array_equal(out[mu].pop(), got[mu]), (variant, tile, mu)
+            if variant in (1, 3):  # variant 2 sums in an order that depends on the tile faces; 2 and 4 fall back to 3 for tiles they lack
+                if first is None:
+                    first = got
+                for mu in range(4):
+                    assert np.array_equal(got[mu], first[mu]), (variant, tile, mu)
+
+
 @pytest.mark.parametrize("prec", ["f32", "f64"])
 def test_unit_gauge_is_a_fixed_point(lqx, prec):
     dims = DIMS_EVEN
