@@ -120,8 +120,10 @@ class ClockSampler(threading.Thread):
                 "reasons": sorted(self.reasons), "samples": len(s)}
 
 
-def _dist():
-    """(rank, world, local_rank, barrier_fn, max_fn) -- torch.distributed only when launched by torchrun."""
+def _dist(backend="nccl"):
+    """(rank, world, local_rank, barrier_fn, max_fn) -- torch.distributed only when launched by torchrun.
+    The path does not shard: the group is used for the barrier and the max over ranks
+    only.  backend "gloo" is what the CPU tests use (world_size 2, no GPU)."""
     world = int(os.environ.get("WORLD_SIZE", "1"))
     if world <= 1:
         return 0, 1, 0, (lambda: None), (lambda x: x)
@@ -129,15 +131,26 @@ def _dist():
     import torch.distributed as dist
 
     rank, local = int(os.environ["RANK"]), int(os.environ.get("LOCAL_RANK", "0"))
-    torch.cuda.set_device(local)
-    dist.init_process_group(backend="nccl", device_id=torch.device(f"cuda:{local}"))
+    if backend == "nccl":
+        torch.cuda.set_device(local)
+        dist.init_process_group(backend="nccl", device_id=torch.device(f"cuda:{local}"))
+        dev = f"cuda:{local}"
+    else:
+        dist.init_process_group(backend=backend)
+        dev = "cpu"
 
     def vmax(x):
-        t = torch.tensor([float(x)], dtype=torch.float64, device=f"cuda:{local}")
+        t = torch.tensor([float(x)], dtype=torch.float64, device=dev)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         return float(t.item())
 
     return rank, world, local, dist.barrier, vmax
+
+
+def replica_value(world, sites, steps, ms_max):
+    """Whole-job throughput of N independent replicas: every rank updates `sites` sites `steps` times and
+    the job takes as long as its slowest rank."""
+    return world * sites * steps / (ms_max * 1e-3)
 
 
 def _gen_links(lat, lqx, li, cfgname, recipe, prec, keep_host=False):
@@ -355,7 +368,7 @@ def run_ours(args):
     plaq_ms, plaq_n = lat.kernel_time(lqx.K_PLAQUETTE)
     lat.set_option("time_kernels", 0)
 
-    value = world * V * K / (ms * 1e-3)
+    value = replica_value(world, V, K, ms)
     k_ms = smear_ms / max(smear_n, 1)  # average duration of the dominant kernel inside the timed region
     alg_bytes = V * SMEAR_REALS_PER_SITE * esize
     variant = "literal"
