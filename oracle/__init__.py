@@ -175,6 +175,18 @@ def hop(dims, u, psi, variant, listing_form=False):
     return chi
 
 
+def jacobi_smear(dims, u, chi, kappa, iters, no_smear_dir, norm, variant):
+    """Listing 1 of the paper, step by step: power series in kappa of the hopping term
+    applied to chi, divided by norm.  no_smear_dir outside 0..3 smears in all four directions."""
+    u = [_inp(t, variant) for t in u]
+    chi = _inp(chi, variant)
+    out = _out(chi.shape, variant)
+    getattr(lib(), f"orc_jacobi_smear_{variant}")(_dims(dims), C.c_int(_nspin(chi, dims)), _p(u[0]), _p(u[1]), _p(u[2]),
+                                                  _p(u[3]), _p(chi), C.c_double(kappa), C.c_int(iters),
+                                                  C.c_int(no_smear_dir), C.c_double(norm), _p(out))
+    return out
+
+
 # ---------------------------------------------------------------- reductions
 def sum_field(dims, f, variant):
     f = _inp(f, variant)

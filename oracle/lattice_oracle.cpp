@@ -34,6 +34,8 @@
 // gauge invariance of the plaquette and covariance of hop and smear step (the transformation
 // is applied with numpy, not with this file); U(1) plane-wave eigenvalue of the hop; point
 // source; sum_{x,mu} Re tr[U S^dag] = 4 * plaquette sum; numpy einsum cross-checks on 2^4.
+// Jacobi routine (tests/test_jacobi_pins.py): truncated power series of Eq. 2 built with numpy rolls,
+// geometric series on unit links, U(1) plane-wave eigenvalue, gauge covariance, iter = 0 / kappa = 0.
 // Parity unpinned: nothing -- every exported function has at least one such pin; absolute
 // values on the random configs have no printed reference in the paper (there is none).
 // ============================================================================================
@@ -330,6 +332,62 @@ void hop_listing(const Geom& g, int nspin, const S* const u[4], const S* psi, O*
         for (int a = 0; a < nspin; ++a) store_vec(chi, s, nspin, a, acc[s * nspin + a]);
 }
 
+// ------------------------------------------------------------------ Jacobi smearing
+// Listing 1 of the paper, step by step in its order (readings A2, A3):
+//   s_0 = chi                                                        (line 16, E0)
+//   for n = 0 .. iter-1:
+//       psi = chi                                                    (line 20, E0)
+//       for mu = 0 .. Nd-1, mu != no_smear_dir:
+//           first mu :  h_smear  = u[mu]*shift(psi,FORWARD,mu) + shift(adj(u[mu])*psi,BACKWARD,mu)   (line 25, E1)
+//           later mu :  h_smear += (the same expression)                                             (line 27, E2)
+//       chi = s_0 + kappa * h_smear                                  (line 30, E3)
+//   chi /= norm                                                      (line 33, E4)
+// which is the power series sum_{n<=iter} kappa^n H^n s_0 / norm of the inverse of K, Eq. 2.
+// Intermediate fields are kept in the arithmetic type A (for the native instantiations A is the storage
+// type, as in a QDP++ build of that precision; for the truth instantiations nothing is rounded on the way).
+template <typename S, typename A, typename O>
+void jacobi_smear(const Geom& g, int nspin, const S* const u[4], const S* chi_in, double kappa, int iter, int no_smear_dir,
+                  double norm, O* chi_out) {
+    const size_t n = (size_t)g.V * nspin;
+    std::vector<Vec<A>> s0(n), chi(n), psi(n), h(n);
+    for (long s = 0; s < g.V; ++s)
+        for (int a = 0; a < nspin; ++a) s0[s * nspin + a] = chi[s * nspin + a] = load_vec<A>(chi_in, s, nspin, a);
+    const A k = (A)(S)kappa, nrm = (A)(S)norm;
+    for (int it = 0; it < iter; ++it) {
+        psi = chi;
+        bool first = true;
+        for (int mu = 0; mu < 4; ++mu) {
+            if (mu == no_smear_dir) continue;
+#pragma omp parallel for schedule(static)
+            for (long s = 0; s < g.V; ++s) {
+                const long f = nbr(g, s, +1, mu), b = nbr(g, s, -1, mu);
+                const Mat<A> uf = load_mat<A>(u[mu], s), ub = adj(load_mat<A>(u[mu], b));
+                for (int a = 0; a < nspin; ++a) {
+                    const Vec<A> t = add(mul(uf, psi[f * nspin + a]), mul(ub, psi[b * nspin + a]));
+                    h[s * nspin + a] = first ? t : add(h[s * nspin + a], t);
+                }
+            }
+            first = false;
+        }
+#pragma omp parallel for schedule(static)
+        for (long i = 0; i < (long)n; ++i)
+            for (int c = 0; c < 3; ++c) {
+                const Cx<A> hh = first ? Cx<A>{(A)0, (A)0} : h[i].e[c];  // every direction excluded: h_smear = 0
+                chi[i].e[c].re = s0[i].e[c].re + k * hh.re;
+                chi[i].e[c].im = s0[i].e[c].im + k * hh.im;
+            }
+    }
+    for (long s = 0; s < g.V; ++s)
+        for (int a = 0; a < nspin; ++a) {
+            Vec<A> v = chi[s * nspin + a];
+            for (int c = 0; c < 3; ++c) {
+                v.e[c].re = v.e[c].re / nrm;
+                v.e[c].im = v.e[c].im / nrm;
+            }
+            store_vec(chi_out, s, nspin, a, v);
+        }
+}
+
 // ------------------------------------------------------------------ O4 reductions (row a9)
 // sum(f): one site object; out[2*ncx] doubles in QDP order.
 template <typename S, typename A>
@@ -506,6 +564,12 @@ void orc_shift_f64(const int* dims, int nreal, const double* in, double* out, in
                                const S* u3, const S* psi, O* chi) {                                        \
         const S* u[4] = {u0, u1, u2, u3};                                                                  \
         hop_listing<S, A, O>(make_geom(dims), nspin, u, psi, chi);                                         \
+    }                                                                                                      \
+    void orc_jacobi_smear_##SUF(const int* dims, int nspin, const S* u0, const S* u1, const S* u2,         \
+                                const S* u3, const S* chi, double kappa, int iter, int no_smear_dir,       \
+                                double norm, O* out) {                                                     \
+        const S* u[4] = {u0, u1, u2, u3};                                                                  \
+        jacobi_smear<S, A, O>(make_geom(dims), nspin, u, chi, kappa, iter, no_smear_dir, norm, out);       \
     }                                                                                                      \
     void orc_sum_##SUF(const int* dims, int ncx, const S* f, double* out) {                                \
         sum_field<S, A>(make_geom(dims), ncx, f, out);                                                     \
