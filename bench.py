@@ -282,6 +282,24 @@ def _extras(torch, lqx, li, hbm_gbs):
             psi = lat.alloc(lqx.FERMION, pcode).import_dev(li.gaussian_field(2, 10, dims, "f", prec, device="cuda"))
             chi = lat.alloc(lqx.FERMION, pcode)
             add("hop 32^3x64 (not a BASELINE config; size check)", prec, lat.volume, 120, 2280, lambda: lqx.hop(chi, u, psi), reps=10)
+    # ---- NEXT-1: the paper's complete Jacobi smearing routine at its Table 1 sizes 16^3x32 and 32^3x64
+    # (PAPER.md:228-238), fermion field, 20 iterations, all four directions.  Per iteration and site the fused
+    # kernel moves U 72 + psi 24 + s_0 24 + chi 24 = 144 reals and does 2280 (hop) + 48 (E3) canonical flops.
+    JIT = 20
+    for dims in (li.CONFIGS["c2"]["dims"], li.CONFIGS["c5"]["dims"]):
+        for prec, pcode in (("f32", lqx.F32), ("f64", lqx.F64)):
+            with lqx.Lattice(dims) as lat:
+                u = []
+                for mu in range(4):
+                    a = li._as_real(li.haar_su3_complex(2, mu, lat.volume, "cuda"), prec)
+                    u.append(lat.alloc(lqx.COLORMAT, pcode).import_dev(a))
+                    del a
+                chi = lat.alloc(lqx.FERMION, pcode).import_dev(li.gaussian_field(2, 10, dims, "f", prec, device="cuda"))
+                tmp = [lat.alloc(lqx.FERMION, pcode) for _ in range(2)]
+                add(f"jacobi_smear {dims[0]}^3x{dims[3]} x{JIT} iterations (NEXT-1; paper Table 1 size)", prec, lat.volume * JIT,
+                    144, 2328, lambda: lqx.jacobi_smear(chi, u, 0.01, JIT, -1, 1.0, tmp), reps=10)
+                out[-1]["l2"] = "iterated on resident fields (working set %.0f MB)" % (lat.volume * 168 * (4 if prec == "f32" else 8) / 1e6)
+                out[-1]["paper_gflops_gtx480"] = {(16, "f32"): 11.86, (16, "f64"): 6.26, (32, "f32"): 21.31}.get((dims[0], prec))
     # ---- C3: smear + plaquette, 32^3x64 fp64
     dims = li.CONFIGS["c3"]["dims"]
     with lqx.Lattice(dims) as lat:

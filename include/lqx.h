@@ -140,6 +140,16 @@ int lqx_axpy(lqx_field* r, const lqx_field* s0, double kappa, const lqx_field* h
 int lqx_scale(lqx_field* r, double s, const lqx_field* a);
 int lqx_divide(lqx_field* r, const lqx_field* a, double nrm);
 
+/* The paper's complete routine (Listing 1 jacobiSmear; Eq. 1-2 :208-218; readings
+ * A2, A3):  s_0 = chi;  iter x { psi = chi;  h = sum_{mu != no_smear_dir} u[mu]*shift(psi,FORWARD,mu)
+ * + shift(adj(u[mu])*psi,BACKWARD,mu);  chi = s_0 + kappa*h };  chi /= norm  -- the power series
+ * sum_{n<=iter} kappa^n H^n chi / norm.  One fused kernel per iteration (E0-E3; E4 in the last).
+ * chi (fermion or colour vector) is input and output; tmp[2] are caller-provided scratch fields of
+ * chi's kind and precision, all distinct.  no_smear_dir outside 0..3 smears in all four directions.
+ * Asynchronous.  LQX_EINVAL for iter < 0 or norm == 0. */
+int lqx_jacobi_smear(lqx_field* chi, const lqx_field* const u[4], double kappa, int iter,
+                     int no_smear_dir, double norm, lqx_field* const tmp[2]);
+
 /* ---------------------------------------------------------------------------------------------
  * Global reductions.  fp64 accumulation for both precisions, fixed summation
  * tree (deterministic run to run).  Results to host double; these calls synchronise.

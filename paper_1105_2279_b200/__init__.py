@@ -76,6 +76,7 @@ SIGNATURES = {
     "lqx_mat_vec": (_i, [_vp, _vp, _vp]),
     "lqx_hop": (_i, [_vp, _pvp, _vp]),
     "lqx_hop_norm2": (_i, [_vp, _pvp, _vp, _pd]),
+    "lqx_jacobi_smear": (_i, [_vp, _pvp, _d, _i, _i, _d, _pvp]),
     "lqx_axpy": (_i, [_vp, _vp, _d, _vp]),
     "lqx_scale": (_i, [_vp, _d, _vp]),
     "lqx_divide": (_i, [_vp, _vp, _d]),
@@ -312,6 +313,12 @@ def hop_norm2(chi, u, psi) -> float:
     out = C.c_double()
     _check(_lib.lqx_hop_norm2(_h(chi), _arr4(u), _h(psi), C.byref(out)), _ctx_of(chi))
     return out.value
+
+
+def jacobi_smear(chi, u, kappa, iters, no_smear_dir, norm, tmp):
+    """chi <- sum_{n<=iters} kappa^n H^n chi / norm (Listing 1 of the paper); tmp = two scratch fields."""
+    arr = (C.c_void_p * 2)(_h(tmp[0]), _h(tmp[1]))
+    _check(_lib.lqx_jacobi_smear(_h(chi), _arr4(u), float(kappa), int(iters), int(no_smear_dir), float(norm), arr), _ctx_of(chi))
 
 
 def axpy(r, s0, kappa, h):

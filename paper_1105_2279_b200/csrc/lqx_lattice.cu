@@ -57,6 +57,62 @@ __global__ void __launch_bounds__(MAP::THREADS, sizeof(T) == 4 ? 1 : 512 / MAP::
 }
 
 // ---------------------------------------------------------------------------------------------
+// One iteration of the paper's Jacobi smearing routine (Listing 1 lines 20-30):
+//   chi_new(x) = s_0(x) + kappa * sum_{mu != no_smear_dir} [U_mu(x) psi(x+mu^) + adj(U_mu(x-mu^)) psi(x-mu^)]
+// i.e. E0 (psi = chi: here the ping-pong), E1, E2 x (Nd-1) and E3 of the listing in ONE pass instead of
+// six; DIV: the last iteration also applies E4, chi /= norm (a true division, reading A22).
+// dirmask bit mu = direction mu takes part.
+// ---------------------------------------------------------------------------------------------
+template <typename T, int NSPIN, bool DIV>
+__global__ void __launch_bounds__(128, sizeof(T) == 4 ? 6 : 4) k_jacobi_step(const __grid_constant__ Geo g, const __grid_constant__ Links<T> u,
+                                                                             int dirmask, const T* __restrict__ psi, const T* __restrict__ s0,
+                                                                             T kappa, T nrm, T* __restrict__ chi) {
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= g.V) return;
+    int x[4];
+    site_coords(g, s, x);
+    Vec3<T> acc[NSPIN];
+#pragma unroll
+    for (int a = 0; a < NSPIN; ++a)
+#pragma unroll
+        for (int i = 0; i < 3; ++i) acc[a].re[i] = acc[a].im[i] = T(0);
+#pragma unroll
+    for (int mu = 0; mu < 4; ++mu) {
+        if (!((dirmask >> mu) & 1)) continue;
+        const int f = nbr_fwd(g, s, x, mu), b = nbr_bwd(g, s, x, mu);
+        {
+            const Mat3<T> m = load_mat(u.u[mu], s);
+            Vec3<T> v[NSPIN];
+            load_vecs<T, NSPIN>(psi, f, v);
+#pragma unroll
+            for (int a = 0; a < NSPIN; ++a) mac_mv(acc[a], m, v[a]);
+        }
+        {
+            const Mat3<T> m = load_mat(u.u[mu], b);
+            Vec3<T> v[NSPIN];
+            load_vecs<T, NSPIN>(psi, b, v);
+#pragma unroll
+            for (int a = 0; a < NSPIN; ++a) mac_adj_mv(acc[a], m, v[a]);
+        }
+    }
+    Vec3<T> src[NSPIN];
+    load_vecs<T, NSPIN>(s0, s, src);
+#pragma unroll
+    for (int a = 0; a < NSPIN; ++a)
+#pragma unroll
+        for (int i = 0; i < 3; ++i) {
+            T re = fma(kappa, acc[a].re[i], src[a].re[i]), im = fma(kappa, acc[a].im[i], src[a].im[i]);
+            if (DIV) {
+                re = re / nrm;
+                im = im / nrm;
+            }
+            acc[a].re[i] = re;
+            acc[a].im[i] = im;
+        }
+    store_vecs<T, NSPIN>(chi, s, acc);
+}
+
+// ---------------------------------------------------------------------------------------------
 // plaquette: sum_{mu<nu} Re tr[U_mu(x) U_nu(x+mu^) adj(U_mu(x+nu^)) adj(U_nu(x))]
 //          = sum_{mu<nu} Re tr[Q_munu(x) adj(Q_numu(x))],  Q_ab(x) = U_a(x) U_b(x+a^)
 // ---------------------------------------------------------------------------------------------
@@ -326,4 +382,57 @@ extern "C" int lqx_smear_iterate_host(lqx_ctx* ctx, lqx_prec prec, const void* c
         if (t[mu]) lqx_field_free(t[mu]);
     }
     return rc;
+}
+
+// The paper's routine (Listing 1): chi <- sum_{n<=iter} kappa^n H^n chi / norm.
+extern "C" int lqx_jacobi_smear(lqx_field* chi, const lqx_field* const u[4], double kappa, int iter, int no_smear_dir,
+                                double norm, lqx_field* const tmp[2]) {
+    lqx_ctx* ctx;
+    int rc = check_links(&ctx, u);
+    if (rc) return rc;
+    if (!chi || !tmp || !tmp[0] || !tmp[1]) return LQX_EINVAL;
+    if (iter < 0) return lqx_fail(ctx, LQX_EINVAL, "jacobi_smear: iter < 0");
+    if (norm == 0.0) return lqx_fail(ctx, LQX_EINVAL, "jacobi_smear: norm == 0");
+    if (chi->kind != LQX_FERMION && chi->kind != LQX_COLORVEC) return lqx_fail(ctx, LQX_ETYPE, "jacobi_smear: chi must be a fermion or a colour vector");
+    for (int k = 0; k < 2; ++k) {
+        if (tmp[k]->ctx != ctx || chi->ctx != ctx) return lqx_fail(ctx, LQX_EGEOM, "jacobi_smear: different contexts");
+        if (tmp[k]->kind != chi->kind || tmp[k]->prec != chi->prec) return lqx_fail(ctx, LQX_ETYPE, "jacobi_smear: scratch fields must match chi");
+        if (lqx_same(tmp[k], chi)) return lqx_fail(ctx, LQX_EALIAS, "jacobi_smear: scratch aliases chi");
+    }
+    if (lqx_same(tmp[0], tmp[1])) return lqx_fail(ctx, LQX_EALIAS, "jacobi_smear: scratch fields alias each other");
+    if (chi->prec != u[0]->prec) return lqx_fail(ctx, LQX_ETYPE, "jacobi_smear: mixed precision");
+    LQX_CUDA(ctx, cudaSetDevice(ctx->device));
+    if (iter == 0) return lqx_divide(chi, chi, norm);  // s_0 = chi; chi /= norm
+    const Geo& g = ctx->geo;
+    int dirmask = 0xF;
+    if (no_smear_dir >= 0 && no_smear_dir < 4) dirmask &= ~(1 << no_smear_dir);
+    // s_0 = chi (E0, Listing line 16).  The iterate ping-pongs so that the last write lands in chi: for an odd
+    // iteration count the first iteration reads the copy and writes chi, otherwise it reads chi and writes tmp[1].
+    rc = lqx_copy(tmp[0], chi);
+    if (rc) return rc;
+    const lqx_field* cur = (iter & 1) ? tmp[0] : chi;
+    lqx_field* nxt = (iter & 1) ? chi : tmp[1];
+    const int grid = (g.V + 127) / 128;
+    const bool ferm = chi->kind == LQX_FERMION;
+    for (int it = 0; it < iter; ++it) {
+        const bool last = it == iter - 1;
+        {
+            LqxTimed timed(ctx, LQX_K_HOP);
+#define LQX_JAC(T, NSPIN, DIV)                                                                                                   \
+    k_jacobi_step<T, NSPIN, DIV><<<grid, 128, 0, ctx->stream>>>(g, make_links<T>(u), dirmask, (const T*)cur->data,           \
+                                                                (const T*)tmp[0]->data, (T)kappa, (T)norm, (T*)nxt->data)
+            if (chi->prec == LQX_F32) {
+                if (ferm) { if (last) LQX_JAC(float, 4, true); else LQX_JAC(float, 4, false); }
+                else      { if (last) LQX_JAC(float, 1, true); else LQX_JAC(float, 1, false); }
+            } else {
+                if (ferm) { if (last) LQX_JAC(double, 4, true); else LQX_JAC(double, 4, false); }
+                else      { if (last) LQX_JAC(double, 1, true); else LQX_JAC(double, 1, false); }
+            }
+#undef LQX_JAC
+        }
+        LQX_LAUNCH_CHECK(ctx);
+        cur = nxt;
+        nxt = (nxt == chi) ? tmp[1] : chi;
+    }
+    return LQX_OK;
 }

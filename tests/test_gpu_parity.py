@@ -407,3 +407,47 @@ def test_error_codes(lqx):
         assert code(lqx.hop, v32, u, v32) == -4
         with pytest.raises(lqx.LqxError):
             lqx.Lattice((4, 0, 4, 4))
+
+
+# ------------------------------------------------------------------------------------------------
+# NEXT-1: the paper's complete Jacobi smearing routine (Listing 1)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dims", [DIMS_RAGGED, DIMS_EVEN, (2, 2, 2, 2)])
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+@pytest.mark.parametrize("kind", ["f", "cv"])
+def test_jacobi_smear(lqx, dims, prec, kind):
+    tv = orc.truth_variant(prec)
+    u = _links(2, dims, prec)
+    chi0 = _gauss(2, 10, dims, kind, prec)
+    with lqx.Lattice(dims) as lat:
+        fu = [lat.from_host(t) for t in u]
+        for (kappa, iters, skip, norm) in [(0.21, 5, -1, 1.7), (0.21, 4, 3, 1.7), (0.3, 1, 0, 0.5), (0.3, 0, -1, 2.0), (0.1, 2, 9, 1.0)]:
+            chi = lat.from_host(chi0)
+            tmp = [lat.alloc(chi.kind, chi.prec) for _ in range(2)]
+            lqx.jacobi_smear(chi, fu, kappa, iters, skip, norm, tmp)
+            want = orc.jacobi_smear(dims, u, chi0, kappa, iters, skip, norm, tv)
+            assert site_rel_err(chi.pop(), want) < TOL[prec] * max(1, iters), (kappa, iters, skip)
+        # error behaviour: scratch must not alias, iter >= 0, norm != 0
+        chi = lat.from_host(chi0)
+        t0 = lat.alloc(chi.kind, chi.prec)
+        for bad in (lambda: lqx.jacobi_smear(chi, fu, 0.1, 2, -1, 1.0, [t0, t0]),
+                    lambda: lqx.jacobi_smear(chi, fu, 0.1, 2, -1, 1.0, [chi, t0]),
+                    lambda: lqx.jacobi_smear(chi, fu, 0.1, -1, -1, 1.0, [t0, lat.alloc(chi.kind, chi.prec)]),
+                    lambda: lqx.jacobi_smear(chi, fu, 0.1, 2, -1, 0.0, [t0, lat.alloc(chi.kind, chi.prec)])):
+            with pytest.raises(lqx.LqxError):
+                bad()
+
+
+def test_jacobi_smear_config2_size(lqx):
+    """16^3x32 fp32 (the lattice of configs[1], a Table-1 size of the paper), 10 iterations, fermion."""
+    cfg = li.CONFIGS["c2"]
+    dims = cfg["dims"]
+    u = _links(cfg["seed"], dims, "f32")
+    chi0 = _gauss(cfg["seed"], 10, dims, "f", "f32")
+    with lqx.Lattice(dims) as lat:
+        fu = [lat.from_host(t) for t in u]
+        chi = lat.from_host(chi0)
+        tmp = [lat.alloc(chi.kind, chi.prec) for _ in range(2)]
+        lqx.jacobi_smear(chi, fu, 0.05, 10, 3, 1.5, tmp)
+        want = orc.jacobi_smear(dims, u, chi0, 0.05, 10, 3, 1.5, "t32")
+        assert site_rel_err(chi.pop(), want) < TOL["f32"] * 10
