@@ -523,12 +523,22 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="c4", choices=sorted(WORKLOADS))
     ap.add_argument("--no-extras", action="store_true", help="skip the per-kernel numbers of the other configs")
+    ap.add_argument("--extras-only", action="store_true",
+                    help="only the per-kernel numbers of configs 2, 3, 5 and the Jacobi routine (one JSON line with key "
+                         "'kernels'): the command ncu wraps for the catalogue / hop / Jacobi kernels")
     ap.add_argument("--kernel-only", action="store_true",
                     help="timed device region only (no e2e, no cpu_baseline, no extras): the command ncu wraps")
     ap.add_argument("--e2e-steps", type=int, default=5, help="cap on host-buffer steps timed for e2e")
     ap.add_argument("--ref-sites", type=int, default=400000, help="sites per step of the --impl reference sample")
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.extras_only:
+        import torch
+
+        import lattice_inputs as li
+        import paper_1105_2279_b200 as lqx
+
+        print(json.dumps({"kernels": _extras(torch, lqx, li, _peaks()[0])}))
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)
