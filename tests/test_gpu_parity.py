@@ -8,7 +8,7 @@ import pytest
 
 import lattice_inputs as li
 import oracle as orc
-from helpers import site_rel_err
+from helpers import cplx, site_rel_err
 
 pytestmark = pytest.mark.gpu
 
@@ -451,3 +451,141 @@ def test_jacobi_smear_config2_size(lqx):
         lqx.jacobi_smear(chi, fu, 0.05, 10, 3, 1.5, tmp)
         want = orc.jacobi_smear(dims, u, chi0, 0.05, 10, 3, 1.5, "t32")
         assert site_rel_err(chi.pop(), want) < TOL["f32"] * 10
+
+
+# ------------------------------------------------------------------------------------------------
+# BASELINE.json's full sizes, in the launch configuration bench.py times (default variant / tile):
+# sampled outputs the oracle computes one by one, plus properties that hold at any size
+# ------------------------------------------------------------------------------------------------
+def _full_size_links(lqx, lat, cfgname, recipe, prec):
+    """Same generator calls as bench.py: fields made on the GPU, imported, and copied to the host for the oracle."""
+    import torch
+
+    cfg = li.CONFIGS[cfgname]
+    fields, host = [], []
+    for mu in range(4):
+        if recipe == "haar":
+            z = li.haar_su3_complex(cfg["seed"], mu, lat.volume, "cuda")
+        else:
+            z = li.near_unit_su3_complex(cfg["seed"], mu, lat.volume, 0.1, "cuda")
+        a = li._as_real(z, prec)
+        del z
+        fields.append(lat.alloc(lqx.COLORMAT, _prec(lqx, prec)).import_dev(a))
+        torch.cuda.synchronize()
+        host.append(a.cpu().numpy())
+        del a
+    torch.cuda.empty_cache()
+    return fields, host
+
+
+def _sample_sites(dims, n, seed):
+    """Random sites plus the corners and faces where every kind of wrap-around happens."""
+    rng = np.random.default_rng(seed)
+    v = int(np.prod(dims))
+    s = list(rng.integers(0, v, size=n))
+    ext = [(0, d - 1, d // 2) for d in dims]
+    for x0 in ext[0]:
+        for x1 in ext[1]:
+            for x2 in ext[2]:
+                for x3 in ext[3]:
+                    s.append(x0 + dims[0] * (x1 + dims[1] * (x2 + dims[2] * x3)))
+    return np.unique(np.array(s, dtype=np.int64))
+
+
+@pytest.mark.parametrize("cfgname,recipe", [("c4", "near_unit"), ("c3", "haar")])
+def test_full_size_smear_step_sampled(lqx, cfgname, recipe):
+    import torch
+
+    cfg = li.CONFIGS[cfgname]
+    dims, prec = cfg["dims"], cfg["prec"]
+    tv = orc.truth_variant(prec)
+    with lqx.Lattice(dims) as lat:
+        fu, hu = _full_size_links(lqx, lat, cfgname, recipe, prec)
+        out = [lat.alloc(lqx.COLORMAT, fu[0].prec) for _ in range(4)]
+        p_fused = lqx.smear_step(out, fu, 0.5, want_plaq_in=True)
+        sites = _sample_sites(dims, 3000, 17)
+        dt = torch.float32 if prec == "f32" else torch.float64
+        buf = torch.empty((lat.volume, 3, 3, 2), dtype=dt, device="cuda")
+        idx = torch.from_numpy(sites).cuda()
+        for mu in range(4):
+            out[mu].export_dev(buf)
+            got = buf[idx].cpu().numpy()
+            want = orc.smear_links(dims, hu, 0.5, sites, np.full(sites.size, mu, dtype=np.int32), tv)
+            assert site_rel_err(got, want) < TOL[prec], mu
+        # plaquette: the fused sum equals the standalone kernel's (two code paths), and the per-site mean over
+        # the sample agrees with the oracle's integrand within its statistical error
+        p_alone, _ = lqx.plaquette(fu)
+        scale = np.sqrt(18.0 * lat.volume)
+        assert abs(p_fused - p_alone) / max(abs(p_alone), scale) < RTOL[prec]
+        dens = orc.plaquette_sites(dims, hu, sites, tv)
+        assert abs(p_alone / lat.volume - dens.mean()) < 6 * dens.std() / np.sqrt(sites.size) + 1e-6
+        # property at any size: sum_{x,mu} Re tr[U S^dag] = 4 P, with S recovered from U' = (1-a) U + (a/6) S
+        acc = 0.0
+        for mu in range(4):
+            out[mu].export_dev(buf)
+            uin = torch.from_numpy(hu[mu]).cuda().to(torch.float64)
+            stp = (buf.to(torch.float64) - 0.5 * uin) * 12.0
+            acc += float((uin * stp).sum())
+            del uin, stp
+        assert abs(acc - 4.0 * p_alone) / max(abs(4.0 * p_alone), scale) < RTOL[prec] * 4
+
+
+def test_full_size_c4_ten_steps_properties(lqx):
+    """configs[3]: ten iterated steps with the plaquette after each; the first step's plaquette equals the
+    plaquette of a single smear_step output, and the trajectory is reproducible bit for bit."""
+    cfg = li.CONFIGS["c4"]
+    dims = cfg["dims"]
+    with lqx.Lattice(dims) as lat:
+        fu, _ = _full_size_links(lqx, lat, "c4", "near_unit", "f32")
+        tmp = [lat.alloc(lqx.COLORMAT, lqx.F32) for _ in range(4)]
+        keep = [lat.alloc(lqx.COLORMAT, lqx.F32) for _ in range(4)]
+        for a, b in zip(keep, fu):
+            lqx.copy(a, b)
+        lqx.smear_step(tmp, fu, 0.5)
+        _, p1 = lqx.plaquette(tmp)
+        plaqs = lqx.smear_iterate(fu, tmp, 0.5, 10)
+        assert len(plaqs) == 10 and all(np.isfinite(plaqs))
+        assert abs(plaqs[0] - p1) < RTOL["f32"]
+        assert all(0.0 < p < 1.0 for p in plaqs)
+        n_a = lqx.norm2(fu[2])
+        plaqs2 = lqx.smear_iterate(keep, tmp, 0.5, 10)
+        assert plaqs2 == plaqs and lqx.norm2(keep[2]) == n_a
+
+
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+def test_full_size_c5_expression_sweep(lqx, prec):
+    """configs[4]: 32^3x64, the four forms each followed by its reduction, against the truth oracle."""
+    dims = li.CONFIGS["c5"]["dims"]
+    tv = orc.truth_variant(prec)
+    a, b, c, d = (_gauss(7, k, dims, "cm", prec) for k in range(4))
+    v = _gauss(7, 4, dims, "cv", prec)
+    with lqx.Lattice(dims) as lat:
+        fa, fb, fc, fd, fv = (lat.from_host(t) for t in (a, b, c, d, v))
+        r = lat.alloc(lqx.COLORMAT, fa.prec)
+        cx = lat.alloc(lqx.COMPLEX, fa.prec)
+        w = lat.alloc(lqx.COLORVEC, fa.prec)
+        lqx.mm_plus_madj(r, fa, fb, fc, fd)
+        want = orc.mm_plus_madj(dims, a, b, c, d, tv)
+        assert site_rel_err(r.pop(), want) < TOL[prec]
+        n2 = lqx.norm2(r)
+        wn2 = orc.norm2(dims, want.astype(np.float64), "t64")
+        assert abs(n2 - wn2) / wn2 < RTOL[prec]
+        lqx.trace_mm(cx, fa, fb)
+        want = orc.trace_mm(dims, a, b, tv)
+        # form ii reduces nine products to ONE complex number per site: among 2 million sites some cancel
+        # almost completely, so the error is measured against the size of what was summed,
+        # sum_ik |A_ik| |B_ki| (reading A14 with the summands as the site object)
+        mag = np.einsum("xik,xki->x", np.abs(cplx(a)), np.abs(cplx(b)))
+        assert float((np.abs(cx.pop().astype(np.float64) - want).max(axis=1) / mag).max()) < TOL[prec]
+        rms = float(np.sqrt((want.astype(np.float64) ** 2).sum()))
+        assert _red_err(lqx.sum(cx), orc.sum_field(dims, want.astype(np.float64), "t64"), rms) < RTOL[prec]
+        lqx.ax_minus_shift(r, 2.5, fa, fb, lqx.BACKWARD, 2)
+        assert np.array_equal(r.pop(), orc.ax_minus_shift(dims, 2.5, a, b, -1, 2, orc.native_variant(prec)))
+        want = orc.ax_minus_shift(dims, 2.5, a, b, -1, 2, tv).astype(np.float64)
+        rms = float(np.sqrt((want ** 2).sum()))
+        assert _red_err(lqx.trace(r), orc.trace(dims, want, "t64"), rms) < RTOL[prec]
+        lqx.mat_vec(w, fa, fv)
+        want = orc.mat_vec(dims, a, v, tv)
+        assert site_rel_err(w.pop(), want) < TOL[prec]
+        wn2 = float((want.astype(np.float64) ** 2).sum())
+        assert abs(lqx.norm2(w) - wn2) / wn2 < RTOL[prec]
