@@ -151,6 +151,41 @@ int lqx_jacobi_smear(lqx_field* chi, const lqx_field* const u[4], double kappa, 
                      int no_smear_dir, double norm, lqx_field* const tmp[2]);
 
 /* ---------------------------------------------------------------------------------------------
+ * Run-time expression fusion -- the paper's own mechanism:
+ * the expression arrives as a flattened POD tree in postfix order ("a linear
+ * container"), the library generates ONE fused kernel for it, compiles it with NVRTC for sm_100a
+ * on first use and keeps it loaded until lqx_finalize, so that every expression is compiled once
+ * per process.  Scalars are kernel arguments: expressions that differ only in their
+ * scalars share a kernel.
+ *   LEAF  a = index into leaves[]           pushes that field
+ *   ADJ                                     adj(top)                    colour matrix
+ *   MUL                                     left * right                matrix*matrix, matrix*vector, matrix*fermion
+ *   ADD / SUB                               left + right, left - right  same kind
+ *   SCALE s = real scalar                   s * top                     any kind
+ *   SHIFT a = LQX_FORWARD/LQX_BACKWARD, b = mu   shift(top, a, b): the operand evaluated at x + a*mu^
+ * (shifts nest: shift(adj(u)*psi, BACKWARD, mu) is the Listing's form).
+ * dst = expr (accumulate == 0) or dst += expr (accumulate != 0, E2 of the Listing).  dst may alias
+ * a leaf that is not read through a shift; otherwise LQX_EALIAS.  At most 16 leaves and 16 scalars.
+ * Errors: LQX_EINVAL malformed sequence, LQX_ETYPE kind mismatch, LQX_ECUDA compilation / load
+ * failure (lqx_last_error holds the NVRTC log).  Asynchronous on the context's stream.
+ * ------------------------------------------------------------------------------------------- */
+typedef enum { LQX_X_LEAF = 0, LQX_X_ADJ = 1, LQX_X_MUL = 2, LQX_X_ADD = 3, LQX_X_SUB = 4, LQX_X_SCALE = 5,
+               LQX_X_SHIFT = 6 } lqx_xop;
+typedef struct {
+    int32_t op; /* lqx_xop */
+    int32_t a, b;
+    double s;
+} lqx_xnode;
+int lqx_expr_eval(lqx_field* dst, int accumulate, const lqx_xnode* nodes, int nnodes,
+                  const lqx_field* const* leaves, int nleaves);
+/* The CUDA source the library generates for an expression (for inspection and tests; needs no GPU:
+ * ctx may be NULL): written NUL-terminated into buf; returns its full length or a negative status. */
+int lqx_expr_source(lqx_ctx* ctx, lqx_kind dst_kind, lqx_prec prec, int accumulate, const lqx_xnode* nodes,
+                    int nnodes, const lqx_kind* leaf_kinds, int nleaves, char* buf, size_t buflen);
+/* Number of distinct expression kernels this context has compiled so far. */
+int lqx_expr_cache_size(const lqx_ctx* ctx);
+
+/* ---------------------------------------------------------------------------------------------
  * Global reductions.  fp64 accumulation for both precisions, fixed summation
  * tree (deterministic run to run).  Results to host double; these calls synchronise.
  * ------------------------------------------------------------------------------------------- */

@@ -187,6 +187,51 @@ def jacobi_smear(dims, u, chi, kappa, iters, no_smear_dir, norm, variant):
     return out
 
 
+# ---------------------------------------------------------------- generic expressions (NEXT-2)
+X_LEAF, X_ADJ, X_MUL, X_ADD, X_SUB, X_SCALE, X_SHIFT = range(7)
+
+
+def eval_expr(dims, nodes, leaves):
+    """Plain per-site evaluation of a QDP++-style expression given in postfix order (the whole
+    expression per site; :101: shift reads its operand at the periodic neighbour; Listing 1 operators * + -
+    adj shift, PAPER.md:154-182).  nodes: sequence of (op, a, b, s) with the operator codes above;
+    leaves: QDP-order real arrays [V, ..., 2].  Arithmetic in complex128 (the truth for both precisions);
+    returns a QDP-order float64 array.  A shift of a sub-expression is the sub-expression's field gathered
+    through the oracle's neighbour table: shift(e, sign, mu)(x) = e(x + sign*mu^)."""
+    stack = []
+    for (op, a, b, s) in nodes:
+        if op == X_LEAF:
+            f = np.asarray(leaves[a], dtype=np.float64)
+            stack.append(f[..., 0] + 1j * f[..., 1])
+        elif op == X_ADJ:
+            m = stack.pop()
+            stack.append(np.conj(np.swapaxes(m, -1, -2)))
+        elif op == X_MUL:
+            r, l = stack.pop(), stack.pop()
+            if r.ndim == 3 and r.shape[1:] == (3, 3):
+                stack.append(np.einsum("xik,xkj->xij", l, r))
+            elif r.ndim == 2:
+                stack.append(np.einsum("xij,xj->xi", l, r))
+            else:
+                stack.append(np.einsum("xij,xaj->xai", l, r))
+        elif op == X_ADD:
+            r, l = stack.pop(), stack.pop()
+            stack.append(l + r)
+        elif op == X_SUB:
+            r, l = stack.pop(), stack.pop()
+            stack.append(l - r)
+        elif op == X_SCALE:
+            stack.append(float(s) * stack.pop())
+        elif op == X_SHIFT:
+            stack.append(stack.pop()[neighbor_table(dims, int(a), int(b))])
+        else:
+            raise ValueError(f"unknown operator {op}")
+    if len(stack) != 1:
+        raise ValueError("the postfix sequence does not reduce to one value")
+    z = stack[0]
+    return np.ascontiguousarray(np.stack((z.real, z.imag), axis=-1))
+
+
 # ---------------------------------------------------------------- reductions
 def sum_field(dims, f, variant):
     f = _inp(f, variant)

@@ -77,6 +77,9 @@ SIGNATURES = {
     "lqx_hop": (_i, [_vp, _pvp, _vp]),
     "lqx_hop_norm2": (_i, [_vp, _pvp, _vp, _pd]),
     "lqx_jacobi_smear": (_i, [_vp, _pvp, _d, _i, _i, _d, _pvp]),
+    "lqx_expr_eval": (_i, [_vp, _i, _vp, _i, _pvp, _i]),
+    "lqx_expr_source": (_i, [_vp, _i, _i, _i, _vp, _i, C.POINTER(C.c_int), _i, C.c_char_p, C.c_size_t]),
+    "lqx_expr_cache_size": (_i, [_vp]),
     "lqx_axpy": (_i, [_vp, _vp, _d, _vp]),
     "lqx_scale": (_i, [_vp, _d, _vp]),
     "lqx_divide": (_i, [_vp, _vp, _d]),
@@ -220,6 +223,9 @@ class Lattice:
         _check(_lib.lqx_kernel_time(self.ctx, kernel_class, C.byref(ms), C.byref(n)), self.ctx)
         return ms.value, n.value
 
+    def expr_cache_size(self) -> int:
+        return int(_lib.lqx_expr_cache_size(self.ctx))
+
     def launch_count(self) -> int:
         return int(_lib.lqx_launch_count(self.ctx))
 
@@ -319,6 +325,99 @@ def jacobi_smear(chi, u, kappa, iters, no_smear_dir, norm, tmp):
     """chi <- sum_{n<=iters} kappa^n H^n chi / norm (Listing 1 of the paper); tmp = two scratch fields."""
     arr = (C.c_void_p * 2)(_h(tmp[0]), _h(tmp[1]))
     _check(_lib.lqx_jacobi_smear(_h(chi), _arr4(u), float(kappa), int(iters), int(no_smear_dir), float(norm), arr), _ctx_of(chi))
+
+
+# ---- run-time expression fusion: a tiny builder for the flattened postfix tree of lqx_expr_eval
+X_LEAF, X_ADJ, X_MUL, X_ADD, X_SUB, X_SCALE, X_SHIFT = range(7)
+
+
+class _XNode(C.Structure):
+    _fields_ = [("op", C.c_int32), ("a", C.c_int32), ("b", C.c_int32), ("s", C.c_double)]
+
+
+class Expr:
+    """Expression over fields with the paper's operators: `*`, `+`, `-`, real `scalar * e`, adj(e),
+    shift(e, direction, mu).  Leaves are Field objects (or, for expr_source, bare kind codes)."""
+
+    def __init__(self, nodes, leaves):
+        self.nodes, self.leaves = nodes, leaves  # nodes: list of (op, a, b, s); leaves: list of fields
+
+    @staticmethod
+    def leaf(field):
+        return Expr([(X_LEAF, 0, 0, 0.0)], [field])
+
+    def _merge(self, other):
+        """Postfix of other re-indexed onto this expression's leaf list (identical fields share a slot)."""
+        leaves = list(self.leaves)
+        remap = {}
+        for i, f in enumerate(other.leaves):
+            for j, g in enumerate(leaves):
+                if g is f:
+                    remap[i] = j
+                    break
+            else:
+                remap[i] = len(leaves)
+                leaves.append(f)
+        nodes = [(op, remap[a] if op == X_LEAF else a, b, s) for (op, a, b, s) in other.nodes]
+        return nodes, leaves
+
+    def _binary(self, other, op):
+        if not isinstance(other, Expr):
+            other = Expr.leaf(other)
+        nodes, leaves = self._merge(other)
+        return Expr(self.nodes + nodes + [(op, 0, 0, 0.0)], leaves)
+
+    def __mul__(self, other):
+        if isinstance(other, (int, float)):
+            return Expr(self.nodes + [(X_SCALE, 0, 0, float(other))], self.leaves)
+        return self._binary(other, X_MUL)
+
+    def __rmul__(self, other):
+        return Expr(self.nodes + [(X_SCALE, 0, 0, float(other))], self.leaves)
+
+    def __add__(self, other):
+        return self._binary(other, X_ADD)
+
+    def __sub__(self, other):
+        return self._binary(other, X_SUB)
+
+    def adj(self):
+        return Expr(self.nodes + [(X_ADJ, 0, 0, 0.0)], self.leaves)
+
+    def shift(self, direction, mu):
+        return Expr(self.nodes + [(X_SHIFT, int(direction), int(mu), 0.0)], self.leaves)
+
+    def _c_nodes(self):
+        arr = (_XNode * len(self.nodes))()
+        for i, (op, a, b, s) in enumerate(self.nodes):
+            arr[i].op, arr[i].a, arr[i].b, arr[i].s = op, a, b, s
+        return arr
+
+
+def adj(e):
+    return (e if isinstance(e, Expr) else Expr.leaf(e)).adj()
+
+
+def shifted(e, direction, mu):
+    return (e if isinstance(e, Expr) else Expr.leaf(e)).shift(direction, mu)
+
+
+def expr_eval(dst, expr, accumulate=False):
+    """dst = expr (or dst += expr): one fused kernel, NVRTC-compiled on first use and cached."""
+    leaves = (C.c_void_p * max(1, len(expr.leaves)))(*[_h(f) for f in expr.leaves])
+    _check(_lib.lqx_expr_eval(_h(dst), 1 if accumulate else 0, expr._c_nodes(), len(expr.nodes), leaves, len(expr.leaves)),
+           _ctx_of(dst))
+
+
+def expr_source(lat, dst_kind, prec, expr, accumulate=False) -> str:
+    """The CUDA source generated for expr; leaves may be Field objects or kind codes."""
+    kinds = (C.c_int * max(1, len(expr.leaves)))(*[f.kind if isinstance(f, Field) else int(f) for f in expr.leaves])
+    buf = C.create_string_buffer(1 << 16)
+    n = _lib.lqx_expr_source(lat.ctx if isinstance(lat, Lattice) else lat, dst_kind, prec, 1 if accumulate else 0, expr._c_nodes(),
+                             len(expr.nodes), kinds, len(expr.leaves), buf, len(buf))
+    if n < 0:
+        raise LqxError(n, _lib.lqx_last_error(lat.ctx if isinstance(lat, Lattice) else lat).decode())
+    return buf.value.decode()
 
 
 def axpy(r, s0, kappa, h):

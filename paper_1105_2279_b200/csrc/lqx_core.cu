@@ -115,6 +115,7 @@ extern "C" int lqx_finalize(lqx_ctx* ctx) {
     if (!ctx) return LQX_EINVAL;
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
+    lqx_jit_release(ctx);
     for (lqx_field* f : ctx->fields) {
         if (f->owned && f->data) cudaFree(f->data);
         delete f;

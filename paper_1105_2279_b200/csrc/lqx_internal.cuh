@@ -79,6 +79,7 @@ struct lqx_field {
 };
 
 int lqx_fail(lqx_ctx* ctx, int code, const char* what);
+void lqx_jit_release(lqx_ctx* ctx);  // unloads the context's run-time compiled expression kernels (lqx_jit.cu)
 int lqx_cuda_fail(lqx_ctx* ctx, cudaError_t e, const char* where);
 int lqx_ensure_partials(lqx_ctx* ctx, size_t ndoubles);
 // synchronises the stream and copies ctx->h_result[0..n) (written by a reduction kernel) to `out`

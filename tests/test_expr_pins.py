@@ -1,0 +1,135 @@
+"""Pins of the oracle's generic expression evaluator (NEXT-2) and, without a GPU, of the code generator:
+the evaluator must reduce to the already pinned oracle routines on the expressions they implement
+(form i, form iii, the paper's hop written exactly as Listing 1 lines 25/27, the staple sum written with
+nested shifts), and the CUDA source generated for those expressions must compile for sm_100a."""
+import os
+import shutil
+import subprocess
+
+import numpy as np
+import pytest
+
+import lattice_inputs as li
+import oracle as orc
+from helpers import site_rel_err
+
+L, ADJ, MUL, ADD, SUB, SCALE, SHIFT = range(7)
+
+
+def links(seed, dims, prec="f64"):
+    return [t.numpy() for t in li.gauge_field(seed, dims, prec, "haar")]
+
+
+def gauss(seed, fid, dims, kind, prec="f64"):
+    return li.gaussian_field(seed, fid, dims, kind, prec).numpy()
+
+
+def hop_nodes():
+    """sum_mu u[mu]*shift(psi,FORWARD,mu) + shift(adj(u[mu])*psi,BACKWARD,mu); leaves u0..u3 = 0..3, psi = 4"""
+    n = []
+    for mu in range(4):
+        n += [(L, mu, 0, 0), (L, 4, 0, 0), (SHIFT, +1, mu, 0), (MUL, 0, 0, 0)]
+        n += [(L, mu, 0, 0), (ADJ, 0, 0, 0), (L, 4, 0, 0), (MUL, 0, 0, 0), (SHIFT, -1, mu, 0), (ADD, 0, 0, 0)]
+        if mu:
+            n += [(ADD, 0, 0, 0)]
+    return n
+
+
+def staple_nodes(mu):
+    """sum_{nu != mu} u[nu]*shift(u[mu],F,nu)*adj(shift(u[nu],F,mu)) + shift(adj(u[nu])*u[mu]*shift(u[nu],F,mu), B, nu)"""
+    n, first = [], True
+    for nu in range(4):
+        if nu == mu:
+            continue
+        n += [(L, nu, 0, 0), (L, mu, 0, 0), (SHIFT, +1, nu, 0), (MUL, 0, 0, 0), (L, nu, 0, 0), (SHIFT, +1, mu, 0), (ADJ, 0, 0, 0),
+              (MUL, 0, 0, 0)]
+        n += [(L, nu, 0, 0), (ADJ, 0, 0, 0), (L, mu, 0, 0), (MUL, 0, 0, 0), (L, nu, 0, 0), (SHIFT, +1, mu, 0), (MUL, 0, 0, 0),
+              (SHIFT, -1, nu, 0), (ADD, 0, 0, 0)]
+        if not first:
+            n += [(ADD, 0, 0, 0)]
+        first = False
+    return n
+
+
+FORM_I = [(L, 0, 0, 0), (L, 1, 0, 0), (MUL, 0, 0, 0), (L, 2, 0, 0), (L, 3, 0, 0), (ADJ, 0, 0, 0), (MUL, 0, 0, 0), (ADD, 0, 0, 0)]
+FORM_III = [(L, 0, 0, 0), (SCALE, 0, 0, 2.5), (L, 1, 0, 0), (SHIFT, -1, 2, 0), (SUB, 0, 0, 0)]
+
+
+@pytest.mark.parametrize("dims", [(4, 6, 2, 4), (3, 5, 2, 4)])
+def test_evaluator_reduces_to_the_pinned_routines(dims):
+    a, b, c, d = (gauss(7, k, dims, "cm") for k in range(4))
+    assert site_rel_err(orc.eval_expr(dims, FORM_I, [a, b, c, d]), orc.mm_plus_madj(dims, a, b, c, d, "t64")) < 1e-14
+    assert site_rel_err(orc.eval_expr(dims, FORM_III, [a, b]), orc.ax_minus_shift(dims, 2.5, a, b, -1, 2, "t64")) < 1e-15
+    u = links(2, dims)
+    for kind in ("f", "cv"):
+        psi = gauss(2, 10, dims, kind)
+        assert site_rel_err(orc.eval_expr(dims, hop_nodes(), u + [psi]), orc.hop(dims, u, psi, "t64")) < 1e-14
+    for mu in range(4):
+        assert site_rel_err(orc.eval_expr(dims, staple_nodes(mu), u), orc.staple_sum(dims, u, mu, "t64")) < 1e-14
+
+
+def test_evaluator_rejects_malformed_sequences():
+    a = gauss(1, 0, (2, 2, 2, 2), "cm")
+    with pytest.raises(ValueError):
+        orc.eval_expr((2, 2, 2, 2), [(L, 0, 0, 0), (L, 0, 0, 0)], [a])
+    with pytest.raises(ValueError):
+        orc.eval_expr((2, 2, 2, 2), [(L, 0, 0, 0), (99, 0, 0, 0)], [a])
+
+
+# ------------------------------------------------------------------ the code generator, without a GPU
+def _source(nodes, leaf_kinds, dst_kind, prec, accumulate=False):
+    import paper_1105_2279_b200 as lqx
+
+    e = lqx.Expr(list(nodes), list(leaf_kinds))
+    return lqx.expr_source(None, dst_kind, prec, e, accumulate)
+
+
+def test_generated_source_is_one_fused_kernel():
+    import paper_1105_2279_b200 as lqx
+
+    src = _source(hop_nodes(), [lqx.COLORMAT] * 4 + [lqx.FERMION], lqx.FERMION, lqx.F32)
+    assert src.count("__global__") == 1 and src.count("jstore<12>") == 1
+    assert src.count("jnbr(g, s0, 1, ") == 4 and src.count(", -1, ") == 4  # eight neighbour sites, computed
+    assert src.count("jload<9>") == 8 and src.count("jload<12>") == 8
+    # scalars are arguments, not text: 2.5*A - shift(B) and 7*A - shift(B) generate the same source
+    s1 = _source(FORM_III, [lqx.COLORMAT] * 2, lqx.COLORMAT, lqx.F64)
+    s2 = _source([(L, 0, 0, 0), (SCALE, 0, 0, 7.0), (L, 1, 0, 0), (SHIFT, -1, 2, 0), (SUB, 0, 0, 0)], [lqx.COLORMAT] * 2,
+                 lqx.COLORMAT, lqx.F64)
+    assert s1 == s2 and "2.5" not in s1
+    # accumulate ('+=', E2 of the Listing) reads the destination
+    assert "jload<12>(dst, s0)" in _source(hop_nodes(), [lqx.COLORMAT] * 4 + [lqx.FERMION], lqx.FERMION, lqx.F32, True)
+
+
+def test_generator_type_and_shape_errors():
+    import paper_1105_2279_b200 as lqx
+
+    with pytest.raises(lqx.LqxError):  # vector * matrix
+        _source([(L, 0, 0, 0), (L, 1, 0, 0), (MUL, 0, 0, 0)], [lqx.COLORVEC, lqx.COLORMAT], lqx.COLORVEC, lqx.F32)
+    with pytest.raises(lqx.LqxError):  # adj of a vector
+        _source([(L, 0, 0, 0), (ADJ, 0, 0, 0)], [lqx.COLORVEC], lqx.COLORVEC, lqx.F32)
+    with pytest.raises(lqx.LqxError):  # matrix + vector
+        _source([(L, 0, 0, 0), (L, 1, 0, 0), (ADD, 0, 0, 0)], [lqx.COLORMAT, lqx.COLORVEC], lqx.COLORMAT, lqx.F32)
+    with pytest.raises(lqx.LqxError):  # destination kind
+        _source(FORM_I, [lqx.COLORMAT] * 4, lqx.COLORVEC, lqx.F32)
+    with pytest.raises(lqx.LqxError):  # does not reduce to one value
+        _source([(L, 0, 0, 0), (L, 0, 0, 0)], [lqx.COLORMAT], lqx.COLORMAT, lqx.F32)
+    with pytest.raises(lqx.LqxError):  # shift direction
+        _source([(L, 0, 0, 0), (SHIFT, 2, 0, 0)], [lqx.COLORMAT], lqx.COLORMAT, lqx.F32)
+
+
+@pytest.mark.skipif(shutil.which("nvcc") is None and not os.path.exists("/usr/local/cuda/bin/nvcc"), reason="no nvcc")
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+def test_generated_source_compiles_for_sm_100a(tmp_path, prec):
+    import paper_1105_2279_b200 as lqx
+
+    pc = lqx.F32 if prec == "f32" else lqx.F64
+    nvcc = shutil.which("nvcc") or "/usr/local/cuda/bin/nvcc"
+    cases = {"hop": (hop_nodes(), [lqx.COLORMAT] * 4 + [lqx.FERMION], lqx.FERMION),
+             "staple": (staple_nodes(1), [lqx.COLORMAT] * 4, lqx.COLORMAT),
+             "form_iii": (FORM_III, [lqx.COLORMAT] * 2, lqx.COLORMAT)}
+    for name, (nodes, kinds, dk) in cases.items():
+        f = tmp_path / f"{name}_{prec}.cu"
+        f.write_text(_source(nodes, kinds, dk, pc))
+        r = subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-std=c++17", "-cubin", "-o", str(f) + ".cubin", str(f)],
+                           capture_output=True, text=True)
+        assert r.returncode == 0, r.stderr[-3000:]
