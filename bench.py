@@ -282,6 +282,12 @@ def _extras(torch, lqx, li, hbm_gbs):
             psi = lat.alloc(lqx.FERMION, pcode).import_dev(li.gaussian_field(2, 10, dims, "f", prec, device="cuda"))
             chi = lat.alloc(lqx.FERMION, pcode)
             add("hop 32^3x64 (not a BASELINE config; size check)", prec, lat.volume, 120, 2280, lambda: lqx.hop(chi, u, psi), reps=10)
+            eh = None
+            for mu in range(4):  # the Listing's E1/E2 expression, summed over mu, as ONE run-time expression
+                t = lqx.Expr.leaf(u[mu]) * lqx.shifted(psi, lqx.FORWARD, mu) + lqx.shifted(lqx.adj(u[mu]) * lqx.Expr.leaf(psi), lqx.BACKWARD, mu)
+                eh = t if eh is None else eh + t
+            lqx.expr_eval(chi, eh)
+            add("hop 32^3x64 as a run-time expression (NVRTC)", prec, lat.volume, 120, 2280, lambda: lqx.expr_eval(chi, eh), reps=10)
     # ---- NEXT-1: the paper's complete Jacobi smearing routine at its Table 1 sizes 16^3x32 and 32^3x64
     # (PAPER.md:228-238), fermion field, 20 iterations, all four directions.  Per iteration and site the fused
     # kernel moves U 72 + psi 24 + s_0 24 + chi 24 = 144 reals and does 2280 (hop) + 48 (E3) canonical flops.
@@ -326,6 +332,16 @@ def _extras(torch, lqx, li, hbm_gbs):
             add("form iii 2.5*A-shift(B,BACKWARD,2) c5", prec, v, 54, 36, lambda: lqx.ax_minus_shift(r, 2.5, cm[0], cm[1], lqx.BACKWARD, 2))
             add("form iii' 2.5*A-shift(B,FORWARD,0) c5", prec, v, 54, 36, lambda: lqx.ax_minus_shift(r, 2.5, cm[0], cm[1], lqx.FORWARD, 0))
             add("form iv M*v c5", prec, v, 30, 66, lambda: lqx.mat_vec(w, cm[0], vec))
+            # NEXT-2: the same forms as run-time expressions (one NVRTC-compiled fused kernel each, cached)
+            e1 = lqx.Expr.leaf(cm[0]) * lqx.Expr.leaf(cm[1]) + lqx.Expr.leaf(cm[2]) * lqx.adj(cm[3])
+            t0 = time.perf_counter()
+            lqx.expr_eval(r, e1)
+            torch.cuda.synchronize()
+            jit_s = time.perf_counter() - t0
+            add("form i  as a run-time expression (NVRTC) c5", prec, v, 90, 414, lambda: lqx.expr_eval(r, e1))
+            out[-1]["first_use_compile_s"] = round(jit_s, 3)
+            e3 = 2.5 * lqx.Expr.leaf(cm[0]) - lqx.shifted(cm[1], lqx.BACKWARD, 2)
+            add("form iii as a run-time expression (NVRTC) c5", prec, v, 54, 36, lambda: lqx.expr_eval(r, e3))
             add("shift(A,FORWARD,3) c5", prec, v, 36, 0, lambda: lqx.shift(r, cm[0], lqx.FORWARD, 3))
             add("norm2(colour matrix) c5 (incl. sync)", prec, v, 18, 36, lambda: lqx.norm2(cm[0]), lat=lat, kclass=lqx.K_REDUCE)
             add("sum(colour matrix) c5 (incl. sync)", prec, v, 18, 18, lambda: lqx.sum(cm[0]), lat=lat, kclass=lqx.K_REDUCE)

@@ -57,11 +57,6 @@ Nvrtc g_nvrtc;
 // --------------------------------------------------------------------------------------------
 const char* kPrelude = R"SRC(
 struct JGeo { int L[4]; int st[4]; int V; };
-__device__ __forceinline__ int jnbr(const JGeo& g, int s, int dir, int mu) {
-    const int x = (s / g.st[mu]) % g.L[mu];
-    if (dir > 0) return x + 1 == g.L[mu] ? s - (g.L[mu] - 1) * g.st[mu] : s + g.st[mu];
-    return x == 0 ? s + (g.L[mu] - 1) * g.st[mu] : s - g.st[mu];
-}
 template <int N> struct Obj { T re[N], im[N]; };   // N complex numbers in QDP order
 template <int N>
 __device__ __forceinline__ Obj<N> jload(const T* __restrict__ base, int s) {
@@ -202,19 +197,34 @@ struct JitCache {
 };
 std::map<lqx_ctx*, JitCache> g_caches;  // per context; emptied by lqx_jit_release (called from lqx_finalize)
 
-// recursive code generation: emits statements into `os`, returns the name of the value's variable
+// recursive code generation: emits statements into `os`, returns the name of the value's variable.
+// A site is a variable holding its index plus the names of its four coordinates, so that a shift is a
+// compare-and-select on ONE coordinate (no division), however deeply shifts nest.
+struct Site {
+    std::string s, x[4];
+};
 struct Gen {
     const std::vector<XNode>& n;
     std::ostringstream os;
     int tmp = 0, sites = 0;
     explicit Gen(const std::vector<XNode>& nodes) : n(nodes) {}
-    std::string val(int i, const std::string& site) {
+    std::string val(int i, const Site& site) {
         const XNode& x = n[i];
-        std::string v = "v" + std::to_string(tmp++);
         const std::string ty = "Obj<" + std::to_string(x.kind) + ">";
+        if (x.op == LQX_X_SHIFT) {  // shift(expr, dir, mu)(x) = expr(x + dir*mu^): evaluate the operand at the neighbour
+            const std::string k = std::to_string(++sites), mu = std::to_string(x.b);
+            Site s2 = site;
+            s2.s = "s" + k;
+            s2.x[x.b] = "x" + k;
+            if (x.a > 0) os << "    const int x" << k << " = " << site.x[x.b] << " + 1 == g.L[" << mu << "] ? 0 : " << site.x[x.b] << " + 1;\n";
+            else os << "    const int x" << k << " = " << site.x[x.b] << " == 0 ? g.L[" << mu << "] - 1 : " << site.x[x.b] << " - 1;\n";
+            os << "    const int s" << k << " = " << site.s << " + (x" << k << " - " << site.x[x.b] << ") * g.st[" << mu << "];\n";
+            return val(x.child[0], s2);
+        }
+        std::string v = "v" + std::to_string(tmp++);
         switch (x.op) {
             case LQX_X_LEAF:
-                os << "    const " << ty << " " << v << " = jload<" << x.kind << ">(p" << x.a << ", " << site << ");\n";
+                os << "    const " << ty << " " << v << " = jload<" << x.kind << ">(p" << x.a << ", " << site.s << ");\n";
                 break;
             case LQX_X_ADJ: {
                 std::string c = val(x.child[0], site);
@@ -237,11 +247,6 @@ struct Gen {
                 std::string c = val(x.child[0], site);
                 os << "    const " << ty << " " << v << " = jscale(k" << x.scalar_slot << ", " << c << ");\n";
                 break;
-            }
-            case LQX_X_SHIFT: {  // shift(expr, dir, mu)(x) = expr(x + dir*mu^): evaluate the operand at the neighbour
-                std::string s2 = "s" + std::to_string(++sites);
-                os << "    const int " << s2 << " = jnbr(g, " << site << ", " << x.a << ", " << x.b << ");\n";
-                return val(x.child[0], s2);
             }
         }
         return v;
@@ -331,12 +336,18 @@ std::string make_source(const std::vector<XNode>& tree, int nleaves, int nscalar
     if (f32) src << "typedef float T;\ntypedef float4 VEC;\nconstexpr int W = 4;\n";
     else src << "typedef double T;\ntypedef double2 VEC;\nconstexpr int W = 2;\n";
     src << kPrelude;
-    src << "extern \"C\" __global__ void __launch_bounds__(128) lqx_jit(const JGeo g";
+    // register budget: 128 per thread in fp32 (four CTAs per SM), 255 in fp64 (measured on the hop expression)
+    src << "extern \"C\" __global__ void __launch_bounds__(128, " << (f32 ? 4 : 2) << ") lqx_jit(const JGeo g";
     for (int k = 0; k < nscalars; ++k) src << ", const T k" << k;
     for (int l = 0; l < nleaves; ++l) src << ", const T* __restrict__ p" << l;
     src << ", T* dst) {\n    const int s0 = blockIdx.x * blockDim.x + threadIdx.x;\n    if (s0 >= g.V) return;\n";
+    src << "    const int x0_0 = s0 % g.L[0], q1 = s0 / g.L[0];\n    const int x0_1 = q1 % g.L[1], q2 = q1 / g.L[1];\n"
+           "    const int x0_2 = q2 % g.L[2], x0_3 = q2 / g.L[2];\n";
     Gen gen(tree);
-    const std::string r = gen.val((int)tree.size() - 1, "s0");
+    Site origin;
+    origin.s = "s0";
+    for (int d = 0; d < 4; ++d) origin.x[d] = "x0_" + std::to_string(d);
+    const std::string r = gen.val((int)tree.size() - 1, origin);
     src << gen.os.str();
     if (accumulate) src << "    jstore<" << dst_kind << ">(dst, s0, jadd(jload<" << dst_kind << ">(dst, s0), " << r << "));\n";
     else src << "    jstore<" << dst_kind << ">(dst, s0, " << r << ");\n";

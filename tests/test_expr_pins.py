@@ -89,7 +89,7 @@ def test_generated_source_is_one_fused_kernel():
 
     src = _source(hop_nodes(), [lqx.COLORMAT] * 4 + [lqx.FERMION], lqx.FERMION, lqx.F32)
     assert src.count("__global__") == 1 and src.count("jstore<12>") == 1
-    assert src.count("jnbr(g, s0, 1, ") == 4 and src.count(", -1, ") == 4  # eight neighbour sites, computed
+    assert src.count("const int s") == 1 + 8 and "/ g.st" not in src  # eight neighbour sites, one select each, no division
     assert src.count("jload<9>") == 8 and src.count("jload<12>") == 8
     # scalars are arguments, not text: 2.5*A - shift(B) and 7*A - shift(B) generate the same source
     s1 = _source(FORM_III, [lqx.COLORMAT] * 2, lqx.COLORMAT, lqx.F64)

@@ -589,3 +589,83 @@ def test_full_size_c5_expression_sweep(lqx, prec):
         assert site_rel_err(w.pop(), want) < TOL[prec]
         wn2 = float((want.astype(np.float64) ** 2).sum())
         assert abs(lqx.norm2(w) - wn2) / wn2 < RTOL[prec]
+
+
+# ------------------------------------------------------------------------------------------------
+# NEXT-2: run-time expression fusion (NVRTC) against the oracle's generic evaluator
+# ------------------------------------------------------------------------------------------------
+def _hop_expr(lqx, fu, fpsi):
+    e = None
+    for mu in range(4):
+        t = lqx.Expr.leaf(fu[mu]) * lqx.shifted(fpsi, lqx.FORWARD, mu) + lqx.shifted(lqx.adj(fu[mu]) * lqx.Expr.leaf(fpsi), lqx.BACKWARD, mu)
+        e = t if e is None else e + t
+    return e
+
+
+def _staple_expr(lqx, fu, mu):
+    e = None
+    for nu in range(4):
+        if nu == mu:
+            continue
+        up = lqx.Expr.leaf(fu[nu]) * lqx.shifted(fu[mu], lqx.FORWARD, nu) * lqx.adj(lqx.shifted(fu[nu], lqx.FORWARD, mu))
+        lo = lqx.shifted(lqx.adj(fu[nu]) * lqx.Expr.leaf(fu[mu]) * lqx.shifted(fu[nu], lqx.FORWARD, mu), lqx.BACKWARD, nu)
+        e = up + lo if e is None else e + (up + lo)
+    return e
+
+
+@pytest.mark.parametrize("dims", [DIMS_RAGGED, (2, 2, 2, 2)])
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+def test_expr_eval_against_oracle(lqx, dims, prec):
+    u = _links(2, dims, prec)
+    a, b, c, d = (_gauss(7, k, dims, "cm", prec) for k in range(4))
+    with lqx.Lattice(dims) as lat:
+        fu = [lat.from_host(t) for t in u]
+        fa, fb, fc, fd = (lat.from_host(t) for t in (a, b, c, d))
+        r = lat.alloc(lqx.COLORMAT, fa.prec)
+        host = {id(f): h for f, h in zip(fu + [fa, fb, fc, fd], u + [a, b, c, d])}
+
+        def want_of(e):  # the oracle on the expression's own postfix sequence and leaf order
+            return orc.eval_expr(dims, e.nodes, [host[id(f)] for f in e.leaves])
+
+        # form i and form iii as run-time expressions
+        e = lqx.Expr.leaf(fa) * lqx.Expr.leaf(fb) + lqx.Expr.leaf(fc) * lqx.adj(fd)
+        lqx.expr_eval(r, e)
+        assert site_rel_err(r.pop(), want_of(e)) < TOL[prec]
+        n0 = lat.expr_cache_size()
+        e3 = 2.5 * lqx.Expr.leaf(fa) - lqx.shifted(fb, lqx.BACKWARD, 2)
+        lqx.expr_eval(r, e3)
+        got = r.pop()
+        assert site_rel_err(got, want_of(e3)) < TOL[prec]
+        lqx.ax_minus_shift(r, 2.5, fa, fb, lqx.BACKWARD, 2)
+        assert site_rel_err(got, r.pop()) < TOL[prec]  # the hand-written kernel of the same expression
+        assert lat.expr_cache_size() == n0 + 1
+        lqx.expr_eval(r, 7.0 * lqx.Expr.leaf(fa) - lqx.shifted(fb, lqx.BACKWARD, 2))  # other scalar: same kernel
+        assert lat.expr_cache_size() == n0 + 1
+        assert site_rel_err(r.pop(), orc.eval_expr(dims, [(0, 0, 0, 0), (5, 0, 0, 7.0), (0, 1, 0, 0), (6, -1, 2, 0), (4, 0, 0, 0)], [a, b])) < TOL[prec]
+        # the paper's E1/E2 expression, exactly as Listing 1 writes it, summed over mu; '=' then '+='
+        for kind in ("f", "cv"):
+            psi = _gauss(2, 10, dims, kind, prec)
+            fpsi = lat.from_host(psi)
+            host[id(fpsi)] = psi
+            chi = lat.alloc(fpsi.kind, fpsi.prec)
+            eh = _hop_expr(lqx, fu, fpsi)
+            lqx.expr_eval(chi, eh)
+            want = want_of(eh)
+            assert site_rel_err(want, orc.hop(dims, u, psi, orc.truth_variant(prec))) < 1e-12
+            assert site_rel_err(chi.pop(), want) < TOL[prec]
+            lqx.expr_eval(chi, eh, accumulate=True)
+            assert site_rel_err(chi.pop(), 2.0 * want) < TOL[prec]
+            ref = lat.alloc(fpsi.kind, fpsi.prec)
+            lqx.hop(ref, fu, fpsi)
+            assert site_rel_err(ref.pop(), want) < TOL[prec]
+        # nested shifts: the staple sum of one direction as ONE expression
+        es = _staple_expr(lqx, fu, 1)
+        lqx.expr_eval(r, es)
+        assert site_rel_err(r.pop(), orc.staple_sum(dims, u, 1, orc.truth_variant(prec))) < TOL[prec]
+        # in place where it is legal, refused where the destination is read through a shift
+        lqx.expr_eval(fa, lqx.Expr.leaf(fa) * lqx.Expr.leaf(fb))
+        assert site_rel_err(fa.pop(), orc.eval_expr(dims, [(0, 0, 0, 0), (0, 1, 0, 0), (2, 0, 0, 0)], [a, b])) < TOL[prec]
+        with pytest.raises(lqx.LqxError):
+            lqx.expr_eval(fb, lqx.Expr.leaf(fc) - lqx.shifted(fb, lqx.FORWARD, 0))
+        with pytest.raises(lqx.LqxError):  # kind mismatch with the destination
+            lqx.expr_eval(r, _hop_expr(lqx, fu, lat.from_host(_gauss(2, 10, dims, "cv", prec))))
