@@ -351,6 +351,48 @@ def _extras(torch, lqx, li, hbm_gbs):
     return out
 
 
+def run_sweep(args):
+    """NEXT-3: the paper's launch-geometry experiment (Figs. 1 and 2: performance against
+    N_threads for N_site in {1,2,4,8} and against N_site for N_threads in {32,..,256}, on E2 at 32^3x64 SP) redone
+    on the fused Jacobi iteration: P(N_threads, N_site) in GFLOPS (canonical 2328 flops per site and iteration)
+    and as a fraction of the HBM roofline.  Prints one JSON line with key "geometry_sweep"."""
+    import torch
+
+    import lattice_inputs as li
+    import paper_1105_2279_b200 as lqx
+
+    hbm_gbs = _peaks()[0]
+    dims = li.CONFIGS["c5"]["dims"]  # 32^3x64, the paper's sweep lattice
+    rows = []
+    iters = 20
+    for prec, pcode in (("f32", lqx.F32), ("f64", lqx.F64)):
+        with lqx.Lattice(dims) as lat:
+            u = []
+            for mu in range(4):
+                a = li._as_real(li.haar_su3_complex(2, mu, lat.volume, "cuda"), prec)
+                u.append(lat.alloc(lqx.COLORMAT, pcode).import_dev(a))
+                del a
+            chi = lat.alloc(lqx.FERMION, pcode).import_dev(li.gaussian_field(2, 10, dims, "f", prec, device="cuda"))
+            tmp = [lat.alloc(lqx.FERMION, pcode) for _ in range(2)]
+            for nthreads in (32, 64, 128, 256):
+                for nsite in (1, 2, 4):
+                    lat.set_option("jacobi_block", nthreads)
+                    lat.set_option("jacobi_sites", nsite)
+                    fn = lambda: lqx.jacobi_smear(chi, u, 0.01, iters, -1, 1.0, tmp)
+                    for _ in range(3):
+                        fn()
+                    torch.cuda.synchronize()
+                    med, best = _time_kernel(torch, fn, 7)
+                    per_it = med / iters
+                    nbytes = lat.volume * 144 * (4 if prec == "f32" else 8)
+                    rows.append({"dtype": prec, "n_threads": nthreads, "n_site": nsite, "us_per_iteration": round(per_it * 1e3, 2),
+                                 "gflops": lat.volume * 2328 / (per_it * 1e-3) / 1e9, "hbm_frac": nbytes / (per_it * 1e-3) / 1e9 / hbm_gbs})
+    best = {p: max((r for r in rows if r["dtype"] == p), key=lambda r: r["gflops"]) for p in ("f32", "f64")}
+    print(json.dumps({"geometry_sweep": {"kernel": "k_jacobi_step (one fused Jacobi iteration, fermion)", "dims": list(dims), "rows": rows,
+                                         "best": best, "paper": "GTX 480: N_threads = 32 best for every expression, N_site 4 or 8 "
+                                                                "slightly better than 1 (PAPER.md:248, :260)"}}))
+
+
 def run_ours(args):
     import torch
 
@@ -539,6 +581,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="c4", choices=sorted(WORKLOADS))
     ap.add_argument("--no-extras", action="store_true", help="skip the per-kernel numbers of the other configs")
+    ap.add_argument("--sweep-geometry", action="store_true",
+                    help="NEXT-3: P(N_threads, N_site) of the fused Jacobi iteration at 32^3x64 (the paper's Figs. 1-2)")
     ap.add_argument("--extras-only", action="store_true",
                     help="only the per-kernel numbers of configs 2, 3, 5 and the Jacobi routine (one JSON line with key "
                          "'kernels'): the command ncu wraps for the catalogue / hop / Jacobi kernels")
@@ -547,7 +591,9 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=5, help="cap on host-buffer steps timed for e2e")
     ap.add_argument("--ref-sites", type=int, default=400000, help="sites per step of the --impl reference sample")
     args = ap.parse_args()
-    if args.extras_only:
+    if args.sweep_geometry:
+        run_sweep(args)
+    elif args.extras_only:
         import torch
 
         import lattice_inputs as li

@@ -242,7 +242,9 @@ int64_t lqx_launch_count(const lqx_ctx* ctx);
  * threads per site; variants fall back to 3 where none of their tile shapes divides the lattice.
  * "tile" -1 = automatic, 0 = linear 128-site blocks, 1..6 = CTA tile shape (8x4x4x2, 8x4x2x2,
  * 4x4x4x2, 16x4x2x2, 16x2x2x2, 32x2x2x2) of the nearest-neighbour kernels, used if it divides the
- * lattice.  "time_kernels" 0/1 (see above).  All variants agree within rounding; DESIGN.md sec.6. */
+ * lattice.  "jacobi_block" (32, 64, 128, 256) and "jacobi_sites" (1, 2, 4): the paper's launch
+ * geometry parameters N_threads and N_site for lqx_jacobi_smear; 0 = tuned default.
+ * "time_kernels" 0/1 (see above).  All variants agree within rounding; DESIGN.md sec.6. */
 int lqx_set_option(lqx_ctx* ctx, const char* key, int value);
 
 const char* lqx_strerror(int code);

@@ -45,6 +45,7 @@ struct lqx_ctx {
     int num_sms;
     int opt_smear_variant;
     int opt_block;
+    int opt_jacobi_block, opt_jacobi_sites;  // launch geometry of the Jacobi step (0 = default 128 x 1)
     int opt_tile;  // -1 = automatic, 0 = Linear, 1..3 = TileA..TileC (lqx_smear.cuh)
     // optional per-kernel-class device timing (bench harness): cudaEvent pairs on the stream
     bool timing;

@@ -63,53 +63,58 @@ __global__ void __launch_bounds__(MAP::THREADS, (sizeof(T) == 4 ? 768 : 512) / M
 // six; DIV: the last iteration also applies E4, chi /= norm (a true division, reading A22).
 // dirmask bit mu = direction mu takes part.
 // ---------------------------------------------------------------------------------------------
-template <typename T, int NSPIN, bool DIV>
-__global__ void __launch_bounds__(128, sizeof(T) == 4 ? 6 : 4) k_jacobi_step(const __grid_constant__ Geo g, const __grid_constant__ Links<T> u,
+// Launch geometry (the paper's two tuning parameters): N_threads = blockDim.x (32..256)
+// and N_site = NSITE sites per thread, taken grid-strided so that a warp still reads 32 consecutive sites.
+template <typename T, int NSPIN, bool DIV, int NSITE>
+__global__ void __launch_bounds__(256, sizeof(T) == 4 ? 3 : 2) k_jacobi_step(const __grid_constant__ Geo g, const __grid_constant__ Links<T> u,
                                                                              int dirmask, const T* __restrict__ psi, const T* __restrict__ s0,
                                                                              T kappa, T nrm, T* __restrict__ chi) {
-    const int s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= g.V) return;
-    int x[4];
-    site_coords(g, s, x);
-    Vec3<T> acc[NSPIN];
+#pragma unroll 1
+    for (int k = 0; k < NSITE; ++k) {
+        const int s = (k * gridDim.x + blockIdx.x) * blockDim.x + threadIdx.x;
+        if (s >= g.V) return;
+        int x[4];
+        site_coords(g, s, x);
+        Vec3<T> acc[NSPIN];
 #pragma unroll
-    for (int a = 0; a < NSPIN; ++a)
+        for (int a = 0; a < NSPIN; ++a)
 #pragma unroll
-        for (int i = 0; i < 3; ++i) acc[a].re[i] = acc[a].im[i] = T(0);
+            for (int i = 0; i < 3; ++i) acc[a].re[i] = acc[a].im[i] = T(0);
 #pragma unroll
-    for (int mu = 0; mu < 4; ++mu) {
-        if (!((dirmask >> mu) & 1)) continue;
-        const int f = nbr_fwd(g, s, x, mu), b = nbr_bwd(g, s, x, mu);
-        {
-            const Mat3<T> m = load_mat(u.u[mu], s);
-            Vec3<T> v[NSPIN];
-            load_vecs<T, NSPIN>(psi, f, v);
+        for (int mu = 0; mu < 4; ++mu) {
+            if (!((dirmask >> mu) & 1)) continue;
+            const int f = nbr_fwd(g, s, x, mu), b = nbr_bwd(g, s, x, mu);
+            {
+                const Mat3<T> m = load_mat(u.u[mu], s);
+                Vec3<T> v[NSPIN];
+                load_vecs<T, NSPIN>(psi, f, v);
 #pragma unroll
-            for (int a = 0; a < NSPIN; ++a) mac_mv(acc[a], m, v[a]);
-        }
-        {
-            const Mat3<T> m = load_mat(u.u[mu], b);
-            Vec3<T> v[NSPIN];
-            load_vecs<T, NSPIN>(psi, b, v);
-#pragma unroll
-            for (int a = 0; a < NSPIN; ++a) mac_adj_mv(acc[a], m, v[a]);
-        }
-    }
-    Vec3<T> src[NSPIN];
-    load_vecs<T, NSPIN>(s0, s, src);
-#pragma unroll
-    for (int a = 0; a < NSPIN; ++a)
-#pragma unroll
-        for (int i = 0; i < 3; ++i) {
-            T re = fma(kappa, acc[a].re[i], src[a].re[i]), im = fma(kappa, acc[a].im[i], src[a].im[i]);
-            if (DIV) {
-                re = re / nrm;
-                im = im / nrm;
+                for (int a = 0; a < NSPIN; ++a) mac_mv(acc[a], m, v[a]);
             }
-            acc[a].re[i] = re;
-            acc[a].im[i] = im;
+            {
+                const Mat3<T> m = load_mat(u.u[mu], b);
+                Vec3<T> v[NSPIN];
+                load_vecs<T, NSPIN>(psi, b, v);
+#pragma unroll
+                for (int a = 0; a < NSPIN; ++a) mac_adj_mv(acc[a], m, v[a]);
+            }
         }
-    store_vecs<T, NSPIN>(chi, s, acc);
+        Vec3<T> src[NSPIN];
+        load_vecs<T, NSPIN>(s0, s, src);
+#pragma unroll
+        for (int a = 0; a < NSPIN; ++a)
+#pragma unroll
+            for (int i = 0; i < 3; ++i) {
+                T re = fma(kappa, acc[a].re[i], src[a].re[i]), im = fma(kappa, acc[a].im[i], src[a].im[i]);
+                if (DIV) {
+                    re = re / nrm;
+                    im = im / nrm;
+                }
+                acc[a].re[i] = re;
+                acc[a].im[i] = im;
+            }
+        store_vecs<T, NSPIN>(chi, s, acc);
+    }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -412,15 +417,27 @@ extern "C" int lqx_jacobi_smear(lqx_field* chi, const lqx_field* const u[4], dou
     if (rc) return rc;
     const lqx_field* cur = (iter & 1) ? tmp[0] : chi;
     lqx_field* nxt = (iter & 1) ? chi : tmp[1];
-    const int grid = (g.V + 127) / 128;
+    // launch geometry: options "jacobi_block" (N_threads: 32, 64, 128, 256) and "jacobi_sites" (N_site: 1, 2, 4)
+    // defaults from the sweep on B200 (bench.py --sweep-geometry): 32 x 1 in fp32 -- as on the
+    // paper's GTX 480 --, 128 x 1 in fp64 (where the block size makes no measurable difference)
+    const int ob = ctx->opt_jacobi_block;
+    const int bs = (ob == 32 || ob == 64 || ob == 128 || ob == 256) ? ob : (chi->prec == LQX_F32 ? 32 : 128);
+    const int nsite = (ctx->opt_jacobi_sites == 2 || ctx->opt_jacobi_sites == 4) ? ctx->opt_jacobi_sites : 1;
+    const int grid = (g.V + bs * nsite - 1) / (bs * nsite);
     const bool ferm = chi->kind == LQX_FERMION;
     for (int it = 0; it < iter; ++it) {
         const bool last = it == iter - 1;
         {
             LqxTimed timed(ctx, LQX_K_HOP);
-#define LQX_JAC(T, NSPIN, DIV)                                                                                                   \
-    k_jacobi_step<T, NSPIN, DIV><<<grid, 128, 0, ctx->stream>>>(g, make_links<T>(u), dirmask, (const T*)cur->data,           \
-                                                                (const T*)tmp[0]->data, (T)kappa, (T)norm, (T*)nxt->data)
+#define LQX_JAC3(T, NSPIN, DIV, NS)                                                                                              \
+    k_jacobi_step<T, NSPIN, DIV, NS><<<grid, bs, 0, ctx->stream>>>(g, make_links<T>(u), dirmask, (const T*)cur->data,         \
+                                                                   (const T*)tmp[0]->data, (T)kappa, (T)norm, (T*)nxt->data)
+#define LQX_JAC(T, NSPIN, DIV)                                \
+    do {                                                      \
+        if (nsite == 1) LQX_JAC3(T, NSPIN, DIV, 1);           \
+        else if (nsite == 2) LQX_JAC3(T, NSPIN, DIV, 2);      \
+        else LQX_JAC3(T, NSPIN, DIV, 4);                      \
+    } while (0)
             if (chi->prec == LQX_F32) {
                 if (ferm) { if (last) LQX_JAC(float, 4, true); else LQX_JAC(float, 4, false); }
                 else      { if (last) LQX_JAC(float, 1, true); else LQX_JAC(float, 1, false); }
@@ -429,6 +446,7 @@ extern "C" int lqx_jacobi_smear(lqx_field* chi, const lqx_field* const u[4], dou
                 else      { if (last) LQX_JAC(double, 1, true); else LQX_JAC(double, 1, false); }
             }
 #undef LQX_JAC
+#undef LQX_JAC3
         }
         LQX_LAUNCH_CHECK(ctx);
         cur = nxt;
