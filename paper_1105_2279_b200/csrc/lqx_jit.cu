@@ -10,6 +10,7 @@
 #include <string.h>
 
 #include <map>
+#include <mutex>
 #include <sstream>
 
 #include "lqx_internal.cuh"
@@ -196,6 +197,7 @@ struct JitCache {
     std::map<std::string, JitKernel> kernels;
 };
 std::map<lqx_ctx*, JitCache> g_caches;  // per context; emptied by lqx_jit_release (called from lqx_finalize)
+std::mutex g_caches_mutex;              // contexts may live on different host threads
 
 // recursive code generation: emits statements into `os`, returns the name of the value's variable.
 // A site is a variable holding its index plus the names of its four coordinates, so that a shift is a
@@ -383,6 +385,7 @@ int compile(lqx_ctx* ctx, const std::string& source, JitKernel* out) {
 }  // namespace
 
 void lqx_jit_release(lqx_ctx* ctx) {
+    std::lock_guard<std::mutex> lock(g_caches_mutex);
     auto it = g_caches.find(ctx);
     if (it == g_caches.end()) return;
     for (auto& kv : it->second.kernels) cudaLibraryUnload(kv.second.lib);
@@ -391,6 +394,7 @@ void lqx_jit_release(lqx_ctx* ctx) {
 
 extern "C" int lqx_expr_cache_size(const lqx_ctx* ctx) {
     if (!ctx) return LQX_EINVAL;
+    std::lock_guard<std::mutex> lock(g_caches_mutex);
     auto it = g_caches.find(const_cast<lqx_ctx*>(ctx));
     return it == g_caches.end() ? 0 : (int)it->second.kernels.size();
 }
@@ -442,13 +446,18 @@ extern "C" int lqx_expr_eval(lqx_field* dst, int accumulate, const lqx_xnode* no
     LQX_CUDA(ctx, cudaSetDevice(ctx->device));
     const bool f32 = dst->prec == LQX_F32;
     const std::string src = make_source(tree, nleaves, (int)scalars.size(), (int)dst->kind, f32, accumulate != 0);
-    JitCache& cache = g_caches[ctx];
-    auto it = cache.kernels.find(src);
-    if (it == cache.kernels.end()) {
-        JitKernel k;
-        rc = compile(ctx, src, &k);
-        if (rc) return rc;
-        it = cache.kernels.insert(std::make_pair(src, k)).first;
+    cudaKernel_t fn;
+    {
+        std::lock_guard<std::mutex> lock(g_caches_mutex);
+        JitCache& cache = g_caches[ctx];
+        auto it = cache.kernels.find(src);
+        if (it == cache.kernels.end()) {
+            JitKernel k;
+            rc = compile(ctx, src, &k);
+            if (rc) return rc;
+            it = cache.kernels.insert(std::make_pair(src, k)).first;
+        }
+        fn = it->second.fn;
     }
     // arguments: geometry, scalars (rounded once to the field precision, reading A10), leaf pointers, destination
     struct JGeo {
@@ -479,7 +488,7 @@ extern "C" int lqx_expr_eval(lqx_field* dst, int accumulate, const lqx_xnode* no
     const int grid = (ctx->geo.V + 127) / 128;
     {
         LqxTimed timed(ctx, LQX_K_CATALOGUE);
-        LQX_CUDA(ctx, cudaLaunchKernel((const void*)it->second.fn, dim3(grid), dim3(128), args, 0, ctx->stream));
+        LQX_CUDA(ctx, cudaLaunchKernel((const void*)fn, dim3(grid), dim3(128), args, 0, ctx->stream));
     }
     ctx->launches++;
     return LQX_OK;
