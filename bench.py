@@ -340,6 +340,10 @@ def _extras(torch, lqx, li, hbm_gbs):
             jit_s = time.perf_counter() - t0
             add("form i  as a run-time expression (NVRTC) c5", prec, v, 90, 414, lambda: lqx.expr_eval(r, e1))
             out[-1]["first_use_compile_s"] = round(jit_s, 3)
+            add("norm2(A*B+C*adj(D)) fused into one generated kernel (incl. sync)", prec, v, 72, 414 + 36,
+                lambda: lqx.expr_reduce(lqx.R_NORM2, e1), lat=lat, kclass=lqx.K_REDUCE)
+            add("sum(trace(A*B)) fused into one generated kernel (incl. sync)", prec, v, 36, 70 + 2,
+                lambda: lqx.expr_reduce(lqx.R_SUM, (lqx.Expr.leaf(cm[0]) * lqx.Expr.leaf(cm[1])).trace()), lat=lat, kclass=lqx.K_REDUCE)
             e3 = 2.5 * lqx.Expr.leaf(cm[0]) - lqx.shifted(cm[1], lqx.BACKWARD, 2)
             add("form iii as a run-time expression (NVRTC) c5", prec, v, 54, 36, lambda: lqx.expr_eval(r, e3))
             add("shift(A,FORWARD,3) c5", prec, v, 36, 0, lambda: lqx.shift(r, cm[0], lqx.FORWARD, 3))

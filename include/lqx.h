@@ -163,6 +163,7 @@ int lqx_jacobi_smear(lqx_field* chi, const lqx_field* const u[4], double kappa, 
  *   ADD / SUB                               left + right, left - right  same kind
  *   SCALE s = real scalar                   s * top                     any kind
  *   SHIFT a = LQX_FORWARD/LQX_BACKWARD, b = mu   shift(top, a, b): the operand evaluated at x + a*mu^
+ *   TRACE                                   trace(top): colour matrix -> LatticeComplex (configs[4] form ii)
  * (shifts nest: shift(adj(u)*psi, BACKWARD, mu) is the Listing's form).
  * dst = expr (accumulate == 0) or dst += expr (accumulate != 0, E2 of the Listing).  dst may alias
  * a leaf that is not read through a shift; otherwise LQX_EALIAS.  At most 16 leaves and 16 scalars.
@@ -170,7 +171,8 @@ int lqx_jacobi_smear(lqx_field* chi, const lqx_field* const u[4], double kappa, 
  * failure (lqx_last_error holds the NVRTC log).  Asynchronous on the context's stream.
  * ------------------------------------------------------------------------------------------- */
 typedef enum { LQX_X_LEAF = 0, LQX_X_ADJ = 1, LQX_X_MUL = 2, LQX_X_ADD = 3, LQX_X_SUB = 4, LQX_X_SCALE = 5,
-               LQX_X_SHIFT = 6 } lqx_xop;
+               LQX_X_SHIFT = 6, LQX_X_TRACE = 7 } lqx_xop;
+typedef enum { LQX_R_NORM2 = 1, LQX_R_SUM = 2 } lqx_xreduce;
 typedef struct {
     int32_t op; /* lqx_xop */
     int32_t a, b;
@@ -178,8 +180,16 @@ typedef struct {
 } lqx_xnode;
 int lqx_expr_eval(lqx_field* dst, int accumulate, const lqx_xnode* nodes, int nnodes,
                   const lqx_field* const* leaves, int nleaves);
+/* Global reduction of an expression without materialising it (configs[4]: "each with norm2/sum/trace
+ * reduction"): what = LQX_R_NORM2 -> out[0] = sum_x sum_components |expr|^2; LQX_R_SUM -> out[0..2*kind) =
+ * sum_x expr(x) as one site object in QDP order (sum of trace(expr) is the global trace, reading A12).
+ * fp64 accumulation, fixed summation tree; *out_count (may be NULL) = doubles written.  Synchronises.
+ * The context and precision are those of leaves[0]. */
+int lqx_expr_reduce(int what, const lqx_xnode* nodes, int nnodes, const lqx_field* const* leaves,
+                    int nleaves, double* out, int* out_count);
 /* The CUDA source the library generates for an expression (for inspection and tests; needs no GPU:
- * ctx may be NULL): written NUL-terminated into buf; returns its full length or a negative status. */
+ * ctx may be NULL): written NUL-terminated into buf; returns its full length or a negative status.
+ * accumulate: 0 '=', 1 '+=', 2 / 3 the norm2 / sum kernel lqx_expr_reduce uses (dst_kind = the expression's). */
 int lqx_expr_source(lqx_ctx* ctx, lqx_kind dst_kind, lqx_prec prec, int accumulate, const lqx_xnode* nodes,
                     int nnodes, const lqx_kind* leaf_kinds, int nleaves, char* buf, size_t buflen);
 /* Number of distinct expression kernels this context has compiled so far. */

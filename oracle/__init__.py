@@ -188,7 +188,7 @@ def jacobi_smear(dims, u, chi, kappa, iters, no_smear_dir, norm, variant):
 
 
 # ---------------------------------------------------------------- generic expressions (NEXT-2)
-X_LEAF, X_ADJ, X_MUL, X_ADD, X_SUB, X_SCALE, X_SHIFT = range(7)
+X_LEAF, X_ADJ, X_MUL, X_ADD, X_SUB, X_SCALE, X_SHIFT, X_TRACE = range(8)
 
 
 def eval_expr(dims, nodes, leaves):
@@ -224,6 +224,9 @@ def eval_expr(dims, nodes, leaves):
             stack.append(float(s) * stack.pop())
         elif op == X_SHIFT:
             stack.append(stack.pop()[neighbor_table(dims, int(a), int(b))])
+        elif op == X_TRACE:
+            m = stack.pop()
+            stack.append(m[:, 0, 0] + m[:, 1, 1] + m[:, 2, 2])
         else:
             raise ValueError(f"unknown operator {op}")
     if len(stack) != 1:

@@ -78,6 +78,7 @@ SIGNATURES = {
     "lqx_hop_norm2": (_i, [_vp, _pvp, _vp, _pd]),
     "lqx_jacobi_smear": (_i, [_vp, _pvp, _d, _i, _i, _d, _pvp]),
     "lqx_expr_eval": (_i, [_vp, _i, _vp, _i, _pvp, _i]),
+    "lqx_expr_reduce": (_i, [_i, _vp, _i, _pvp, _i, _pd, C.POINTER(C.c_int)]),
     "lqx_expr_source": (_i, [_vp, _i, _i, _i, _vp, _i, C.POINTER(C.c_int), _i, C.c_char_p, C.c_size_t]),
     "lqx_expr_cache_size": (_i, [_vp]),
     "lqx_axpy": (_i, [_vp, _vp, _d, _vp]),
@@ -328,7 +329,8 @@ def jacobi_smear(chi, u, kappa, iters, no_smear_dir, norm, tmp):
 
 
 # ---- run-time expression fusion: a tiny builder for the flattened postfix tree of lqx_expr_eval
-X_LEAF, X_ADJ, X_MUL, X_ADD, X_SUB, X_SCALE, X_SHIFT = range(7)
+X_LEAF, X_ADJ, X_MUL, X_ADD, X_SUB, X_SCALE, X_SHIFT, X_TRACE = range(8)
+R_NORM2, R_SUM = 1, 2
 
 
 class _XNode(C.Structure):
@@ -387,6 +389,9 @@ class Expr:
     def shift(self, direction, mu):
         return Expr(self.nodes + [(X_SHIFT, int(direction), int(mu), 0.0)], self.leaves)
 
+    def trace(self):
+        return Expr(self.nodes + [(X_TRACE, 0, 0, 0.0)], self.leaves)
+
     def _c_nodes(self):
         arr = (_XNode * len(self.nodes))()
         for i, (op, a, b, s) in enumerate(self.nodes):
@@ -409,11 +414,22 @@ def expr_eval(dst, expr, accumulate=False):
            _ctx_of(dst))
 
 
-def expr_source(lat, dst_kind, prec, expr, accumulate=False) -> str:
+def expr_reduce(what, expr):
+    """norm2 (what = R_NORM2 -> float) or sum (R_SUM -> array of 2*kind doubles, QDP order) of an expression,
+    evaluated and reduced in one generated kernel."""
+    leaves = (C.c_void_p * len(expr.leaves))(*[_h(f) for f in expr.leaves])
+    out = (C.c_double * 24)()
+    n = C.c_int()
+    _check(_lib.lqx_expr_reduce(int(what), expr._c_nodes(), len(expr.nodes), leaves, len(expr.leaves), out, C.byref(n)),
+           _ctx_of(expr.leaves[0]))
+    return out[0] if what == R_NORM2 else np.array(out[: n.value])
+
+
+def expr_source(lat, dst_kind, prec, expr, accumulate=False, reduce=0) -> str:
     """The CUDA source generated for expr; leaves may be Field objects or kind codes."""
     kinds = (C.c_int * max(1, len(expr.leaves)))(*[f.kind if isinstance(f, Field) else int(f) for f in expr.leaves])
     buf = C.create_string_buffer(1 << 16)
-    n = _lib.lqx_expr_source(lat.ctx if isinstance(lat, Lattice) else lat, dst_kind, prec, 1 if accumulate else 0, expr._c_nodes(),
+    n = _lib.lqx_expr_source(lat.ctx if isinstance(lat, Lattice) else lat, dst_kind, prec, (1 + reduce) if reduce else (1 if accumulate else 0), expr._c_nodes(),
                              len(expr.nodes), kinds, len(expr.leaves), buf, len(buf))
     if n < 0:
         raise LqxError(n, _lib.lqx_last_error(lat.ctx if isinstance(lat, Lattice) else lat).decode())

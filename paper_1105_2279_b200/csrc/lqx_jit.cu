@@ -150,6 +150,27 @@ __device__ __forceinline__ Obj<9> jmul(const Obj<9>& a, const Obj<9>& b) {
         }
     return c;
 }
+__device__ __forceinline__ Obj<1> jtrace(const Obj<9>& a) {
+    Obj<1> c;
+    c.re[0] = a.re[0] + a.re[4] + a.re[8];
+    c.im[0] = a.im[0] + a.im[4] + a.im[8];
+    return c;
+}
+// per-CTA sum of NC doubles per thread -> partials[c * gridDim.x + blockIdx.x] (fixed tree: deterministic)
+template <int NC>
+__device__ __forceinline__ void jreduce(double (&v)[NC], double* __restrict__ partials) {
+    __shared__ double sh[4][NC];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int c = 0; c < NC; ++c) {
+        double t = v[c];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+        if (lane == 0) sh[warp][c] = t;
+    }
+    __syncthreads();
+    if (threadIdx.x < NC) partials[(size_t)threadIdx.x * gridDim.x + blockIdx.x] = (sh[0][threadIdx.x] + sh[1][threadIdx.x]) + (sh[2][threadIdx.x] + sh[3][threadIdx.x]);
+}
 template <int NV>
 __device__ __forceinline__ Obj<3 * NV> jmulv(const Obj<9>& m, const Obj<3 * NV>& v) {
     Obj<3 * NV> w;
@@ -245,6 +266,11 @@ struct Gen {
                 os << "    const " << ty << " " << v << " = " << (x.op == LQX_X_ADD ? "jadd" : "jsub") << "(" << l << ", " << r << ");\n";
                 break;
             }
+            case LQX_X_TRACE: {
+                std::string c = val(x.child[0], site);
+                os << "    const " << ty << " " << v << " = jtrace(" << c << ");\n";
+                break;
+            }
             case LQX_X_SCALE: {
                 std::string c = val(x.child[0], site);
                 os << "    const " << ty << " " << v << " = jscale(k" << x.scalar_slot << ", " << c << ");\n";
@@ -282,6 +308,12 @@ int build_tree(lqx_ctx* ctx, const lqx_xnode* nodes, int nnodes, const lqx_field
                 x.child[0] = pop();
                 if (out[x.child[0]].kind != LQX_COLORMAT) return lqx_fail(ctx, LQX_ETYPE, "expr: adj wants a colour matrix");
                 x.kind = LQX_COLORMAT;
+                break;
+            case LQX_X_TRACE:
+                if (stack.empty()) return lqx_fail(ctx, LQX_EINVAL, "expr: trace without operand");
+                x.child[0] = pop();
+                if (out[x.child[0]].kind != LQX_COLORMAT) return lqx_fail(ctx, LQX_ETYPE, "expr: trace wants a colour matrix");
+                x.kind = LQX_COMPLEX;
                 break;
             case LQX_X_MUL:
             case LQX_X_ADD:
@@ -333,7 +365,10 @@ int build_tree(lqx_ctx* ctx, const lqx_xnode* nodes, int nnodes, const lqx_field
     return LQX_OK;
 }
 
-std::string make_source(const std::vector<XNode>& tree, int nleaves, int nscalars, int dst_kind, bool f32, bool accumulate) {
+// reduce: 0 = dst (=|+=) expr ; 1 = norm2(expr) ; 2 = sum(expr).  For the reductions every thread walks a
+// grid-stride loop of sites with fp64 accumulators and the CTA leaves one partial per component.
+std::string make_source(const std::vector<XNode>& tree, int nleaves, int nscalars, int dst_kind, bool f32, bool accumulate,
+                        int reduce) {
     std::ostringstream src;
     if (f32) src << "typedef float T;\ntypedef float4 VEC;\nconstexpr int W = 4;\n";
     else src << "typedef double T;\ntypedef double2 VEC;\nconstexpr int W = 2;\n";
@@ -342,7 +377,14 @@ std::string make_source(const std::vector<XNode>& tree, int nleaves, int nscalar
     src << "extern \"C\" __global__ void __launch_bounds__(128, " << (f32 ? 4 : 2) << ") lqx_jit(const JGeo g";
     for (int k = 0; k < nscalars; ++k) src << ", const T k" << k;
     for (int l = 0; l < nleaves; ++l) src << ", const T* __restrict__ p" << l;
-    src << ", T* dst) {\n    const int s0 = blockIdx.x * blockDim.x + threadIdx.x;\n    if (s0 >= g.V) return;\n";
+    const int nc = reduce == 1 ? 1 : 2 * dst_kind;
+    if (reduce) {
+        src << ", double* __restrict__ partials) {\n    double acc[" << nc << "];\n";
+        src << "#pragma unroll\n    for (int c = 0; c < " << nc << "; ++c) acc[c] = 0.0;\n";
+        src << "    for (int s0 = blockIdx.x * blockDim.x + threadIdx.x; s0 < g.V; s0 += gridDim.x * blockDim.x) {\n";
+    } else {
+        src << ", T* dst) {\n    const int s0 = blockIdx.x * blockDim.x + threadIdx.x;\n    if (s0 >= g.V) return;\n";
+    }
     src << "    const int x0_0 = s0 % g.L[0], q1 = s0 / g.L[0];\n    const int x0_1 = q1 % g.L[1], q2 = q1 / g.L[1];\n"
            "    const int x0_2 = q2 % g.L[2], x0_3 = q2 / g.L[2];\n";
     Gen gen(tree);
@@ -351,8 +393,19 @@ std::string make_source(const std::vector<XNode>& tree, int nleaves, int nscalar
     for (int d = 0; d < 4; ++d) origin.x[d] = "x0_" + std::to_string(d);
     const std::string r = gen.val((int)tree.size() - 1, origin);
     src << gen.os.str();
-    if (accumulate) src << "    jstore<" << dst_kind << ">(dst, s0, jadd(jload<" << dst_kind << ">(dst, s0), " << r << "));\n";
-    else src << "    jstore<" << dst_kind << ">(dst, s0, " << r << ");\n";
+    if (reduce == 1) {
+        src << "#pragma unroll\n    for (int i = 0; i < " << dst_kind << "; ++i) {\n        acc[0] = fma((double)" << r << ".re[i], (double)" << r
+            << ".re[i], acc[0]);\n        acc[0] = fma((double)" << r << ".im[i], (double)" << r << ".im[i], acc[0]);\n    }\n    }\n";
+        src << "    jreduce<1>(acc, partials);\n";
+    } else if (reduce == 2) {
+        src << "#pragma unroll\n    for (int i = 0; i < " << dst_kind << "; ++i) {\n        acc[2 * i] += (double)" << r
+            << ".re[i];\n        acc[2 * i + 1] += (double)" << r << ".im[i];\n    }\n    }\n";
+        src << "    jreduce<" << nc << ">(acc, partials);\n";
+    } else if (accumulate) {
+        src << "    jstore<" << dst_kind << ">(dst, s0, jadd(jload<" << dst_kind << ">(dst, s0), " << r << "));\n";
+    } else {
+        src << "    jstore<" << dst_kind << ">(dst, s0, " << r << ");\n";
+    }
     src << "}\n";
     return src.str();
 }
@@ -418,21 +471,21 @@ extern "C" int lqx_expr_source(lqx_ctx* ctx, lqx_kind dst_kind, lqx_prec prec, i
     int rc = build_tree(ctx, nodes, nnodes, leaves.data(), nleaves, tree, scalars, shifted);
     if (rc) return rc;
     if (tree.back().kind != (int)dst_kind) return lqx_fail(ctx, LQX_ETYPE, "expr: destination kind differs from the expression's");
-    const std::string src = make_source(tree, nleaves, (int)scalars.size(), (int)dst_kind, prec == LQX_F32, accumulate != 0);
+    const int reduce = accumulate >= 2 ? accumulate - 1 : 0;  // 2, 3: the kernels of lqx_expr_reduce (norm2, sum)
+    const std::string src = make_source(tree, nleaves, (int)scalars.size(), (int)dst_kind, prec == LQX_F32, accumulate == 1, reduce);
     strncpy(buf, src.c_str(), buflen - 1);
     buf[buflen - 1] = '\0';
     return (int)src.size();
 }
 
-extern "C" int lqx_expr_eval(lqx_field* dst, int accumulate, const lqx_xnode* nodes, int nnodes, const lqx_field* const* leaves,
-                             int nleaves) {
-    if (!dst || !nodes || nnodes <= 0 || nleaves < 0 || (nleaves > 0 && !leaves)) return LQX_EINVAL;
-    lqx_ctx* ctx = dst->ctx;
+// shared by lqx_expr_eval (reduce = 0, dst != NULL) and lqx_expr_reduce (reduce = 1 norm2 / 2 sum, dst == NULL)
+static int run_expr(lqx_ctx* ctx, lqx_prec prec, lqx_field* dst, int accumulate, int reduce, const lqx_xnode* nodes, int nnodes,
+                    const lqx_field* const* leaves, int nleaves, double* out, int* out_count) {
     if (nleaves > 16) return lqx_fail(ctx, LQX_EINVAL, "expr: at most 16 leaves");
     for (int l = 0; l < nleaves; ++l) {
         if (!leaves[l]) return LQX_EINVAL;
         if (leaves[l]->ctx != ctx) return lqx_fail(ctx, LQX_EGEOM, "expr: leaves belong to different contexts");
-        if (leaves[l]->prec != dst->prec) return lqx_fail(ctx, LQX_ETYPE, "expr: mixed precision");
+        if (leaves[l]->prec != prec) return lqx_fail(ctx, LQX_ETYPE, "expr: mixed precision");
     }
     std::vector<XNode> tree;
     std::vector<double> scalars;
@@ -440,12 +493,15 @@ extern "C" int lqx_expr_eval(lqx_field* dst, int accumulate, const lqx_xnode* no
     int rc = build_tree(ctx, nodes, nnodes, leaves, nleaves, tree, scalars, shifted);
     if (rc) return rc;
     if (scalars.size() > 16) return lqx_fail(ctx, LQX_EINVAL, "expr: at most 16 scalars");
-    if (tree.back().kind != (int)dst->kind) return lqx_fail(ctx, LQX_ETYPE, "expr: destination kind differs from the expression's");
-    for (int l = 0; l < nleaves; ++l)
-        if (shifted[l] && lqx_same(dst, leaves[l])) return lqx_fail(ctx, LQX_EALIAS, "expr: destination is read through a shift");
+    const int kind = tree.back().kind;
+    if (dst) {
+        if (kind != (int)dst->kind) return lqx_fail(ctx, LQX_ETYPE, "expr: destination kind differs from the expression's");
+        for (int l = 0; l < nleaves; ++l)
+            if (shifted[l] && lqx_same(dst, leaves[l])) return lqx_fail(ctx, LQX_EALIAS, "expr: destination is read through a shift");
+    }
     LQX_CUDA(ctx, cudaSetDevice(ctx->device));
-    const bool f32 = dst->prec == LQX_F32;
-    const std::string src = make_source(tree, nleaves, (int)scalars.size(), (int)dst->kind, f32, accumulate != 0);
+    const bool f32 = prec == LQX_F32;
+    const std::string src = make_source(tree, nleaves, (int)scalars.size(), kind, f32, accumulate != 0, reduce);
     cudaKernel_t fn;
     {
         std::lock_guard<std::mutex> lock(g_caches_mutex);
@@ -483,13 +539,40 @@ extern "C" int lqx_expr_eval(lqx_field* dst, int accumulate, const lqx_xnode* no
         ptrs[l] = leaves[l]->data;
         args[na++] = &ptrs[l];
     }
-    void* dptr = dst->data;
+    int grid = (ctx->geo.V + 127) / 128;
+    void* dptr = nullptr;
+    const int nc = reduce == 1 ? 1 : 2 * kind;
+    if (reduce) {
+        grid = std::max(1, std::min(grid, ctx->num_sms * 16));  // fixed function of V: deterministic summation tree
+        rc = lqx_ensure_partials(ctx, (size_t)grid * nc);
+        if (rc) return rc;
+        dptr = ctx->d_partials;
+    } else {
+        dptr = dst->data;
+    }
     args[na++] = &dptr;
-    const int grid = (ctx->geo.V + 127) / 128;
     {
-        LqxTimed timed(ctx, LQX_K_CATALOGUE);
+        LqxTimed timed(ctx, reduce ? LQX_K_REDUCE : LQX_K_CATALOGUE);
         LQX_CUDA(ctx, cudaLaunchKernel((const void*)fn, dim3(grid), dim3(128), args, 0, ctx->stream));
     }
     ctx->launches++;
-    return LQX_OK;
+    if (!reduce) return LQX_OK;
+    rc = lqx_sum_partials(ctx, grid, nc, ctx->h_result);
+    if (rc) return rc;
+    if (out_count) *out_count = nc;
+    return lqx_fetch_result(ctx, nc, out);
+}
+
+extern "C" int lqx_expr_eval(lqx_field* dst, int accumulate, const lqx_xnode* nodes, int nnodes, const lqx_field* const* leaves,
+                             int nleaves) {
+    if (!dst || !nodes || nnodes <= 0 || nleaves < 0 || (nleaves > 0 && !leaves)) return LQX_EINVAL;
+    return run_expr(dst->ctx, dst->prec, dst, accumulate, 0, nodes, nnodes, leaves, nleaves, nullptr, nullptr);
+}
+
+extern "C" int lqx_expr_reduce(int what, const lqx_xnode* nodes, int nnodes, const lqx_field* const* leaves, int nleaves,
+                               double* out, int* out_count) {
+    if (!nodes || nnodes <= 0 || nleaves <= 0 || !leaves || !leaves[0] || !out) return LQX_EINVAL;
+    lqx_ctx* ctx = leaves[0]->ctx;
+    if (what != LQX_R_NORM2 && what != LQX_R_SUM) return lqx_fail(ctx, LQX_EINVAL, "expr_reduce: unknown reduction");
+    return run_expr(ctx, leaves[0]->prec, nullptr, 0, what, nodes, nnodes, leaves, nleaves, out, out_count);
 }

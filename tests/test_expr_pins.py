@@ -13,7 +13,7 @@ import lattice_inputs as li
 import oracle as orc
 from helpers import site_rel_err
 
-L, ADJ, MUL, ADD, SUB, SCALE, SHIFT = range(7)
+L, ADJ, MUL, ADD, SUB, SCALE, SHIFT, TRACE = range(8)
 
 
 def links(seed, dims, prec="f64"):
@@ -66,6 +66,10 @@ def test_evaluator_reduces_to_the_pinned_routines(dims):
         assert site_rel_err(orc.eval_expr(dims, hop_nodes(), u + [psi]), orc.hop(dims, u, psi, "t64")) < 1e-14
     for mu in range(4):
         assert site_rel_err(orc.eval_expr(dims, staple_nodes(mu), u), orc.staple_sum(dims, u, mu, "t64")) < 1e-14
+    # form ii: trace(A*B) -> LatticeComplex
+    tr = orc.eval_expr(dims, [(L, 0, 0, 0), (L, 1, 0, 0), (MUL, 0, 0, 0), (TRACE, 0, 0, 0)], [a, b])
+    want = orc.trace_mm(dims, a, b, "t64")
+    assert tr.shape == want.shape and np.abs(tr - want).max() < 1e-13
 
 
 def test_evaluator_rejects_malformed_sequences():
@@ -127,9 +131,15 @@ def test_generated_source_compiles_for_sm_100a(tmp_path, prec):
     cases = {"hop": (hop_nodes(), [lqx.COLORMAT] * 4 + [lqx.FERMION], lqx.FERMION),
              "staple": (staple_nodes(1), [lqx.COLORMAT] * 4, lqx.COLORMAT),
              "form_iii": (FORM_III, [lqx.COLORMAT] * 2, lqx.COLORMAT)}
-    for name, (nodes, kinds, dk) in cases.items():
+    sources = {name: _source(nodes, kinds, dk, pc) for name, (nodes, kinds, dk) in cases.items()}
+    e = lqx.Expr([(L, 0, 0, 0), (L, 1, 0, 0), (MUL, 0, 0, 0), (TRACE, 0, 0, 0)], [lqx.COLORMAT] * 2)
+    sources["trace_mm"] = lqx.expr_source(None, lqx.COMPLEX, pc, e)
+    sources["norm2_hop"] = lqx.expr_source(None, lqx.FERMION, pc, lqx.Expr(hop_nodes(), [lqx.COLORMAT] * 4 + [lqx.FERMION]), reduce=1)
+    sources["sum_form_i"] = lqx.expr_source(None, lqx.COLORMAT, pc, lqx.Expr(list(FORM_I), [lqx.COLORMAT] * 4), reduce=2)
+    assert "jreduce<1>" in sources["norm2_hop"] and "jreduce<18>" in sources["sum_form_i"] and "jstore" not in sources["norm2_hop"].split("lqx_jit")[1]
+    for name, text in sources.items():
         f = tmp_path / f"{name}_{prec}.cu"
-        f.write_text(_source(nodes, kinds, dk, pc))
+        f.write_text(text)
         r = subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-std=c++17", "-cubin", "-o", str(f) + ".cubin", str(f)],
                            capture_output=True, text=True)
         assert r.returncode == 0, r.stderr[-3000:]

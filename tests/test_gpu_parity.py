@@ -669,3 +669,49 @@ def test_expr_eval_against_oracle(lqx, dims, prec):
             lqx.expr_eval(fb, lqx.Expr.leaf(fc) - lqx.shifted(fb, lqx.FORWARD, 0))
         with pytest.raises(lqx.LqxError):  # kind mismatch with the destination
             lqx.expr_eval(r, _hop_expr(lqx, fu, lat.from_host(_gauss(2, 10, dims, "cv", prec))))
+
+
+@pytest.mark.parametrize("dims", [DIMS_RAGGED, (16, 8, 8, 8)])
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+def test_expr_trace_and_reductions(lqx, dims, prec):
+    """configs[4] through the run-time path: each form followed by its norm2 / sum / trace reduction, the
+    reduction fused into the generated kernel (nothing is materialised)."""
+    a, b, c, d = (_gauss(7, k, dims, "cm", prec) for k in range(4))
+    v = _gauss(7, 4, dims, "cv", prec)
+    with lqx.Lattice(dims) as lat:
+        fa, fb, fc, fd, fv = (lat.from_host(t) for t in (a, b, c, d, v))
+        host = {id(f): h for f, h in zip((fa, fb, fc, fd, fv), (a, b, c, d, v))}
+
+        def want_of(e):
+            return orc.eval_expr(dims, e.nodes, [host[id(f)] for f in e.leaves])
+
+        L = lqx.Expr.leaf
+        # form ii: trace(A*B) into a LatticeComplex, against the hand-written kernel and the oracle
+        e2 = (L(fa) * L(fb)).trace()
+        cx = lat.alloc(lqx.COMPLEX, fa.prec)
+        lqx.expr_eval(cx, e2)
+        got = cx.pop()
+        mag = np.einsum("xik,xki->x", np.abs(cplx(a)), np.abs(cplx(b)))
+        assert float((np.abs(got.astype(np.float64) - want_of(e2)).max(axis=1) / mag).max()) < TOL[prec]
+        cx2 = lat.alloc(lqx.COMPLEX, fa.prec)
+        lqx.trace_mm(cx2, fa, fb)
+        assert float((np.abs(got.astype(np.float64) - cx2.pop()).max(axis=1) / mag).max()) < TOL[prec]
+        for e in (L(fa) * L(fb) + L(fc) * lqx.adj(fd), 2.5 * L(fa) - lqx.shifted(fb, lqx.BACKWARD, 2), L(fa) * L(fv), e2):
+            w = want_of(e)
+            n2w = float((w ** 2).sum())
+            assert abs(lqx.expr_reduce(lqx.R_NORM2, e) - n2w) / n2w < RTOL[prec]
+            sw = w.sum(axis=0).ravel()
+            rms = float(np.sqrt(n2w))
+            assert _red_err(lqx.expr_reduce(lqx.R_SUM, e), sw, rms) < RTOL[prec]
+        # global trace of a matrix expression = sum of its site-wise trace (reading A12)
+        e1 = L(fa) * L(fb) + L(fc) * lqx.adj(fd)
+        r = lat.alloc(lqx.COLORMAT, fa.prec)
+        lqx.expr_eval(r, e1)
+        tr_two_calls = np.asarray(lqx.trace(r))
+        tr_fused = lqx.expr_reduce(lqx.R_SUM, e1.trace())
+        rms = float(np.sqrt((want_of(e1) ** 2).sum()))
+        assert _red_err(tr_fused, tr_two_calls, rms) < RTOL[prec]
+        with pytest.raises(lqx.LqxError):
+            lqx.expr_eval(cx, L(fv).trace())
+        with pytest.raises(lqx.LqxError):
+            lqx.expr_reduce(9, e1)
