@@ -98,6 +98,8 @@ extern "C" int lqx_init(const int dims[4], int device, void* cuda_stream, lqx_ct
     }
     c->num_sms = prop.multiProcessorCount;
     c->d_ticket = nullptr;
+    c->stage = nullptr;
+    c->stage_cap = 0;
     if (cudaMalloc(&c->d_result, 64 * sizeof(double)) != cudaSuccess ||
         cudaMalloc(&c->d_ticket, sizeof(unsigned int)) != cudaSuccess ||
         cudaHostAlloc(&c->h_result, 64 * sizeof(double), cudaHostAllocPortable | cudaHostAllocMapped) != cudaSuccess ||
@@ -127,6 +129,7 @@ extern "C" int lqx_finalize(lqx_ctx* ctx) {
             cudaEventDestroy(pr.second);
         }
     if (ctx->d_partials) cudaFree(ctx->d_partials);
+    if (ctx->stage) cudaFree(ctx->stage);
     if (ctx->d_result) cudaFree(ctx->d_result);
     if (ctx->d_ticket) cudaFree(ctx->d_ticket);
     if (ctx->h_result) cudaFreeHost(ctx->h_result);
@@ -354,44 +357,66 @@ extern "C" int lqx_field_export_dev(const lqx_field* f, void* dev_qdp_order) {
     return transpose_launch(f->ctx, f, f->data, dev_qdp_order, false);
 }
 
+// staging buffer for push/pop (QDP-order copy of one field on the device): cached in the context, grow-only
+static int ensure_stage(lqx_ctx* ctx, size_t bytes) {
+    if (ctx->stage_cap >= bytes) return LQX_OK;
+    if (ctx->stage) {
+        cudaStreamSynchronize(ctx->stream);
+        cudaFree(ctx->stage);
+        ctx->stage = nullptr;
+        ctx->stage_cap = 0;
+    }
+    if (cudaMalloc(&ctx->stage, bytes) != cudaSuccess) {
+        cudaGetLastError();
+        return lqx_fail(ctx, LQX_ENOMEM, "push/pop staging buffer");
+    }
+    ctx->stage_cap = bytes;
+    return LQX_OK;
+}
+
+// sync = false: the copy and the conversion are only enqueued (the caller synchronises before the host buffer
+// is reused or read); stream order keeps successive uses of the one staging buffer apart
+int lqx_push_impl(lqx_field* f, const void* host, bool sync) {
+    lqx_ctx* ctx = f->ctx;
+    const size_t bytes = (size_t)ctx->geo.V * 2 * (int)f->kind * (int)f->prec;
+    int rc = ensure_stage(ctx, bytes);
+    if (rc) return rc;
+    cudaError_t e = cudaMemcpyAsync(ctx->stage, host, bytes, cudaMemcpyHostToDevice, ctx->stream);
+    if (e != cudaSuccess) return lqx_cuda_fail(ctx, e, "push H2D");
+    rc = transpose_launch(ctx, f, ctx->stage, f->data, true);
+    if (rc == LQX_OK && sync) {
+        e = cudaStreamSynchronize(ctx->stream);  // host buffer is only touched during the call
+        if (e != cudaSuccess) rc = lqx_cuda_fail(ctx, e, "push sync");
+    }
+    return rc;
+}
+
+int lqx_pop_impl(const lqx_field* f, void* host, bool sync) {
+    lqx_ctx* ctx = f->ctx;
+    const size_t bytes = (size_t)ctx->geo.V * 2 * (int)f->kind * (int)f->prec;
+    int rc = ensure_stage(ctx, bytes);
+    if (rc) return rc;
+    rc = transpose_launch(ctx, f, f->data, ctx->stage, false);
+    if (rc) return rc;
+    cudaError_t e = cudaMemcpyAsync(host, ctx->stage, bytes, cudaMemcpyDeviceToHost, ctx->stream);
+    if (e != cudaSuccess) return lqx_cuda_fail(ctx, e, "pop D2H");
+    if (sync) {
+        e = cudaStreamSynchronize(ctx->stream);
+        if (e != cudaSuccess) return lqx_cuda_fail(ctx, e, "pop sync");
+    }
+    return LQX_OK;
+}
+
 extern "C" int lqx_field_push(lqx_field* f, const void* host) {
     if (!f || !host) return LQX_EINVAL;
-    lqx_ctx* ctx = f->ctx;
-    LQX_CUDA(ctx, cudaSetDevice(ctx->device));
-    const size_t bytes = (size_t)ctx->geo.V * 2 * (int)f->kind * (int)f->prec;
-    void* stage = nullptr;
-    if (cudaMalloc(&stage, bytes) != cudaSuccess) {
-        cudaGetLastError();
-        return lqx_fail(ctx, LQX_ENOMEM, "push staging buffer");
-    }
-    cudaError_t e = cudaMemcpyAsync(stage, host, bytes, cudaMemcpyHostToDevice, ctx->stream);
-    int rc = LQX_OK;
-    if (e != cudaSuccess) rc = lqx_cuda_fail(ctx, e, "push H2D");
-    if (rc == LQX_OK) rc = transpose_launch(ctx, f, stage, f->data, true);
-    e = cudaStreamSynchronize(ctx->stream);  // host buffer is only touched during the call
-    if (rc == LQX_OK && e != cudaSuccess) rc = lqx_cuda_fail(ctx, e, "push sync");
-    cudaFree(stage);
-    return rc;
+    LQX_CUDA(f->ctx, cudaSetDevice(f->ctx->device));
+    return lqx_push_impl(f, host, true);
 }
 
 extern "C" int lqx_field_pop(const lqx_field* f, void* host) {
     if (!f || !host) return LQX_EINVAL;
-    lqx_ctx* ctx = f->ctx;
-    LQX_CUDA(ctx, cudaSetDevice(ctx->device));
-    const size_t bytes = (size_t)ctx->geo.V * 2 * (int)f->kind * (int)f->prec;
-    void* stage = nullptr;
-    if (cudaMalloc(&stage, bytes) != cudaSuccess) {
-        cudaGetLastError();
-        return lqx_fail(ctx, LQX_ENOMEM, "pop staging buffer");
-    }
-    int rc = transpose_launch(ctx, f, f->data, stage, false);
-    cudaError_t e = cudaSuccess;
-    if (rc == LQX_OK) e = cudaMemcpyAsync(host, stage, bytes, cudaMemcpyDeviceToHost, ctx->stream);
-    if (rc == LQX_OK && e != cudaSuccess) rc = lqx_cuda_fail(ctx, e, "pop D2H");
-    e = cudaStreamSynchronize(ctx->stream);
-    if (rc == LQX_OK && e != cudaSuccess) rc = lqx_cuda_fail(ctx, e, "pop sync");
-    cudaFree(stage);
-    return rc;
+    LQX_CUDA(f->ctx, cudaSetDevice(f->ctx->device));
+    return lqx_pop_impl(f, host, true);
 }
 
 // --------------------------------------------------------------------------------------------

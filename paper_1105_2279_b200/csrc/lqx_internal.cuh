@@ -40,6 +40,8 @@ struct lqx_ctx {
     size_t partials_cap; // in doubles
     double* d_result;    // 64 doubles (device scratch results)
     double* h_result;    // pinned + mapped, 64 doubles: kernels write results straight to the host
+    void* stage;       // device staging buffer of push/pop (one field in QDP order), grow-only
+    size_t stage_cap;
     unsigned int* d_ticket;  // last-block ticket of the one-launch reductions (zero between launches)
     int64_t launches;
     int num_sms;
@@ -80,6 +82,8 @@ struct lqx_field {
 };
 
 int lqx_fail(lqx_ctx* ctx, int code, const char* what);
+int lqx_push_impl(lqx_field* f, const void* host, bool sync);  // lqx_core.cu; sync = false only enqueues
+int lqx_pop_impl(const lqx_field* f, void* host, bool sync);
 void lqx_jit_release(lqx_ctx* ctx);  // unloads the context's run-time compiled expression kernels (lqx_jit.cu)
 int lqx_cuda_fail(lqx_ctx* ctx, cudaError_t e, const char* where);
 int lqx_ensure_partials(lqx_ctx* ctx, size_t ndoubles);

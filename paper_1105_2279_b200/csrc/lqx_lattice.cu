@@ -375,13 +375,21 @@ extern "C" int lqx_smear_iterate_host(lqx_ctx* ctx, lqx_prec prec, const void* c
     lqx_field* u[4] = {nullptr, nullptr, nullptr, nullptr};
     lqx_field* t[4] = {nullptr, nullptr, nullptr, nullptr};
     int rc = LQX_OK;
+    LQX_CUDA(ctx, cudaSetDevice(ctx->device));
+    // all four uploads and conversions are enqueued back to back (no host round trip between them); the
+    // smear kernels follow in stream order; the four downloads are enqueued likewise and ONE synchronisation
+    // ends the call, after which the host buffers are no longer touched
     for (int mu = 0; mu < 4 && rc == LQX_OK; ++mu) {
         rc = lqx_field_alloc(ctx, LQX_COLORMAT, prec, &u[mu]);
         if (rc == LQX_OK) rc = lqx_field_alloc(ctx, LQX_COLORMAT, prec, &t[mu]);
-        if (rc == LQX_OK) rc = lqx_field_push(u[mu], host_u_in[mu]);
+        if (rc == LQX_OK) rc = lqx_push_impl(u[mu], host_u_in[mu], false);
     }
     if (rc == LQX_OK) rc = lqx_smear_iterate(u, t, alpha, nsteps, plaq_avg_after_each);
-    for (int mu = 0; mu < 4 && rc == LQX_OK; ++mu) rc = lqx_field_pop(u[mu], host_u_out[mu]);
+    for (int mu = 0; mu < 4 && rc == LQX_OK; ++mu) rc = lqx_pop_impl(u[mu], host_u_out[mu], false);
+    {
+        cudaError_t e = cudaStreamSynchronize(ctx->stream);
+        if (rc == LQX_OK && e != cudaSuccess) rc = lqx_cuda_fail(ctx, e, "smear_iterate_host sync");
+    }
     for (int mu = 0; mu < 4; ++mu) {
         if (u[mu]) lqx_field_free(u[mu]);
         if (t[mu]) lqx_field_free(t[mu]);
