@@ -328,12 +328,9 @@ int smear_shared_launch(lqx_ctx* ctx, const Links<T>& in, const LinksOut<T>& o, 
     const int grid = MAP::grid(g);
     const TileMap tm = MAP::map(g, kSlabZ);
     const size_t smem = sizeof(T) * 4 * 18 * MAP::THREADS + sizeof(int) * 4 * MAP::THREADS;
-    static bool configured = false;  // per instantiation
-    if (!configured) {
-        LQX_CUDA(ctx, cudaFuncSetAttribute(k_smear_shared<T, true, MAP, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        LQX_CUDA(ctx, cudaFuncSetAttribute(k_smear_shared<T, false, MAP, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        configured = true;
-    }
+    // function attributes are per device: set on every call (microseconds) rather than cached per process
+    if (plaq) LQX_CUDA(ctx, cudaFuncSetAttribute(k_smear_shared<T, true, MAP, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    else LQX_CUDA(ctx, cudaFuncSetAttribute(k_smear_shared<T, false, MAP, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     if (plaq) {
         int rc = lqx_ensure_partials(ctx, (size_t)grid);
         if (rc) return rc;
