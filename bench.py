@@ -256,6 +256,14 @@ def _extras(torch, lqx, li, hbm_gbs):
                 row["kernel_hbm_frac"] = nbytes / (kms / n * 1e-3) / 1e9 / hbm_gbs
         out.append(row)
 
+    # ---- C1: 4^4 fp64, one smear step + plaquette (256 sites: launch latency, exempt from any roofline reading)
+    dims = li.CONFIGS["c1"]["dims"]
+    with lqx.Lattice(dims) as lat:
+        u, _ = _gen_links(lat, lqx, li, "c1", "haar", "f64")
+        o = [lat.alloc(lqx.COLORMAT, lqx.F64) for _ in range(4)]
+        add("smear_step c1 (4^4: launch-latency-bound)", "f64", lat.volume, 144, SMEAR_CANONICAL_FLOPS, lambda: lqx.smear_step(o, u, ALPHA), reps=20)
+        add("smear_step+plaquette(in) fused c1 (incl. sync)", "f64", lat.volume, 144, SMEAR_CANONICAL_FLOPS + 108,
+            lambda: lqx.smear_step(o, u, ALPHA, want_plaq_in=True), reps=20)
     # ---- C2: hop, 16^3x32 fp32 (working set 63 MB < L2: cold and warm)
     dims = li.CONFIGS["c2"]["dims"]
     with lqx.Lattice(dims) as lat:

@@ -99,6 +99,7 @@ extern "C" int lqx_init(const int dims[4], int device, void* cuda_stream, lqx_ct
     c->num_sms = prop.multiProcessorCount;
     c->d_ticket = nullptr;
     c->stage = nullptr;
+    for (int k = 0; k < 8; ++k) c->host_work[k] = nullptr;
     c->stage_cap = 0;
     if (cudaMalloc(&c->d_result, 64 * sizeof(double)) != cudaSuccess ||
         cudaMalloc(&c->d_ticket, sizeof(unsigned int)) != cudaSuccess ||

@@ -40,6 +40,7 @@ struct lqx_ctx {
     size_t partials_cap; // in doubles
     double* d_result;    // 64 doubles (device scratch results)
     double* h_result;    // pinned + mapped, 64 doubles: kernels write results straight to the host
+    lqx_field* host_work[8];  // work fields of lqx_smear_iterate_host, kept between calls
     void* stage;       // device staging buffer of push/pop (one field in QDP order), grow-only
     size_t stage_cap;
     unsigned int* d_ticket;  // last-block ticket of the one-launch reductions (zero between launches)

@@ -372,27 +372,30 @@ extern "C" int lqx_smear_iterate_host(lqx_ctx* ctx, lqx_prec prec, const void* c
     if (!ctx || !host_u_in || !host_u_out) return LQX_EINVAL;
     for (int mu = 0; mu < 4; ++mu)
         if (!host_u_in[mu] || !host_u_out[mu]) return LQX_EINVAL;
-    lqx_field* u[4] = {nullptr, nullptr, nullptr, nullptr};
-    lqx_field* t[4] = {nullptr, nullptr, nullptr, nullptr};
     int rc = LQX_OK;
     LQX_CUDA(ctx, cudaSetDevice(ctx->device));
+    // the eight work fields (links + ping-pong scratch) are kept in the context between calls: allocating and
+    // freeing 6 GB per call costs more than the transfers (and varies wildly); lqx_finalize releases them
+    if (ctx->host_work[0] && ctx->host_work[0]->prec != prec) {
+        for (int k = 0; k < 8; ++k) {
+            if (ctx->host_work[k]) lqx_field_free(ctx->host_work[k]);
+            ctx->host_work[k] = nullptr;
+        }
+    }
+    for (int k = 0; k < 8 && rc == LQX_OK; ++k)
+        if (!ctx->host_work[k]) rc = lqx_field_alloc(ctx, LQX_COLORMAT, prec, &ctx->host_work[k]);
+    if (rc != LQX_OK) return rc;
+    lqx_field* const* u = ctx->host_work;
+    lqx_field* const* t = ctx->host_work + 4;
     // all four uploads and conversions are enqueued back to back (no host round trip between them); the
     // smear kernels follow in stream order; the four downloads are enqueued likewise and ONE synchronisation
     // ends the call, after which the host buffers are no longer touched
-    for (int mu = 0; mu < 4 && rc == LQX_OK; ++mu) {
-        rc = lqx_field_alloc(ctx, LQX_COLORMAT, prec, &u[mu]);
-        if (rc == LQX_OK) rc = lqx_field_alloc(ctx, LQX_COLORMAT, prec, &t[mu]);
-        if (rc == LQX_OK) rc = lqx_push_impl(u[mu], host_u_in[mu], false);
-    }
+    for (int mu = 0; mu < 4 && rc == LQX_OK; ++mu) rc = lqx_push_impl(u[mu], host_u_in[mu], false);
     if (rc == LQX_OK) rc = lqx_smear_iterate(u, t, alpha, nsteps, plaq_avg_after_each);
     for (int mu = 0; mu < 4 && rc == LQX_OK; ++mu) rc = lqx_pop_impl(u[mu], host_u_out[mu], false);
     {
         cudaError_t e = cudaStreamSynchronize(ctx->stream);
         if (rc == LQX_OK && e != cudaSuccess) rc = lqx_cuda_fail(ctx, e, "smear_iterate_host sync");
-    }
-    for (int mu = 0; mu < 4; ++mu) {
-        if (u[mu]) lqx_field_free(u[mu]);
-        if (t[mu]) lqx_field_free(t[mu]);
     }
     return rc;
 }
