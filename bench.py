@@ -320,9 +320,9 @@ def _extras(torch, lqx, li, hbm_gbs):
         u, _ = _gen_links(lat, lqx, li, "c3", "haar", "f64")
         o = [lat.alloc(lqx.COLORMAT, lqx.F64) for _ in range(4)]
         v = lat.volume
-        add("smear_step c3", "f64", v, 144, SMEAR_CANONICAL_FLOPS, lambda: lqx.smear_step(o, u, ALPHA), reps=6)
+        add("smear_step c3", "f64", v, 144, SMEAR_CANONICAL_FLOPS, lambda: lqx.smear_step(o, u, ALPHA), reps=12)
         add("smear_step+plaquette(in) fused c3 (incl. sync)", "f64", v, 144, SMEAR_CANONICAL_FLOPS + 108,
-            lambda: lqx.smear_step(o, u, ALPHA, want_plaq_in=True), reps=6, lat=lat, kclass=lqx.K_SMEAR)
+            lambda: lqx.smear_step(o, u, ALPHA, want_plaq_in=True), reps=12, lat=lat, kclass=lqx.K_SMEAR)
         add("plaquette c3 (incl. sync)", "f64", v, 72, 2591, lambda: lqx.plaquette(u), reps=6, lat=lat, kclass=lqx.K_PLAQUETTE)
     # ---- C5: catalogue sweep, 32^3x64, both precisions
     dims = li.CONFIGS["c5"]["dims"]
