@@ -150,6 +150,46 @@ __device__ __forceinline__ Obj<9> jmul(const Obj<9>& a, const Obj<9>& b) {
         }
     return c;
 }
+// c + a*b with the products accumulated straight into c (what `x + m*y` compiles to)
+__device__ __forceinline__ Obj<9> jmac(const Obj<9>& c0, const Obj<9>& a, const Obj<9>& b) {
+    Obj<9> c;
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            T re = c0.re[3 * i + j], im = c0.im[3 * i + j];
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                re = fma(a.re[3 * i + k], b.re[3 * k + j], re);
+                im = fma(a.re[3 * i + k], b.im[3 * k + j], im);
+                re = fma(-a.im[3 * i + k], b.im[3 * k + j], re);
+                im = fma(a.im[3 * i + k], b.re[3 * k + j], im);
+            }
+            c.re[3 * i + j] = re;
+            c.im[3 * i + j] = im;
+        }
+    return c;
+}
+template <int NV>
+__device__ __forceinline__ Obj<3 * NV> jmacv(const Obj<3 * NV>& w0, const Obj<9>& m, const Obj<3 * NV>& v) {
+    Obj<3 * NV> w;
+#pragma unroll
+    for (int a = 0; a < NV; ++a)
+#pragma unroll
+        for (int i = 0; i < 3; ++i) {
+            T re = w0.re[3 * a + i], im = w0.im[3 * a + i];
+#pragma unroll
+            for (int j = 0; j < 3; ++j) {
+                re = fma(m.re[3 * i + j], v.re[3 * a + j], re);
+                im = fma(m.re[3 * i + j], v.im[3 * a + j], im);
+                re = fma(-m.im[3 * i + j], v.im[3 * a + j], re);
+                im = fma(m.im[3 * i + j], v.re[3 * a + j], im);
+            }
+            w.re[3 * a + i] = re;
+            w.im[3 * a + i] = im;
+        }
+    return w;
+}
 __device__ __forceinline__ Obj<1> jtrace(const Obj<9>& a) {
     Obj<1> c;
     c.re[0] = a.re[0] + a.re[4] + a.re[8];
@@ -231,19 +271,35 @@ struct Gen {
     std::ostringstream os;
     int tmp = 0, sites = 0;
     explicit Gen(const std::vector<XNode>& nodes) : n(nodes) {}
+    // shift(expr, dir, mu)(x) = expr(x + dir*mu^): the operand is evaluated at the neighbour site
+    Site shifted(const Site& site, const XNode& x) {
+        const std::string k = std::to_string(++sites), mu = std::to_string(x.b);
+        Site s2 = site;
+        s2.s = "s" + k;
+        s2.x[x.b] = "x" + k;
+        if (x.a > 0) os << "    const int x" << k << " = " << site.x[x.b] << " + 1 == g.L[" << mu << "] ? 0 : " << site.x[x.b] << " + 1;\n";
+        else os << "    const int x" << k << " = " << site.x[x.b] << " == 0 ? g.L[" << mu << "] - 1 : " << site.x[x.b] << " - 1;\n";
+        os << "    const int s" << k << " = " << site.s << " + (x" << k << " - " << site.x[x.b] << ") * g.st[" << mu << "];\n";
+        return s2;
+    }
+    // `other + m*y` (the product possibly under shifts) -> one multiply-accumulate into `other`
+    bool try_mac(int other, int prod, const Site& site, const std::string& v, const std::string& ty) {
+        Site ps = site;
+        int pi = prod;
+        // only peek: shifts are emitted after the decision
+        while (n[pi].op == LQX_X_SHIFT) pi = n[pi].child[0];
+        if (n[pi].op != LQX_X_MUL) return false;
+        const std::string l = val(other, site);
+        for (pi = prod; n[pi].op == LQX_X_SHIFT; pi = n[pi].child[0]) ps = shifted(ps, n[pi]);
+        const std::string a = val(n[pi].child[0], ps), b = val(n[pi].child[1], ps);
+        if (n[n[pi].child[1]].kind == LQX_COLORMAT) os << "    const " << ty << " " << v << " = jmac(" << l << ", " << a << ", " << b << ");\n";
+        else os << "    const " << ty << " " << v << " = jmacv<" << n[pi].kind / 3 << ">(" << l << ", " << a << ", " << b << ");\n";
+        return true;
+    }
     std::string val(int i, const Site& site) {
         const XNode& x = n[i];
         const std::string ty = "Obj<" + std::to_string(x.kind) + ">";
-        if (x.op == LQX_X_SHIFT) {  // shift(expr, dir, mu)(x) = expr(x + dir*mu^): evaluate the operand at the neighbour
-            const std::string k = std::to_string(++sites), mu = std::to_string(x.b);
-            Site s2 = site;
-            s2.s = "s" + k;
-            s2.x[x.b] = "x" + k;
-            if (x.a > 0) os << "    const int x" << k << " = " << site.x[x.b] << " + 1 == g.L[" << mu << "] ? 0 : " << site.x[x.b] << " + 1;\n";
-            else os << "    const int x" << k << " = " << site.x[x.b] << " == 0 ? g.L[" << mu << "] - 1 : " << site.x[x.b] << " - 1;\n";
-            os << "    const int s" << k << " = " << site.s << " + (x" << k << " - " << site.x[x.b] << ") * g.st[" << mu << "];\n";
-            return val(x.child[0], s2);
-        }
+        if (x.op == LQX_X_SHIFT) return val(x.child[0], shifted(site, x));
         std::string v = "v" + std::to_string(tmp++);
         switch (x.op) {
             case LQX_X_LEAF:
@@ -262,6 +318,7 @@ struct Gen {
             }
             case LQX_X_ADD:
             case LQX_X_SUB: {
+                if (x.op == LQX_X_ADD && (try_mac(x.child[0], x.child[1], site, v, ty) || try_mac(x.child[1], x.child[0], site, v, ty))) break;
                 std::string l = val(x.child[0], site), r = val(x.child[1], site);
                 os << "    const " << ty << " " << v << " = " << (x.op == LQX_X_ADD ? "jadd" : "jsub") << "(" << l << ", " << r << ");\n";
                 break;
