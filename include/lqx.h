@@ -76,6 +76,8 @@ int lqx_init(const int dims[4], int device, void* cuda_stream, lqx_ctx** out);
 /* Frees every field handle still alive, library-owned device memory and scratch
  * (the paper's theDeviceStorage::freeAll). */
 int lqx_finalize(lqx_ctx* ctx);
+/* Switch the stream later calls are enqueued on; synchronises the old stream first (the context's scratch
+ * buffers are ordered by its stream). */
 int lqx_set_stream(lqx_ctx* ctx, void* cuda_stream);
 int64_t lqx_volume(const lqx_ctx* ctx);       /* V = L0*L1*L2*L3, or negative status            */
 int64_t lqx_padded_volume(const lqx_ctx* ctx); /* V rounded up to whole 32-site blocks          */

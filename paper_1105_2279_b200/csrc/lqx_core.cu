@@ -140,6 +140,10 @@ extern "C" int lqx_finalize(lqx_ctx* ctx) {
 
 extern "C" int lqx_set_stream(lqx_ctx* ctx, void* cuda_stream) {
     if (!ctx) return LQX_EINVAL;
+    // the context's scratch (reduction partials, staging buffer, pinned results) is ordered by its stream:
+    // drain the old one before work is enqueued on the new one
+    LQX_CUDA(ctx, cudaSetDevice(ctx->device));
+    LQX_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     ctx->stream = (cudaStream_t)cuda_stream;
     return LQX_OK;
 }
