@@ -275,6 +275,13 @@ def _extras(torch, lqx, li, hbm_gbs):
         out[-1]["l2"] = "flushed between launches"
         add("hop c2 (L2-warm)", "f32", v, 120, 2280, lambda: lqx.hop(chi, u, psi), reps=20)
         out[-1]["l2"] = "warm: 63 MB working set fits the 126 MB L2"
+        def hop20():
+            for _ in range(20):
+                lqx.hop(chi, u, psi)
+
+        add("hop c2, 20 launches back to back (per 20; ramp-up and drain overlap as in the iterated Jacobi routine)", "f32", v * 20, 120, 2280,
+            hop20, reps=10)
+        out[-1]["l2"] = "warm: 63 MB working set fits the 126 MB L2"
         add("hop+norm2 fused c2 (L2-cold, incl. sync)", "f32", v, 120, 2328, lambda: lqx.hop_norm2(chi, u, psi), reps=20, cold=True,
             lat=lat, kclass=lqx.K_HOP)
     # ---- the same hop kernel on a lattice 16x larger (32^3x64: 1 GB moved), where launch ramp-up and
