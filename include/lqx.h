@@ -251,7 +251,8 @@ int lqx_kernel_time(lqx_ctx* ctx, int kernel_class, double* total_ms, int* count
 int64_t lqx_launch_count(const lqx_ctx* ctx);
 /* Options: "smear_variant" 0 or 3 = default (rolled literal kernel), 1 = first-cut literal kernel,
  * 2 = shared-corner kernel (36 products, lower staples exchanged through shared memory), 4 = four
- * threads per site; variants fall back to 3 where none of their tile shapes divides the lattice.
+ * threads per site, 6 = operands staged in shared memory with cp.async (fp32); variants fall back to 3 where
+ * none of their tile shapes divides the lattice.
  * "tile" -1 = automatic, 0 = linear 128-site blocks, 1..6 = CTA tile shape (8x4x4x2, 8x4x2x2,
  * 4x4x4x2, 16x4x2x2, 16x2x2x2, 32x2x2x2) of the nearest-neighbour kernels, used if it divides the
  * lattice.  "jacobi_block" (32, 64, 128, 256) and "jacobi_sites" (1, 2, 4): the paper's launch

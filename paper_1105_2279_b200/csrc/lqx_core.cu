@@ -120,6 +120,7 @@ extern "C" int lqx_finalize(lqx_ctx* ctx) {
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
     lqx_jit_release(ctx);
+    lqx_staged_release(ctx);
     for (lqx_field* f : ctx->fields) {
         if (f->owned && f->data) cudaFree(f->data);
         delete f;

@@ -85,7 +85,8 @@ struct lqx_field {
 int lqx_fail(lqx_ctx* ctx, int code, const char* what);
 int lqx_push_impl(lqx_field* f, const void* host, bool sync);  // lqx_core.cu; sync = false only enqueues
 int lqx_pop_impl(const lqx_field* f, void* host, bool sync);
-void lqx_jit_release(lqx_ctx* ctx);  // unloads the context's run-time compiled expression kernels (lqx_jit.cu)
+void lqx_jit_release(lqx_ctx* ctx);
+void lqx_staged_release(lqx_ctx* ctx);  // frees the staged smear kernel's tables (lqx_smear_staged.cu)  // unloads the context's run-time compiled expression kernels (lqx_jit.cu)
 int lqx_cuda_fail(lqx_ctx* ctx, cudaError_t e, const char* where);
 int lqx_ensure_partials(lqx_ctx* ctx, size_t ndoubles);
 // synchronises the stream and copies ctx->h_result[0..n) (written by a reduction kernel) to `out`

@@ -430,8 +430,14 @@ int smear_launch_t(lqx_ctx* ctx, lqx_field* const uout[4], const lqx_field* cons
     const Links<T> in = make_links<T>(uin);
     const T c0 = (T)(1.0 - alpha), c1 = (T)(alpha / 6.0);
     int variant = ctx->opt_smear_variant;
-    if (variant != 1 && variant != 2 && variant != 4) variant = 3;
+    if (variant != 1 && variant != 2 && variant != 4 && variant != 6) variant = 3;
     if (only_mu >= 0) variant = 1;
+    if (variant == 6) {
+        int rc = 1;
+        if (sizeof(T) == 4) rc = lqx_smear_staged_launch(ctx, reinterpret_cast<const Links<float>&>(in), reinterpret_cast<const LinksOut<float>&>(o), (float)c0, (float)c1, plaq);
+        if (rc <= 0) return rc;
+        variant = 3;  // fp64, or the lattice is not a multiple of the staged kernel's tile
+    }
     if (variant == 2) {
         // option "tile": 1 = 8x4x4x2 (256 threads), 2 = 8x4x2x2, 3 = 4x4x4x2, 4 = 16x4x2x2 (256), 5 = 16x2x2x2
         const int t = ctx->opt_tile;

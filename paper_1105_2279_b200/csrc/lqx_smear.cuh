@@ -52,3 +52,8 @@ static const int kSlabZ = 16;
 // plaquette sum of the INPUT field lands there (device or pinned host memory).
 int lqx_smear_launch(lqx_ctx* ctx, lqx_field* const uout[4], const lqx_field* const uin[4], double alpha, int only_mu,
                      double* plaq);
+
+// shared-memory-staged smear step for fp32 (lqx_smear_staged.cu): LQX_OK, a negative status, or 1 if the
+// lattice is not a multiple of its 8x2x2x2 tile
+int lqx_smear_staged_launch(lqx_ctx* ctx, const Links<float>& in, const LinksOut<float>& out, float c0, float c1, double* plaq);
+void lqx_staged_release(lqx_ctx* ctx);
