@@ -2,6 +2,9 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c4|c3] [--no-extras]
     python bench.py --impl reference ...        # the CPU oracle on a bounded sample of the same workload
+    python bench.py --kernel-only               # timed device region only: the command ncu wraps for the smear kernel
+    python bench.py --extras-only               # per-kernel rows of configs 1, 2, 3, 5, Jacobi routine, run-time expressions
+    python bench.py --sweep-geometry            # P(N_threads, N_site) of the Jacobi step (the paper's Figs. 1-2)
 
 One "step" = one pass of the whole hot path over the link field: a fused staple-sum smearing step
 (alpha = 0.5, all four directions, plaquette of its input accumulated in the same pass) -- K steps
