@@ -553,6 +553,30 @@ def test_full_size_c4_ten_steps_properties(lqx):
         assert plaqs2 == plaqs and lqx.norm2(keep[2]) == n_a
 
 
+def test_full_size_c4_trajectory_against_oracle(lqx):
+    """configs[3] at full size against the truth trajectory (reading A23): three iterated steps, the plaquette
+    average after each, and the links after the last step on sampled sites.  The oracle smears the whole
+    48^3x96 lattice on the host cores (a few seconds per step)."""
+    import torch
+
+    cfg = li.CONFIGS["c4"]
+    dims = cfg["dims"]
+    nsteps = 3
+    with lqx.Lattice(dims) as lat:
+        fu, hu = _full_size_links(lqx, lat, "c4", "near_unit", "f32")
+        tmp = [lat.alloc(lqx.COLORMAT, lqx.F32) for _ in range(4)]
+        plaqs = lqx.smear_iterate(fu, tmp, 0.5, nsteps)
+        want_u, want_p = orc.smear_iterate(dims, hu, 0.5, nsteps, "f32")
+        for k in range(nsteps):
+            assert abs(plaqs[k] - want_p[k]) < RTOL["f32"], k
+        sites = _sample_sites(dims, 3000, 23)
+        idx = torch.from_numpy(sites).cuda()
+        buf = torch.empty((lat.volume, 3, 3, 2), dtype=torch.float32, device="cuda")
+        for mu in range(4):
+            fu[mu].export_dev(buf)
+            assert site_rel_err(buf[idx].cpu().numpy(), want_u[mu][sites]) < TOL["f32"] * nsteps, mu
+
+
 @pytest.mark.parametrize("prec", ["f32", "f64"])
 def test_full_size_c5_expression_sweep(lqx, prec):
     """configs[4]: 32^3x64, the four forms each followed by its reduction, against the truth oracle."""
