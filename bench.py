@@ -229,6 +229,31 @@ def _time_kernel(torch, fn, reps, flush=None):
     return times[len(times) // 2], times[0]
 
 
+def jacobi_listing(lqx, chi, u, kappa, iters, no_smear_dir, norm, work, fused):
+    """The paper's Listing 1 as USER code on top of the run-time expression path, the way a
+    QDP++ program would state it.  fused = False: literally the listing, one expression per line -- E0 copies,
+    E1 for the first direction, E2 ('+=') for the others, E3, E4 (six kernels per iteration).  fused = True:
+    one expression per iteration, chi' = s_0 + kappa * sum_mu (...).  work = (s_0, psi, h_smear) scratch fields."""
+    s0, psi, h = work
+    L = lqx.Expr.leaf
+    lqx.expr_eval(s0, L(chi))                                             # s_0 = chi
+    for _ in range(iters):
+        lqx.expr_eval(psi, L(chi))                                        # psi = chi
+        terms = [L(u[mu]) * lqx.shifted(psi, lqx.FORWARD, mu) + lqx.shifted(lqx.adj(u[mu]) * L(psi), lqx.BACKWARD, mu)
+                 for mu in range(4) if mu != no_smear_dir]
+        if fused:
+            e = terms[0]
+            for t in terms[1:]:
+                e = e + t
+            lqx.expr_eval(chi, L(s0) + kappa * e)                         # E1..E3 in one kernel
+        else:
+            lqx.expr_eval(h, terms[0])                                    # h_smear  = ...   (E1)
+            for t in terms[1:]:
+                lqx.expr_eval(h, t, accumulate=True)                      # h_smear += ...   (E2)
+            lqx.expr_eval(chi, L(s0) + kappa * L(h))                      # chi = s_0 + kappa*h_smear (E3)
+    lqx.expr_eval(chi, (1.0 / norm) * L(chi))                             # chi /= norm (E4; reciprocal multiply, A22)
+
+
 def _extras(torch, lqx, li, hbm_gbs):
     """Per-kernel numbers for the other BASELINE configs (same JSON line, key "kernels"): device time
     per launch, algorithmic GB/s (SURVEY 8(d) bytes/site) and its fraction of the measured HBM peak."""
@@ -324,6 +349,13 @@ def _extras(torch, lqx, li, hbm_gbs):
                     144, 2328, lambda: lqx.jacobi_smear(chi, u, 0.01, JIT, -1, 1.0, tmp), reps=10)
                 out[-1]["l2"] = "iterated on resident fields (working set %.0f MB)" % (lat.volume * 168 * (4 if prec == "f32" else 8) / 1e6)
                 out[-1]["paper_gflops_gtx480"] = {(16, "f32"): 11.86, (16, "f64"): 6.26, (32, "f32"): 21.31}.get((dims[0], prec))
+                if dims[0] == 32:  # the same routine as user code on the run-time expression path (NEXT-2)
+                    work = [lat.alloc(lqx.FERMION, pcode) for _ in range(3)]
+                    for fused, label in ((True, "one run-time expression per iteration"), (False, "Listing 1 literally: E0..E4 as six run-time expressions per iteration")):
+                        jacobi_listing(lqx, chi, u, 0.01, 1, -1, 1.0, work, fused)  # compiles the kernels
+                        add(f"jacobi_smear {dims[0]}^3x{dims[3]} x{JIT} iterations, {label}", prec, lat.volume * JIT, 144, 2328,
+                            lambda: jacobi_listing(lqx, chi, u, 0.01, JIT, -1, 1.0, work, fused), reps=5)
+                        out[-1]["l2"] = "fused: 144 reals per site and iteration; literal listing: 24+24 (E0) + 66+3*90 (E1,E2) + 72 (E3) = 456"
     # ---- C3: smear + plaquette, 32^3x64 fp64
     dims = li.CONFIGS["c3"]["dims"]
     with lqx.Lattice(dims) as lat:

@@ -740,3 +740,27 @@ def test_expr_trace_and_reductions(lqx, dims, prec):
             lqx.expr_eval(cx, L(fv).trace())
         with pytest.raises(lqx.LqxError):
             lqx.expr_reduce(9, e1)
+
+
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+@pytest.mark.parametrize("fused", [True, False])
+def test_jacobi_listing_through_runtime_expressions(lqx, prec, fused):
+    """The paper's Listing 1 written as user code on the run-time expression path (bench.jacobi_listing), literally
+    (E0..E4) and fused, against the oracle's routine and the hand-written lqx_jacobi_smear."""
+    import bench
+
+    dims = DIMS_RAGGED
+    u = _links(2, dims, prec)
+    chi0 = _gauss(2, 10, dims, "f", prec)
+    kappa, iters, skip, norm = 0.21, 4, 3, 1.7
+    with lqx.Lattice(dims) as lat:
+        fu = [lat.from_host(t) for t in u]
+        chi = lat.from_host(chi0)
+        work = [lat.alloc(chi.kind, chi.prec) for _ in range(3)]
+        bench.jacobi_listing(lqx, chi, fu, kappa, iters, skip, norm, work, fused)
+        want = orc.jacobi_smear(dims, u, chi0, kappa, iters, skip, norm, orc.truth_variant(prec))
+        got = chi.pop()
+        assert site_rel_err(got, want) < TOL[prec] * iters
+        ref = lat.from_host(chi0)
+        lqx.jacobi_smear(ref, fu, kappa, iters, skip, norm, work[:2])
+        assert site_rel_err(got, ref.pop()) < TOL[prec] * iters
