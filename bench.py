@@ -551,7 +551,7 @@ def run_ours(args):
         fbytes = V * 18 * esize * 4
         line["e2e"] = {"value": V * ke / te, "unit": "site-updates/s", "h2d_bytes_per_step": fbytes,
                        "d2h_bytes_per_step": fbytes + 8, "steps": ke, "ms_per_step": te / ke * 1e3,
-                       "call": "lqx_smear_iterate_host(nsteps=1) on pinned host buffers in QDP order"}
+                       "call": "lqx_smear_iterate_host(nsteps=1) on pinned host buffers in QDP order (time-slice slabs streamed: upload / step / download overlap)"}
         # ---- cpu baseline: the oracle on this box's host cores
         import oracle as orc
 

@@ -227,7 +227,12 @@ int lqx_smear_step(lqx_field* const uout[4], const lqx_field* const uin[4], doub
 int lqx_smear_iterate(lqx_field* const u[4], lqx_field* const tmp[4], double alpha, int nsteps,
                       double* plaq_avg_after_each);
 /* End-to-end form with HOST buffers (bench `e2e`): host_u_in[4] / host_u_out[4] are host colour
- * matrix fields in QDP order of precision `prec`; pushes, iterates, pops. */
+ * matrix fields in QDP order of precision `prec` (host_u_out[mu] may be host_u_in[mu]); pushes,
+ * iterates, pops; the host buffers are not touched after the call returns.  Work fields stay cached
+ * in the context until lqx_finalize.  A single step (nsteps == 1) is streamed: the lattice is cut
+ * into slabs of time slices whose upload, update and download overlap on three streams (page-locked
+ * host buffers are needed for the copies to overlap; pageable ones work, serially); the result is
+ * bit-identical to the serial path.  Option "host_slabs": -1 automatic, 0 serial, n at most n slabs. */
 int lqx_smear_iterate_host(lqx_ctx* ctx, lqx_prec prec, const void* const host_u_in[4],
                            void* const host_u_out[4], double alpha, int nsteps,
                            double* plaq_avg_after_each);
@@ -257,6 +262,7 @@ int64_t lqx_launch_count(const lqx_ctx* ctx);
  * 4x4x4x2, 16x4x2x2, 16x2x2x2, 32x2x2x2) of the nearest-neighbour kernels, used if it divides the
  * lattice.  "jacobi_block" (32, 64, 128, 256) and "jacobi_sites" (1, 2, 4): the paper's launch
  * geometry parameters N_threads and N_site for lqx_jacobi_smear; 0 = tuned default.
+ * "host_slabs": see lqx_smear_iterate_host.
  * "time_kernels" 0/1 (see above).  All variants agree within rounding; DESIGN.md sec.6. */
 int lqx_set_option(lqx_ctx* ctx, const char* key, int value);
 

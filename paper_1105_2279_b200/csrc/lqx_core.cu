@@ -99,7 +99,9 @@ extern "C" int lqx_init(const int dims[4], int device, void* cuda_stream, lqx_ct
     c->num_sms = prop.multiProcessorCount;
     c->d_ticket = nullptr;
     c->stage = nullptr;
-    for (int k = 0; k < 8; ++k) c->host_work[k] = nullptr;
+    for (int k = 0; k < 12; ++k) c->host_work[k] = nullptr;
+    c->pipe_stream[0] = c->pipe_stream[1] = nullptr;
+    c->opt_host_slabs = -1;
     c->stage_cap = 0;
     if (cudaMalloc(&c->d_result, 64 * sizeof(double)) != cudaSuccess ||
         cudaMalloc(&c->d_ticket, sizeof(unsigned int)) != cudaSuccess ||
@@ -130,6 +132,9 @@ extern "C" int lqx_finalize(lqx_ctx* ctx) {
             cudaEventDestroy(pr.first);
             cudaEventDestroy(pr.second);
         }
+    for (cudaEvent_t e : ctx->pipe_events) cudaEventDestroy(e);
+    for (int k = 0; k < 2; ++k)
+        if (ctx->pipe_stream[k]) cudaStreamDestroy(ctx->pipe_stream[k]);
     if (ctx->d_partials) cudaFree(ctx->d_partials);
     if (ctx->stage) cudaFree(ctx->stage);
     if (ctx->d_result) cudaFree(ctx->d_result);
@@ -175,6 +180,7 @@ extern "C" int lqx_set_option(lqx_ctx* ctx, const char* key, int value) {
     else if (!strcmp(key, "jacobi_block")) ctx->opt_jacobi_block = value;
     else if (!strcmp(key, "jacobi_sites")) ctx->opt_jacobi_sites = value;
     else if (!strcmp(key, "time_kernels")) ctx->timing = value != 0;
+    else if (!strcmp(key, "host_slabs")) ctx->opt_host_slabs = value;
     else return lqx_fail(ctx, LQX_EINVAL, "unknown option");
     return LQX_OK;
 }
@@ -295,11 +301,11 @@ extern "C" int lqx_field_prec(const lqx_field* f) { return f ? (int)f->prec : LQ
 // the same 32*nreal contiguous reals, so the conversion is a permutation staged through shared
 // memory with coalesced reads and writes on both sides.
 template <typename T, bool TO_SOA>
-__global__ void k_transpose(int V, int nreal, const T* __restrict__ src, T* __restrict__ dst) {
+__global__ void k_transpose(int V, int nreal, int blk0, const T* __restrict__ src, T* __restrict__ dst) {
     extern __shared__ unsigned char smem_raw[];
     T* tile = reinterpret_cast<T*>(smem_raw);  // [32][nreal+1], QDP order
     constexpr int W = 16 / (int)sizeof(T);
-    const int s0 = blockIdx.x * 32;
+    const int s0 = (blk0 + blockIdx.x) * 32;
     const int ns = min(32, V - s0);
     const int pitch = nreal + 1;
     const int nfull = nreal / W, rem = nreal - nfull * W;
@@ -337,16 +343,20 @@ __global__ void k_transpose(int V, int nreal, const T* __restrict__ src, T* __re
 }
 
 static int transpose_launch(lqx_ctx* ctx, const lqx_field* f, const void* src, void* dst, bool to_soa) {
+    return lqx_transpose_range(ctx, f->kind, f->prec, src, dst, to_soa, 0, (ctx->geo.V + 31) / 32, ctx->stream);
+}
+
+int lqx_transpose_range(lqx_ctx* ctx, lqx_kind kind, lqx_prec prec, const void* src, void* dst, bool to_soa, int blk0,
+                        int nblk, cudaStream_t stream) {
     const Geo& g = ctx->geo;
-    const int nreal = 2 * (int)f->kind;
-    const int nblk = (g.V + 31) / 32;
-    const size_t sm = (size_t)32 * (nreal + 1) * (int)f->prec;
-    if (f->prec == LQX_F32) {
-        if (to_soa) k_transpose<float, true><<<nblk, 256, sm, ctx->stream>>>(g.V, nreal, (const float*)src, (float*)dst);
-        else k_transpose<float, false><<<nblk, 256, sm, ctx->stream>>>(g.V, nreal, (const float*)src, (float*)dst);
+    const int nreal = 2 * (int)kind;
+    const size_t sm = (size_t)32 * (nreal + 1) * (int)prec;
+    if (prec == LQX_F32) {
+        if (to_soa) k_transpose<float, true><<<nblk, 256, sm, stream>>>(g.V, nreal, blk0, (const float*)src, (float*)dst);
+        else k_transpose<float, false><<<nblk, 256, sm, stream>>>(g.V, nreal, blk0, (const float*)src, (float*)dst);
     } else {
-        if (to_soa) k_transpose<double, true><<<nblk, 256, sm, ctx->stream>>>(g.V, nreal, (const double*)src, (double*)dst);
-        else k_transpose<double, false><<<nblk, 256, sm, ctx->stream>>>(g.V, nreal, (const double*)src, (double*)dst);
+        if (to_soa) k_transpose<double, true><<<nblk, 256, sm, stream>>>(g.V, nreal, blk0, (const double*)src, (double*)dst);
+        else k_transpose<double, false><<<nblk, 256, sm, stream>>>(g.V, nreal, blk0, (const double*)src, (double*)dst);
     }
     LQX_LAUNCH_CHECK(ctx);
     return LQX_OK;

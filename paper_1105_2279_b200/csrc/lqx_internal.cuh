@@ -40,7 +40,11 @@ struct lqx_ctx {
     size_t partials_cap; // in doubles
     double* d_result;    // 64 doubles (device scratch results)
     double* h_result;    // pinned + mapped, 64 doubles: kernels write results straight to the host
-    lqx_field* host_work[8];  // work fields of lqx_smear_iterate_host, kept between calls
+    lqx_field* host_work[12];  // work fields of lqx_smear_iterate_host, kept between calls: links, ping-pong
+                               // scratch, and (streamed one-step path) four QDP-order staging fields
+    cudaStream_t pipe_stream[2];          // upload and download streams of the streamed host path (lazy)
+    std::vector<cudaEvent_t> pipe_events; // its per-slab events (lazy, no timing)
+    int opt_host_slabs;                   // -1 = automatic, 0 = off (serial push / step / pop), n = at most n slabs
     void* stage;       // device staging buffer of push/pop (one field in QDP order), grow-only
     size_t stage_cap;
     unsigned int* d_ticket;  // last-block ticket of the one-launch reductions (zero between launches)
@@ -85,6 +89,9 @@ struct lqx_field {
 int lqx_fail(lqx_ctx* ctx, int code, const char* what);
 int lqx_push_impl(lqx_field* f, const void* host, bool sync);  // lqx_core.cu; sync = false only enqueues
 int lqx_pop_impl(const lqx_field* f, void* host, bool sync);
+// QDP order <-> blocked layout for the 32-site blocks [blk0, blk0 + nblk) of a field, on `stream` (lqx_core.cu)
+int lqx_transpose_range(lqx_ctx* ctx, lqx_kind kind, lqx_prec prec, const void* src, void* dst, bool to_soa, int blk0,
+                        int nblk, cudaStream_t stream);
 void lqx_jit_release(lqx_ctx* ctx);
 void lqx_staged_release(lqx_ctx* ctx);  // frees the staged smear kernel's tables (lqx_smear_staged.cu)  // unloads the context's run-time compiled expression kernels (lqx_jit.cu)
 int lqx_cuda_fail(lqx_ctx* ctx, cudaError_t e, const char* where);
@@ -619,8 +626,10 @@ int lqx_sum_partials(lqx_ctx* ctx, int nblocks, int ncomp, double* out);
 // Linear: generic fallback for extents no tile shape divides: 128 consecutive lexicographic sites.
 // --------------------------------------------------------------------------------------------
 struct TileMap {
-    int nt[4];  // tiles per direction
-    int zs;     // z-tiles per slab
+    int nt[4];   // tiles per direction (nt[3]: t-tiles this launch covers)
+    int zs;      // z-tiles per slab
+    int toff;    // first t-tile of the launch (a launch may cover a range of time slices, see restrict_t)
+    int s0, s1;  // Linear: site range of the launch
 };
 
 template <int TX, int TY, int TZ, int TT>
@@ -645,12 +654,19 @@ struct Tiled {
         x[0] = tx * TX + (l % TX);
         x[1] = ty * TY + (l / TX) % TY;
         x[2] = (tz + k * m.zs) * TZ + (l / (TX * TY)) % TZ;
-        x[3] = tt * TT + l / (TX * TY * TZ);
+        x[3] = (tt + m.toff) * TT + l / (TX * TY * TZ);
         s = x[0] + g.L[0] * (x[1] + g.L[1] * (x[2] + g.L[2] * x[3]));
         return true;
     }
     static bool fits(const Geo& g) { return g.L[0] % TX == 0 && g.L[1] % TY == 0 && g.L[2] % TZ == 0 && g.L[3] % TT == 0; }
     static int grid(const Geo& g) { return (g.L[0] / TX) * (g.L[1] / TY) * (g.L[2] / TZ) * (g.L[3] / TT); }
+    // restrict the launch to the time slices [t0, t1) (both multiples of TT); returns its grid size
+    static int restrict_t(const Geo&, TileMap& m, int t0, int t1) {
+        m.toff = t0 / TT;
+        m.nt[3] = (t1 - t0) / TT;
+        return m.nt[0] * m.nt[1] * m.nt[2] * m.nt[3];
+    }
+    static bool splits_t(int t) { return t % TT == 0; }
     static TileMap map(const Geo& g, int slab_sites_z) {
         TileMap m;
         m.nt[0] = g.L[0] / TX;
@@ -658,22 +674,32 @@ struct Tiled {
         m.nt[2] = g.L[2] / TZ;
         m.nt[3] = g.L[3] / TT;
         m.zs = std::max(1, std::min(m.nt[2], slab_sites_z / TZ));
+        m.toff = 0;
+        m.s0 = 0;
+        m.s1 = g.V;
         return m;
     }
 };
 
 struct Linear {
     static constexpr int THREADS = 128;
-    __device__ static __forceinline__ bool site(const Geo& g, const TileMap&, int x[4], int& s) {
-        s = blockIdx.x * THREADS + threadIdx.x;
-        if (s >= g.V) return false;
+    __device__ static __forceinline__ bool site(const Geo& g, const TileMap& m, int x[4], int& s) {
+        s = m.s0 + blockIdx.x * THREADS + threadIdx.x;
+        if (s >= m.s1) return false;
         site_coords(g, s, x);
         return true;
     }
     static bool fits(const Geo&) { return true; }
     static int grid(const Geo& g) { return (g.V + THREADS - 1) / THREADS; }
-    static TileMap map(const Geo&, int) {
-        TileMap m = {{0, 0, 0, 0}, 1};
+    static TileMap map(const Geo& g, int) {
+        TileMap m = {{0, 0, 0, 0}, 1, 0, 0, g.V};
         return m;
     }
+    static int restrict_t(const Geo& g, TileMap& m, int t0, int t1) {
+        const int v3 = g.L[0] * g.L[1] * g.L[2];
+        m.s0 = t0 * v3;
+        m.s1 = t1 * v3;
+        return (m.s1 - m.s0 + THREADS - 1) / THREADS;
+    }
+    static bool splits_t(int) { return true; }
 };

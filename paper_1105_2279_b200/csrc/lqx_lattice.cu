@@ -366,18 +366,126 @@ extern "C" int lqx_smear_iterate(lqx_field* const u[4], lqx_field* const tmp[4],
     return rc;
 }
 
+// Streamed one-step host path: the lattice is cut into slabs of time slices; slab k is uploaded (and converted to the
+// blocked layout on the context's stream) on an upload stream, smeared on the context's stream as soon as its two
+// neighbour slabs are in, converted back and downloaded on a download stream -- so the PCIe link carries both directions at once and the
+// kernels hide under the copies.  A slab is a contiguous site range in QDP order and in the blocked layout alike
+// (t is the slowest index), provided its volume is a multiple of the 32-site block.
+// Returns the slab thickness (time slices) to use, or 0 if this lattice / option setting does not stream.
+static int host_slab_thickness(const lqx_ctx* ctx, lqx_prec prec) {
+    const Geo& g = ctx->geo;
+    if (ctx->opt_host_slabs == 0) return 0;
+    if (ctx->opt_smear_variant != 0 && ctx->opt_smear_variant != 3) return 0;  // only the default kernel takes a t-range
+    // automatic: at most 48 slabs (the three slabs left after the last upload are the un-overlapped tail: 48 slabs at
+    // configs[3] measured 68-71 ms per call, 24: 72-75, 12: 76-78, serial: 119) of at least 4 MB per link, below
+    // which the per-slab launches and copies cost more than the overlap gains; option "host_slabs" = n > 0 forces
+    // up to n slabs whatever their size
+    const bool forced = ctx->opt_host_slabs > 0;
+    const int max_slabs = forced ? ctx->opt_host_slabs : 48;
+    const int64_t min_bytes = forced ? 0 : (int64_t)4 << 20;
+    const int64_t v3 = (int64_t)g.L[0] * g.L[1] * g.L[2];
+    for (int th = 2; th * 3 <= g.L[3]; th += 2) {  // even: every tile shape has a t-extent of 1 or 2
+        if (g.L[3] % th || (v3 * th) % 32) continue;
+        if (g.L[3] / th <= max_slabs && v3 * th * 18 * (int)prec >= min_bytes) return th;
+    }
+    return 0;
+}
+
+static int smear_host_streamed(lqx_ctx* ctx, lqx_prec prec, const void* const host_u_in[4], void* const host_u_out[4],
+                               double alpha, int th, double* plaq_avg) {
+    const Geo& g = ctx->geo;
+    const int K = g.L[3] / th;
+    int rc = LQX_OK;
+    for (int k = 8; k < 12 && rc == LQX_OK; ++k)
+        if (!ctx->host_work[k]) rc = lqx_field_alloc(ctx, LQX_COLORMAT, prec, &ctx->host_work[k]);
+    if (rc != LQX_OK) return rc;
+    for (int k = 0; k < 2; ++k)
+        if (!ctx->pipe_stream[k]) LQX_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->pipe_stream[k], cudaStreamNonBlocking));
+    while ((int)ctx->pipe_events.size() < 2 * K + 2) {
+        cudaEvent_t e;
+        LQX_CUDA(ctx, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        ctx->pipe_events.push_back(e);
+    }
+    lqx_field* const* u = ctx->host_work;       // input links, blocked layout
+    lqx_field* const* t = ctx->host_work + 4;   // smeared links, blocked layout
+    lqx_field* const* q = ctx->host_work + 8;   // QDP-order staging: slab k holds the input until it is converted,
+                                                // then the output from its conversion until it is downloaded
+    cudaStream_t up = ctx->pipe_stream[0], down = ctx->pipe_stream[1], main = ctx->stream;
+    cudaEvent_t* ev_in = ctx->pipe_events.data();        // [K]  slab uploaded
+    cudaEvent_t* ev_out = ctx->pipe_events.data() + K;   // [K]  slab smeared and converted back
+    cudaEvent_t ev_begin = ctx->pipe_events[2 * K], ev_end = ctx->pipe_events[2 * K + 1];
+    const size_t slab_sites = (size_t)g.L[0] * g.L[1] * g.L[2] * th;
+    const size_t slab_bytes = slab_sites * 18 * (int)prec;
+    const int slab_blocks = (int)(slab_sites / 32);
+    // a failing runtime call records the error in rc and the remaining steps are skipped; the join below still runs
+#define PIPE_TRY(call)                                                                       \
+    do {                                                                                     \
+        if (rc == LQX_OK) {                                                                  \
+            cudaError_t e__ = (call);                                                        \
+            if (e__ != cudaSuccess) rc = lqx_cuda_fail(ctx, e__, #call);                     \
+        }                                                                                    \
+    } while (0)
+    // everything enqueued earlier on the context's stream comes first
+    PIPE_TRY(cudaEventRecord(ev_begin, main));
+    PIPE_TRY(cudaStreamWaitEvent(up, ev_begin, 0));
+    PIPE_TRY(cudaStreamWaitEvent(down, ev_begin, 0));
+    auto smear_slab = [&](int j) -> int {
+        int r = lqx_smear_launch_range(ctx, t, (const lqx_field* const*)u, alpha, j * th, (j + 1) * th);
+        if (r > 0) r = lqx_fail(ctx, LQX_EGEOM, "smear_iterate_host: tile does not split at the slab boundary");
+        for (int mu = 0; mu < 4 && r == LQX_OK; ++mu)
+            r = lqx_transpose_range(ctx, LQX_COLORMAT, prec, t[mu]->data, q[mu]->data, false, j * slab_blocks, slab_blocks, main);
+        if (r != LQX_OK) return r;
+        PIPE_TRY(cudaEventRecord(ev_out[j], main));
+        PIPE_TRY(cudaStreamWaitEvent(down, ev_out[j], 0));
+        for (int mu = 0; mu < 4 && rc == LQX_OK; ++mu)
+            PIPE_TRY(cudaMemcpyAsync((char*)host_u_out[mu] + (size_t)j * slab_bytes, (const char*)q[mu]->data + (size_t)j * slab_bytes,
+                                          slab_bytes, cudaMemcpyDeviceToHost, down));
+        return rc;
+    };
+    for (int k = 0; k < K && rc == LQX_OK; ++k) {
+        for (int mu = 0; mu < 4 && rc == LQX_OK; ++mu)
+            PIPE_TRY(cudaMemcpyAsync((char*)q[mu]->data + (size_t)k * slab_bytes, (const char*)host_u_in[mu] + (size_t)k * slab_bytes,
+                                          slab_bytes, cudaMemcpyHostToDevice, up));
+        // the side streams carry copies only, so neither copy engine ever waits for a kernel
+        PIPE_TRY(cudaEventRecord(ev_in[k], up));
+        PIPE_TRY(cudaStreamWaitEvent(main, ev_in[k], 0));
+        for (int mu = 0; mu < 4 && rc == LQX_OK; ++mu)
+            rc = lqx_transpose_range(ctx, LQX_COLORMAT, prec, q[mu]->data, u[mu]->data, true, k * slab_blocks, slab_blocks, main);
+        if (rc != LQX_OK) break;
+        // slab k-1 has both neighbours now (slabs 0 and K-1 wait for the wrap-around, below)
+        if (k >= 2) rc = smear_slab(k - 1);
+    }
+    if (rc == LQX_OK) rc = smear_slab(K - 1);
+    if (rc == LQX_OK) rc = smear_slab(0);
+    if (rc == LQX_OK && plaq_avg)
+        rc = prec == LQX_F32 ? plaquette_launch<float>(ctx, (const lqx_field* const*)t, ctx->h_result)
+                             : plaquette_launch<double>(ctx, (const lqx_field* const*)t, ctx->h_result);
+#undef PIPE_TRY
+    // join the side streams into the context's stream even on failure, so nothing is left in flight
+    cudaEventRecord(ev_end, down);
+    cudaStreamWaitEvent(main, ev_end, 0);
+    cudaEventRecord(ev_end, up);
+    cudaStreamWaitEvent(main, ev_end, 0);
+    cudaError_t e = cudaStreamSynchronize(main);
+    if (rc == LQX_OK && e != cudaSuccess) rc = lqx_cuda_fail(ctx, e, "smear_iterate_host sync");
+    if (rc == LQX_OK && plaq_avg) plaq_avg[0] = ctx->h_result[0] / (18.0 * (double)g.V);
+    return rc;
+}
+
 extern "C" int lqx_smear_iterate_host(lqx_ctx* ctx, lqx_prec prec, const void* const host_u_in[4],
                                       void* const host_u_out[4], double alpha, int nsteps,
                                       double* plaq_avg_after_each) {
     if (!ctx || !host_u_in || !host_u_out) return LQX_EINVAL;
     for (int mu = 0; mu < 4; ++mu)
         if (!host_u_in[mu] || !host_u_out[mu]) return LQX_EINVAL;
+    if (prec != LQX_F32 && prec != LQX_F64) return LQX_EINVAL;
     int rc = LQX_OK;
     LQX_CUDA(ctx, cudaSetDevice(ctx->device));
-    // the eight work fields (links + ping-pong scratch) are kept in the context between calls: allocating and
+    // the work fields (links + ping-pong scratch + staging) are kept in the context between calls: allocating and
     // freeing 6 GB per call costs more than the transfers (and varies wildly); lqx_finalize releases them
     if (ctx->host_work[0] && ctx->host_work[0]->prec != prec) {
-        for (int k = 0; k < 8; ++k) {
+        LQX_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+        for (int k = 0; k < 12; ++k) {
             if (ctx->host_work[k]) lqx_field_free(ctx->host_work[k]);
             ctx->host_work[k] = nullptr;
         }
@@ -385,6 +493,10 @@ extern "C" int lqx_smear_iterate_host(lqx_ctx* ctx, lqx_prec prec, const void* c
     for (int k = 0; k < 8 && rc == LQX_OK; ++k)
         if (!ctx->host_work[k]) rc = lqx_field_alloc(ctx, LQX_COLORMAT, prec, &ctx->host_work[k]);
     if (rc != LQX_OK) return rc;
+    if (nsteps == 1) {
+        const int th = host_slab_thickness(ctx, prec);
+        if (th > 0) return smear_host_streamed(ctx, prec, host_u_in, host_u_out, alpha, th, plaq_avg_after_each);
+    }
     lqx_field* const* u = ctx->host_work;
     lqx_field* const* t = ctx->host_work + 4;
     // all four uploads and conversions are enqueued back to back (no host round trip between them); the

@@ -490,7 +490,34 @@ int smear_launch_t(lqx_ctx* ctx, lqx_field* const uout[4], const lqx_field* cons
     return plaq ? lqx_sum_partials(ctx, nblocks, 1, plaq) : LQX_OK;
 }
 
+// one smear step restricted to the time slices [t0, t1): the rolled kernel on a sub-grid (streamed host path)
+template <typename T>
+int smear_range_t(lqx_ctx* ctx, lqx_field* const uout[4], const lqx_field* const uin[4], double alpha, int t0, int t1) {
+    const Geo& g = ctx->geo;
+    LinksOut<T> o;
+    for (int mu = 0; mu < 4; ++mu) o.u[mu] = (T*)uout[mu]->data;
+    const Links<T> in = make_links<T>(uin);
+    const T c0 = (T)(1.0 - alpha), c1 = (T)(alpha / 6.0);
+    const int choice = lqx_pick_tile(ctx, sizeof(T) == 4 ? 1 : 0);
+    LQX_WITH_MAP(choice, {
+        if (!MAP::splits_t(t0) || !MAP::splits_t(t1)) return 1;
+        TileMap tm = MAP::map(g, kSlabZ);
+        const int grid = MAP::restrict_t(g, tm, t0, t1);
+        constexpr int MB = sizeof(T) == 4 ? (MAP::THREADS >= 256 ? 3 : 6) : (MAP::THREADS >= 256 ? 1 : 3);
+        LqxTimed timed(ctx, LQX_K_SMEAR);
+        k_smear_rolled<T, false, MAP, MB><<<grid, MAP::THREADS, 0, ctx->stream>>>(g, tm, in, o, c0, c1, nullptr, nullptr, nullptr);
+    })
+    LQX_LAUNCH_CHECK(ctx);
+    return LQX_OK;
+}
+
 }  // namespace
+
+int lqx_smear_launch_range(lqx_ctx* ctx, lqx_field* const uout[4], const lqx_field* const uin[4], double alpha, int t0,
+                           int t1) {
+    return uin[0]->prec == LQX_F32 ? smear_range_t<float>(ctx, uout, uin, alpha, t0, t1)
+                                   : smear_range_t<double>(ctx, uout, uin, alpha, t0, t1);
+}
 
 int lqx_smear_launch(lqx_ctx* ctx, lqx_field* const uout[4], const lqx_field* const uin[4], double alpha, int only_mu,
                      double* plaq) {

@@ -378,6 +378,74 @@ def test_smear_iterate_host_end_to_end(lqx):
         assert site_rel_err(out[mu], want_u[mu]) < 2 * TOL["f32"]
 
 
+# The one-step host call streams the lattice through the GPU in slabs of time slices (upload, smear and download of
+# different slabs overlap).  It must give exactly what the serial push / step / pop path gives -- same kernel, same
+# per-site arithmetic -- on every tile map, including the wrap-around slabs, and agree with the oracle.
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+@pytest.mark.parametrize("dims,slabs", [((8, 8, 8, 16), 48), ((8, 8, 8, 16), 4), ((4, 4, 4, 8), 48),
+                                        ((6, 6, 6, 12), 48), ((16, 4, 4, 6), 48), ((8, 4, 4, 24), 3)])
+def test_smear_host_streamed_equals_serial_and_oracle(lqx, dims, slabs, prec):
+    u = _links(11, dims, prec, "near_unit")
+    code = lqx.F32 if prec == "f32" else lqx.F64
+    serial = [np.empty_like(t) for t in u]
+    streamed = [np.full_like(t, np.nan) for t in u]
+    with lqx.Lattice(dims) as lat:
+        lat.set_option("host_slabs", 0)
+        p_serial = lqx.smear_iterate_host(lat, code, u, serial, 0.4, 1)
+        lat.set_option("host_slabs", slabs)
+        n0 = lat.launch_count()
+        p_streamed = lqx.smear_iterate_host(lat, code, u, streamed, 0.4, 1)
+        n_streamed = lat.launch_count() - n0
+        # second call on the same context (events, streams and staging fields are reused), in place
+        inplace = [t.copy() for t in u]
+        p_inplace = lqx.smear_iterate_host(lat, code, inplace, inplace, 0.4, 1)
+    # the serial path launches 4 + 1 + 4 + 2 + 4 kernels; a streamed call launches 9 per slab + 2
+    assert n_streamed > 17, "the streamed path did not run for this lattice"
+    for mu in range(4):
+        assert np.array_equal(serial[mu], streamed[mu])
+        assert np.array_equal(serial[mu], inplace[mu])
+    assert p_serial == p_streamed == p_inplace
+    want_u, want_p = orc.smear_iterate(dims, u, 0.4, 1, prec)
+    assert abs(p_streamed[0] - want_p[0]) < RTOL[prec]
+    for mu in range(4):
+        assert site_rel_err(streamed[mu], want_u[mu]) < 2 * TOL[prec]
+
+
+def test_smear_host_streams_by_default_at_production_slab_sizes(lqx):
+    # automatic setting: 32^3 x 64 in fp32 has 4.7 MB per link in a two-slice slab -> 32 slabs
+    dims = (32, 32, 32, 64)
+    u = _links(13, dims, "f32", "near_unit")
+    serial = [np.empty_like(t) for t in u]
+    streamed = [np.empty_like(t) for t in u]
+    with lqx.Lattice(dims) as lat:
+        n0 = lat.launch_count()
+        p_streamed = lqx.smear_iterate_host(lat, lqx.F32, u, streamed, 0.4, 1)
+        assert lat.launch_count() - n0 == 32 * 9 + 2
+        lat.set_option("host_slabs", 0)
+        p_serial = lqx.smear_iterate_host(lat, lqx.F32, u, serial, 0.4, 1)
+    assert p_serial == p_streamed
+    for mu in range(4):
+        assert np.array_equal(serial[mu], streamed[mu])
+
+
+@pytest.mark.parametrize("slabs", [-1, 48])
+def test_smear_host_falls_back_to_serial_when_slabs_do_not_fit(lqx, slabs):
+    # 6^3 x 6: no even slab thickness gives a multiple of 32 sites and at least three slabs (and, on the automatic
+    # setting, a lattice this small stays serial anyway)
+    dims = (6, 6, 6, 6)
+    u = _links(12, dims, "f32", "near_unit")
+    out = [np.empty_like(t) for t in u]
+    with lqx.Lattice(dims) as lat:
+        lat.set_option("host_slabs", slabs)
+        n0 = lat.launch_count()
+        p = lqx.smear_iterate_host(lat, lqx.F32, u, out, 0.4, 1)
+        assert lat.launch_count() - n0 <= 17
+    want_u, want_p = orc.smear_iterate(dims, u, 0.4, 1, "f32")
+    assert abs(p[0] - want_p[0]) < RTOL["f32"]
+    for mu in range(4):
+        assert site_rel_err(out[mu], want_u[mu]) < 2 * TOL["f32"]
+
+
 # ------------------------------------------------------------------------------------------------
 # error behaviour of the boundary
 # ------------------------------------------------------------------------------------------------
