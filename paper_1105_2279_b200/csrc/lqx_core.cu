@@ -297,48 +297,94 @@ extern "C" void* lqx_field_data(const lqx_field* f) { return f ? f->data : nullp
 extern "C" int lqx_field_kind(const lqx_field* f) { return f ? (int)f->kind : LQX_EINVAL; }
 extern "C" int lqx_field_prec(const lqx_field* f) { return f ? (int)f->prec : LQX_EINVAL; }
 
-// AoS (QDP order) <-> blocked SoA.  One CUDA block handles one 32-site layout block: both sides are
-// the same 32*nreal contiguous reals, so the conversion is a permutation staged through shared
-// memory with coalesced reads and writes on both sides.
-template <typename T, bool TO_SOA>
-__global__ void k_transpose(int V, int nreal, int blk0, const T* __restrict__ src, T* __restrict__ dst) {
-    extern __shared__ unsigned char smem_raw[];
-    T* tile = reinterpret_cast<T*>(smem_raw);  // [32][nreal+1], QDP order
-    constexpr int W = 16 / (int)sizeof(T);
-    const int s0 = (blk0 + blockIdx.x) * 32;
-    const int ns = min(32, V - s0);
-    const int pitch = nreal + 1;
-    const int nfull = nreal / W, rem = nreal - nfull * W;
-    const size_t blk = (size_t)s0 * nreal;
-    // internal position i of the block -> (local site, real)
-    auto decode = [&](int i, int& ls, int& r) {
-        const int q = i / (32 * W);
-        if (q < nfull) {
-            const int t = i - q * 32 * W;
-            ls = t / W;
-            r = q * W + (t - ls * W);
+// AoS (QDP order) <-> blocked SoA.  Both sides of a 32-site layout block are the same 32*NREAL contiguous
+// reals, so the conversion is a permutation staged through shared memory.  One CTA converts kTransposeBlocks
+// consecutive layout blocks with 128-bit global accesses on both sides (a block starts on a 16-byte boundary
+// in either order); NREAL is a template parameter so that the index arithmetic divides by constants -- with
+// run-time divisors and 4-byte accesses the kernel was instruction-bound at 2.2 TB/s.  The last block of a
+// lattice whose volume is not a multiple of 32 takes the element-wise path on its QDP-order side.
+static const int kTransposeBlocks = 4;
+
+template <typename T, int NREAL, bool TO_SOA>
+__global__ void __launch_bounds__(256) k_transpose(int V, int blk0, int blk_end, const T* __restrict__ src, T* __restrict__ dst) {
+    typedef typename Vec128<T>::type VT;
+    constexpr int W = Vec128<T>::W, PITCH = NREAL + 1, NFULL = NREAL / W, REM = NREAL - NFULL * W, REMD = REM ? REM : 1;
+    constexpr int E = 32 * NREAL, EV = E / W;  // reals and 128-bit vectors per block
+    __shared__ T tiles[kTransposeBlocks][32 * PITCH];  // [block][local site][real], QDP order, padded pitch
+    const int first = blk0 + blockIdx.x * kTransposeBlocks;
+    const int nb = min(kTransposeBlocks, blk_end - first);
+    // (local site, real) of element e of vector vi: QDP-order side / blocked side
+    auto aos_pos = [](int vi, int e, int& ls, int& r) {
+        const int idx = vi * W + e;
+        ls = idx / NREAL;
+        r = idx - ls * NREAL;
+    };
+    auto soa_pos = [](int vi, int e, int& ls, int& r) {
+        if (vi < NFULL * 32) {
+            ls = vi & 31;
+            r = (vi >> 5) * W + e;
         } else {
-            const int t = i - nfull * 32 * W;
-            ls = t / rem;
-            r = nfull * W + (t - ls * rem);
+            const int t = (vi - NFULL * 32) * W + e;
+            ls = t / REMD;
+            r = NFULL * W + (t - ls * REMD);
         }
     };
-    if (TO_SOA) {
-        for (int i = threadIdx.x; i < ns * nreal; i += blockDim.x) tile[(i / nreal) * pitch + (i % nreal)] = src[blk + i];
-        __syncthreads();
-        for (int i = threadIdx.x; i < 32 * nreal; i += blockDim.x) {
-            int ls, r;
-            decode(i, ls, r);
-            dst[blk + i] = ls < ns ? tile[ls * pitch + r] : T(0);  // pad lanes of the last block stay zero
+    for (int v = threadIdx.x; v < nb * EV; v += 256) {
+        const int b = v / EV, vi = v - b * EV, blkid = first + b;
+        const int ns = min(32, V - blkid * 32);
+        const T* sp = src + (size_t)blkid * E;
+        T* tile = tiles[b];
+        if (ns == 32 || !TO_SOA) {  // the blocked side is padded to whole blocks
+            T x[W];
+            unpack(*reinterpret_cast<const VT*>(sp + vi * W), x);
+#pragma unroll
+            for (int e = 0; e < W; ++e) {
+                int ls, r;
+                if (TO_SOA) aos_pos(vi, e, ls, r);
+                else soa_pos(vi, e, ls, r);
+                tile[ls * PITCH + r] = x[e];
+            }
+        } else {
+#pragma unroll
+            for (int e = 0; e < W; ++e) {
+                int ls, r;
+                aos_pos(vi, e, ls, r);
+                if (ls < ns) tile[ls * PITCH + r] = sp[vi * W + e];
+            }
         }
-    } else {
-        for (int i = threadIdx.x; i < 32 * nreal; i += blockDim.x) {
-            int ls, r;
-            decode(i, ls, r);
-            if (ls < ns) tile[ls * pitch + r] = src[blk + i];
+    }
+    __syncthreads();
+    for (int v = threadIdx.x; v < nb * EV; v += 256) {
+        const int b = v / EV, vi = v - b * EV, blkid = first + b;
+        const int ns = min(32, V - blkid * 32);
+        T* dp = dst + (size_t)blkid * E;
+        const T* tile = tiles[b];
+        if (TO_SOA) {
+            T x[W];
+#pragma unroll
+            for (int e = 0; e < W; ++e) {
+                int ls, r;
+                soa_pos(vi, e, ls, r);
+                x[e] = ls < ns ? tile[ls * PITCH + r] : T(0);  // pad lanes of the last block stay zero
+            }
+            *reinterpret_cast<VT*>(dp + vi * W) = pack(x);
+        } else if (ns == 32) {
+            T x[W];
+#pragma unroll
+            for (int e = 0; e < W; ++e) {
+                int ls, r;
+                aos_pos(vi, e, ls, r);
+                x[e] = tile[ls * PITCH + r];
+            }
+            *reinterpret_cast<VT*>(dp + vi * W) = pack(x);
+        } else {
+#pragma unroll
+            for (int e = 0; e < W; ++e) {
+                int ls, r;
+                aos_pos(vi, e, ls, r);
+                if (ls < ns) dp[vi * W + e] = tile[ls * PITCH + r];
+            }
         }
-        __syncthreads();
-        for (int i = threadIdx.x; i < ns * nreal; i += blockDim.x) dst[blk + i] = tile[(i / nreal) * pitch + (i % nreal)];
     }
 }
 
@@ -350,14 +396,23 @@ int lqx_transpose_range(lqx_ctx* ctx, lqx_kind kind, lqx_prec prec, const void* 
                         int nblk, cudaStream_t stream) {
     const Geo& g = ctx->geo;
     const int nreal = 2 * (int)kind;
-    const size_t sm = (size_t)32 * (nreal + 1) * (int)prec;
-    if (prec == LQX_F32) {
-        if (to_soa) k_transpose<float, true><<<nblk, 256, sm, stream>>>(g.V, nreal, blk0, (const float*)src, (float*)dst);
-        else k_transpose<float, false><<<nblk, 256, sm, stream>>>(g.V, nreal, blk0, (const float*)src, (float*)dst);
-    } else {
-        if (to_soa) k_transpose<double, true><<<nblk, 256, sm, stream>>>(g.V, nreal, blk0, (const double*)src, (double*)dst);
-        else k_transpose<double, false><<<nblk, 256, sm, stream>>>(g.V, nreal, blk0, (const double*)src, (double*)dst);
+    const int grid = (nblk + kTransposeBlocks - 1) / kTransposeBlocks, end = blk0 + nblk;
+    if (grid <= 0) return LQX_OK;
+#define LQX_TR(T, NREAL)                                                                                        \
+    do {                                                                                                        \
+        if (to_soa) k_transpose<T, NREAL, true><<<grid, 256, 0, stream>>>(g.V, blk0, end, (const T*)src, (T*)dst); \
+        else k_transpose<T, NREAL, false><<<grid, 256, 0, stream>>>(g.V, blk0, end, (const T*)src, (T*)dst);       \
+    } while (0)
+#define LQX_TR_KIND(T)                      \
+    switch (nreal) {                        \
+        case 2: LQX_TR(T, 2); break;        \
+        case 6: LQX_TR(T, 6); break;        \
+        case 18: LQX_TR(T, 18); break;      \
+        default: LQX_TR(T, 24); break;      \
     }
+    if (prec == LQX_F32) { LQX_TR_KIND(float) } else { LQX_TR_KIND(double) }
+#undef LQX_TR_KIND
+#undef LQX_TR
     LQX_LAUNCH_CHECK(ctx);
     return LQX_OK;
 }
