@@ -237,24 +237,35 @@ def jacobi_listing(lqx, chi, u, kappa, iters, no_smear_dir, norm, work, fused):
     """The paper's Listing 1 as USER code on top of the run-time expression path, the way a
     QDP++ program would state it.  fused = False: literally the listing, one expression per line -- E0 copies,
     E1 for the first direction, E2 ('+=') for the others, E3, E4 (six kernels per iteration).  fused = True:
-    one expression per iteration, chi' = s_0 + kappa * sum_mu (...).  work = (s_0, psi, h_smear) scratch fields."""
+    one expression per iteration, chi' = s_0 + kappa * sum_mu (...), the iterate ping-ponging between chi and psi
+    (no copy).  work = (s_0, psi, h_smear) scratch fields."""
     s0, psi, h = work
     L = lqx.Expr.leaf
     lqx.expr_eval(s0, L(chi))                                             # s_0 = chi
-    for _ in range(iters):
-        lqx.expr_eval(psi, L(chi))                                        # psi = chi
-        terms = [L(u[mu]) * lqx.shifted(psi, lqx.FORWARD, mu) + lqx.shifted(lqx.adj(u[mu]) * L(psi), lqx.BACKWARD, mu)
-                 for mu in range(4) if mu != no_smear_dir]
-        if fused:
+
+    def hop_terms(f):
+        return [L(u[mu]) * lqx.shifted(f, lqx.FORWARD, mu) + lqx.shifted(lqx.adj(u[mu]) * L(f), lqx.BACKWARD, mu)
+                for mu in range(4) if mu != no_smear_dir]
+
+    if fused:
+        # E0 (psi = chi) disappears too: the iterate ping-pongs between chi and psi, E4 reads whichever holds it
+        cur, nxt = chi, psi
+        for _ in range(iters):
+            terms = hop_terms(cur)
             e = terms[0]
             for t in terms[1:]:
                 e = e + t
-            lqx.expr_eval(chi, L(s0) + kappa * e)                         # E1..E3 in one kernel
-        else:
-            lqx.expr_eval(h, terms[0])                                    # h_smear  = ...   (E1)
-            for t in terms[1:]:
-                lqx.expr_eval(h, t, accumulate=True)                      # h_smear += ...   (E2)
-            lqx.expr_eval(chi, L(s0) + kappa * L(h))                      # chi = s_0 + kappa*h_smear (E3)
+            lqx.expr_eval(nxt, L(s0) + kappa * e)                         # E1..E3 in one kernel
+            cur, nxt = nxt, cur
+        lqx.expr_eval(chi, (1.0 / norm) * L(cur))                         # chi = iterate / norm (E4)
+        return
+    for _ in range(iters):
+        lqx.expr_eval(psi, L(chi))                                        # psi = chi
+        terms = hop_terms(psi)
+        lqx.expr_eval(h, terms[0])                                        # h_smear  = ...   (E1)
+        for t in terms[1:]:
+            lqx.expr_eval(h, t, accumulate=True)                          # h_smear += ...   (E2)
+        lqx.expr_eval(chi, L(s0) + kappa * L(h))                          # chi = s_0 + kappa*h_smear (E3)
     lqx.expr_eval(chi, (1.0 / norm) * L(chi))                             # chi /= norm (E4; reciprocal multiply, A22)
 
 

@@ -296,6 +296,36 @@ struct Gen {
         else os << "    const " << ty << " " << v << " = jmacv<" << n[pi].kind / 3 << ">(" << l << ", " << a << ", " << b << ");\n";
         return true;
     }
+    // the terms of a tree of additions, left to right; a shift of a sum is the sum of the shifted terms
+    void collect_terms(int i, const Site& site, std::vector<std::pair<int, Site>>& terms) {
+        const XNode& x = n[i];
+        if (x.op == LQX_X_ADD) {
+            collect_terms(x.child[0], site, terms);
+            collect_terms(x.child[1], site, terms);
+            return;
+        }
+        if (x.op == LQX_X_SHIFT) {
+            int c = x.child[0];
+            while (n[c].op == LQX_X_SHIFT) c = n[c].child[0];
+            if (n[c].op == LQX_X_ADD) {
+                collect_terms(x.child[0], shifted(site, x), terms);
+                return;
+            }
+        }
+        terms.push_back(std::make_pair(i, site));
+    }
+    // acc + m*y (the product possibly under shifts) as one multiply-accumulate named v; false if term is no product
+    bool emit_mac(const std::string& acc, int prod, const Site& site, const std::string& v, const std::string& ty) {
+        int pi = prod;
+        while (n[pi].op == LQX_X_SHIFT) pi = n[pi].child[0];
+        if (n[pi].op != LQX_X_MUL) return false;
+        Site ps = site;
+        for (pi = prod; n[pi].op == LQX_X_SHIFT; pi = n[pi].child[0]) ps = shifted(ps, n[pi]);
+        const std::string a = val(n[pi].child[0], ps), b = val(n[pi].child[1], ps);
+        if (n[n[pi].child[1]].kind == LQX_COLORMAT) os << "    const " << ty << " " << v << " = jmac(" << acc << ", " << a << ", " << b << ");\n";
+        else os << "    const " << ty << " " << v << " = jmacv<" << n[pi].kind / 3 << ">(" << acc << ", " << a << ", " << b << ");\n";
+        return true;
+    }
     std::string val(int i, const Site& site) {
         const XNode& x = n[i];
         const std::string ty = "Obj<" + std::to_string(x.kind) + ">";
@@ -318,6 +348,25 @@ struct Gen {
             }
             case LQX_X_ADD:
             case LQX_X_SUB: {
+                if (x.op == LQX_X_ADD) {
+                    // a sum of three or more terms is evaluated as ONE accumulation chain in the order written
+                    // (t0 + t1 + t2 ... ; products become multiply-accumulates): no partial sums are kept alive
+                    // beside the accumulator, which is what lets the hop run at six CTAs per SM
+                    std::vector<std::pair<int, Site>> terms;
+                    collect_terms(i, site, terms);
+                    if (terms.size() > 2) {
+                        std::string acc = val(terms[0].first, terms[0].second);
+                        for (size_t t = 1; t < terms.size(); ++t) {
+                            const std::string name = t + 1 == terms.size() ? v : "v" + std::to_string(tmp++);
+                            if (!emit_mac(acc, terms[t].first, terms[t].second, name, ty)) {
+                                const std::string r = val(terms[t].first, terms[t].second);
+                                os << "    const " << ty << " " << name << " = jadd(" << acc << ", " << r << ");\n";
+                            }
+                            acc = name;
+                        }
+                        break;
+                    }
+                }
                 if (x.op == LQX_X_ADD && (try_mac(x.child[0], x.child[1], site, v, ty) || try_mac(x.child[1], x.child[0], site, v, ty))) break;
                 std::string l = val(x.child[0], site), r = val(x.child[1], site);
                 os << "    const " << ty << " " << v << " = " << (x.op == LQX_X_ADD ? "jadd" : "jsub") << "(" << l << ", " << r << ");\n";
@@ -431,7 +480,7 @@ std::string make_source(const std::vector<XNode>& tree, int nleaves, int nscalar
     else src << "typedef double T;\ntypedef double2 VEC;\nconstexpr int W = 2;\n";
     src << kPrelude;
     // register budget: 128 per thread in fp32 (four CTAs per SM), 255 in fp64 (measured on the hop expression)
-    src << "extern \"C\" __global__ void __launch_bounds__(128, " << (f32 ? 4 : 2) << ") lqx_jit(const JGeo g";
+    src << "extern \"C\" __global__ void __launch_bounds__(128, " << (f32 ? 6 : 3) << ") lqx_jit(const JGeo g";
     for (int k = 0; k < nscalars; ++k) src << ", const T k" << k;
     for (int l = 0; l < nleaves; ++l) src << ", const T* __restrict__ p" << l;
     const int nc = reduce == 1 ? 1 : 2 * dst_kind;

@@ -65,7 +65,10 @@ __global__ void __launch_bounds__(MAP::THREADS, (sizeof(T) == 4 ? 768 : 512) / M
 // ---------------------------------------------------------------------------------------------
 // Launch geometry (the paper's two tuning parameters): N_threads = blockDim.x (32..256)
 // and N_site = NSITE sites per thread, taken grid-strided so that a warp still reads 32 consecutive sites.
-template <typename T, int NSPIN, bool DIV, int NSITE>
+// MASK >= 0: the set of smeared directions is a compile-time constant (all four, or all but time -- the two cases
+// that occur), so the body is straight-line code and the loads of all directions can be in flight together;
+// MASK < 0: the run-time dirmask decides per direction.
+template <typename T, int NSPIN, bool DIV, int NSITE, int MASK>
 __global__ void __launch_bounds__(256, sizeof(T) == 4 ? 3 : 2) k_jacobi_step(const __grid_constant__ Geo g, const __grid_constant__ Links<T> u,
                                                                              int dirmask, const T* __restrict__ psi, const T* __restrict__ s0,
                                                                              T kappa, T nrm, T* __restrict__ chi) {
@@ -82,7 +85,7 @@ __global__ void __launch_bounds__(256, sizeof(T) == 4 ? 3 : 2) k_jacobi_step(con
             for (int i = 0; i < 3; ++i) acc[a].re[i] = acc[a].im[i] = T(0);
 #pragma unroll
         for (int mu = 0; mu < 4; ++mu) {
-            if (!((dirmask >> mu) & 1)) continue;
+            if (MASK >= 0 ? !((MASK >> mu) & 1) : !((dirmask >> mu) & 1)) continue;
             const int f = nbr_fwd(g, s, x, mu), b = nbr_bwd(g, s, x, mu);
             {
                 const Mat3<T> m = load_mat(u.u[mu], s);
@@ -552,14 +555,16 @@ extern "C" int lqx_jacobi_smear(lqx_field* chi, const lqx_field* const u[4], dou
         const bool last = it == iter - 1;
         {
             LqxTimed timed(ctx, LQX_K_HOP);
-#define LQX_JAC3(T, NSPIN, DIV, NS)                                                                                              \
-    k_jacobi_step<T, NSPIN, DIV, NS><<<grid, bs, 0, ctx->stream>>>(g, make_links<T>(u), dirmask, (const T*)cur->data,         \
-                                                                   (const T*)tmp[0]->data, (T)kappa, (T)norm, (T*)nxt->data)
-#define LQX_JAC(T, NSPIN, DIV)                                \
-    do {                                                      \
-        if (nsite == 1) LQX_JAC3(T, NSPIN, DIV, 1);           \
-        else if (nsite == 2) LQX_JAC3(T, NSPIN, DIV, 2);      \
-        else LQX_JAC3(T, NSPIN, DIV, 4);                      \
+#define LQX_JAC3(T, NSPIN, DIV, NS, MASK)                                                                                          \
+    k_jacobi_step<T, NSPIN, DIV, NS, MASK><<<grid, bs, 0, ctx->stream>>>(g, make_links<T>(u), dirmask, (const T*)cur->data,         \
+                                                                         (const T*)tmp[0]->data, (T)kappa, (T)norm, (T*)nxt->data)
+#define LQX_JAC(T, NSPIN, DIV)                                          \
+    do {                                                                \
+        if (nsite == 1 && dirmask == 0xF) LQX_JAC3(T, NSPIN, DIV, 1, 0xF); \
+        else if (nsite == 1 && dirmask == 0x7) LQX_JAC3(T, NSPIN, DIV, 1, 0x7); \
+        else if (nsite == 1) LQX_JAC3(T, NSPIN, DIV, 1, -1);            \
+        else if (nsite == 2) LQX_JAC3(T, NSPIN, DIV, 2, -1);            \
+        else LQX_JAC3(T, NSPIN, DIV, 4, -1);                            \
     } while (0)
             if (chi->prec == LQX_F32) {
                 if (ferm) { if (last) LQX_JAC(float, 4, true); else LQX_JAC(float, 4, false); }
