@@ -528,6 +528,8 @@ def run_ours(args):
         "peak_source": f"148 SMs x {128 if prec == 'f32' else 64} FMA lanes x 2 x {sm_max:.0f} MHz (DESIGN.md sec.7); "
                        f"FMA-chain micro-benchmark in this run: {2 * fma_peak / 1e12:.1f} TFLOP/s"
                        + (f", packed f32x2: {2 * fma2_peak / 1e12:.1f}" if fma2_peak else ""),
+        "frac_at_measured_clock": (2 * lane_ops / (k_ms * 1e-3) / 1e12) / (alu_peak_tflops * clocks["sm_mhz"] / sm_max)
+        if clocks.get("sm_mhz") else None,
         "flops_counted": f"executed FMA lane-ops x 2 ({SMEAR_LANE_OPS[variant]} lane-ops/site, {variant} evaluation)",
         "traffic": traffic, "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum)",
         "traffic_source": traffic_src, "ms_per_launch": k_ms, "launches": smear_n,
