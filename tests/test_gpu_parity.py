@@ -832,3 +832,41 @@ def test_jacobi_listing_through_runtime_expressions(lqx, prec, fused):
         ref = lat.from_host(chi0)
         lqx.jacobi_smear(ref, fu, kappa, iters, skip, norm, work[:2])
         assert site_rel_err(got, ref.pop()) < TOL[prec] * iters
+
+
+# ------------------------------------------------------------------------------------------------
+# bench.py: the JSON line the driver reads (a smaller workload than the default, same code path)
+# ------------------------------------------------------------------------------------------------
+def test_bench_line_contract():
+    import json
+    import os
+    import subprocess
+    import sys
+
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    out = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--workload", "c3", "--steps", "2", "--warmup", "3",
+                          "--e2e-steps", "2", "--no-extras"], capture_output=True, text=True, cwd=root, timeout=600)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [ln for ln in out.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1, "exactly one JSON line on stdout"
+    line = json.loads(lines[0])
+    assert line["metric"] == "smear-step site-updates/s" and line["unit"] == "site-updates/s"
+    assert line["n_gpus"] == 1 and line["steps"] == 2 and line["warmup"] >= 3
+    assert line["higher_is_better"] is True and line["scaling"] == "weak" and line["data"] == "synthetic"
+    assert line["dtype"] == "f64" and line["vs_baseline"] is None
+    assert "workload" in line["config"] and "model" not in line["config"]
+    sites = line["config"]["sites"]
+    assert abs(line["value"] - sites * 2 / (line["ms_per_step"] * 2 * 1e-3)) < 1e-6 * line["value"]
+    assert line["gpu_launches"] >= 2 * 1  # at least one smear kernel per step
+    r = line["roofline"]
+    assert r["bound"] in ("hbm", "tensor", "alu") and r["unit"] in ("GB/s", "TFLOP/s")
+    assert 0.0 < r["frac"] < 1.0 and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-9
+    assert "traffic" in r and 0.0 < r["hbm"]["frac"] < 1.0
+    e = line["e2e"]
+    assert e["unit"] == line["unit"] and 0.0 < e["value"] < line["value"]
+    assert e["h2d_bytes_per_step"] == sites * 4 * 18 * 8 and e["d2h_bytes_per_step"] >= e["h2d_bytes_per_step"]
+    c = line["cpu_baseline"]
+    assert c["kind"] == "oracle" and c["cores"] >= 1 and 0.0 < c["value"] < line["value"] and c["sample"]
+    k = line["clocks"]
+    assert k["sm_max_mhz"] > 0 and isinstance(k["reasons"], list)
+    assert len(line["plaquette_avg_after_each_step"]) == 2 and all(abs(p) <= 1.0 for p in line["plaquette_avg_after_each_step"])
