@@ -239,10 +239,11 @@ __global__ void __launch_bounds__(256) k_trace(int V, const T* __restrict__ m, d
     block_reduce_finish<2>(acc, partials, ticket, out);
 }
 
-int reduce_grid(const lqx_ctx* ctx, int sites_per_thread) {
-    // fixed function of V only => deterministic summation tree
+int reduce_grid(const lqx_ctx* ctx, int sites_per_thread, int ctas_per_sm = 8) {
+    // fixed function of V (and the SM count) only => deterministic summation tree; the cap is the number of CTAs
+    // that are resident at once, so that the grid is one wave
     long want = ((long)ctx->geo.V / sites_per_thread + 255) / 256;
-    long cap = (long)ctx->num_sms * 8;
+    long cap = (long)ctx->num_sms * ctas_per_sm;
     return (int)std::max<long>(1, std::min(want, cap));
 }
 
@@ -374,7 +375,8 @@ extern "C" int lqx_sum(const lqx_field* f, double* out) {
     lqx_ctx* ctx = f->ctx;
     LQX_CUDA(ctx, cudaSetDevice(ctx->device));
     const int nc = 2 * (int)f->kind;
-    const int grid = reduce_grid(ctx, 2);
+    // the site-object sum keeps 2*kind fp64 accumulators per thread: fewer resident CTAs than the scalar reductions
+    const int grid = reduce_grid(ctx, 2, nc <= 6 ? 8 : (f->prec == LQX_F32 ? 4 : 3));
     int rc = lqx_ensure_partials(ctx, (size_t)grid * nc);
     if (rc) return rc;
     const int V = ctx->geo.V;
