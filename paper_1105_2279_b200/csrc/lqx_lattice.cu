@@ -13,7 +13,7 @@ namespace {
 // (Listing 1 lines 25/27 summed over mu; Eq. 2; BASELINE configs[1])
 // ---------------------------------------------------------------------------------------------
 template <typename T, int NSPIN, bool NORM2, typename MAP>
-__global__ void __launch_bounds__(MAP::THREADS, (sizeof(T) == 4 ? 768 : 512) / MAP::THREADS) k_hop(const __grid_constant__ Geo g, const __grid_constant__ TileMap tm,
+__global__ void __launch_bounds__(MAP::THREADS, (sizeof(T) == 4 ? 896 : 512) / MAP::THREADS) k_hop(const __grid_constant__ Geo g, const __grid_constant__ TileMap tm,
                                                       const __grid_constant__ Links<T> u, const T* __restrict__ psi, T* __restrict__ chi,
                                                       double* __restrict__ partials, unsigned int* ticket, double* __restrict__ out) {
     int x[4], s;
