@@ -381,6 +381,17 @@ def _extras(torch, lqx, li, hbm_gbs):
         add("smear_step+plaquette(in) fused c3 (incl. sync)", "f64", v, 144, SMEAR_CANONICAL_FLOPS + 108,
             lambda: lqx.smear_step(o, u, ALPHA, want_plaq_in=True), reps=12, lat=lat, kclass=lqx.K_SMEAR)
         add("plaquette c3 (incl. sync)", "f64", v, 72, 2591, lambda: lqx.plaquette(u), reps=6, lat=lat, kclass=lqx.K_PLAQUETTE)
+        # the same quantity stated by the user as an expression and reduced inside ONE generated kernel
+        L = lqx.Expr.leaf
+        pe = None
+        for mu in range(3):
+            for nu in range(mu + 1, 4):
+                t = (L(u[mu]) * lqx.shifted(u[nu], lqx.FORWARD, mu)) * lqx.adj(L(u[nu]) * lqx.shifted(u[mu], lqx.FORWARD, nu))
+                pe = t if pe is None else pe + t
+        pe = pe.trace()
+        lqx.expr_reduce(lqx.R_SUM, pe)  # compiles
+        add("plaquette c3 as a run-time expression: sum(trace(sum_{mu<nu} ...)) in one generated kernel (incl. sync)", "f64", v, 72, 2591,
+            lambda: lqx.expr_reduce(lqx.R_SUM, pe), reps=6, lat=lat, kclass=lqx.K_REDUCE)
     # ---- C5: catalogue sweep, 32^3x64, both precisions
     dims = li.CONFIGS["c5"]["dims"]
     for prec, pcode in (("f32", lqx.F32), ("f64", lqx.F64)):

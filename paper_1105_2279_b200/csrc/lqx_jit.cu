@@ -471,6 +471,57 @@ int build_tree(lqx_ctx* ctx, const lqx_xnode* nodes, int nnodes, const lqx_field
     return LQX_OK;
 }
 
+// Estimate of the reals a thread holds at the widest point of the evaluation (operands are evaluated left to
+// right, a sum is one accumulation chain): picks the CTAs-per-SM bound of the generated kernel, so that a small
+// expression (the hop: accumulator + one matrix + one fermion) runs at six CTAs per SM and a product of
+// products (the plaquette: four matrices and an accumulator) is not forced to spill.
+static void live_terms(const std::vector<XNode>& n, int i, std::vector<int>& terms) {
+    if (n[i].op == LQX_X_ADD) {
+        live_terms(n, n[i].child[0], terms);
+        live_terms(n, n[i].child[1], terms);
+        return;
+    }
+    if (n[i].op == LQX_X_SHIFT) {
+        int c = n[i].child[0];
+        while (n[c].op == LQX_X_SHIFT) c = n[c].child[0];
+        if (n[c].op == LQX_X_ADD) {
+            live_terms(n, c, terms);
+            return;
+        }
+    }
+    terms.push_back(i);
+}
+static int live_reals(const std::vector<XNode>& n, int i) {
+    const XNode& x = n[i];
+    const int sz = 2 * x.kind;
+    switch (x.op) {
+        case LQX_X_LEAF: return sz;
+        case LQX_X_MUL: {
+            const int l = live_reals(n, x.child[0]), r = live_reals(n, x.child[1]);
+            const int sl = 2 * n[x.child[0]].kind, sr = 2 * n[x.child[1]].kind;
+            return std::max(std::max(l, sl + r), sl + sr + sz);
+        }
+        case LQX_X_SUB: return std::max(live_reals(n, x.child[0]), sz + live_reals(n, x.child[1]));
+        case LQX_X_ADD: {
+            std::vector<int> terms;
+            live_terms(n, i, terms);
+            int m = live_reals(n, terms[0]);
+            for (size_t t = 1; t < terms.size(); ++t) {
+                int p = terms[t];
+                while (n[p].op == LQX_X_SHIFT) p = n[p].child[0];
+                if (n[p].op == LQX_X_MUL) {  // multiply-accumulate: the product has no result of its own
+                    const int sl = 2 * n[n[p].child[0]].kind, sr = 2 * n[n[p].child[1]].kind;
+                    m = std::max(m, sz + std::max(std::max(live_reals(n, n[p].child[0]), sl + live_reals(n, n[p].child[1])), sl + sr));
+                } else {
+                    m = std::max(m, sz + live_reals(n, terms[t]));
+                }
+            }
+            return m;
+        }
+        default: return live_reals(n, x.child[0]);  // adj, shift, scale, trace
+    }
+}
+
 // reduce: 0 = dst (=|+=) expr ; 1 = norm2(expr) ; 2 = sum(expr).  For the reductions every thread walks a
 // grid-stride loop of sites with fp64 accumulators and the CTA leaves one partial per component.
 std::string make_source(const std::vector<XNode>& tree, int nleaves, int nscalars, int dst_kind, bool f32, bool accumulate,
@@ -479,8 +530,12 @@ std::string make_source(const std::vector<XNode>& tree, int nleaves, int nscalar
     if (f32) src << "typedef float T;\ntypedef float4 VEC;\nconstexpr int W = 4;\n";
     else src << "typedef double T;\ntypedef double2 VEC;\nconstexpr int W = 2;\n";
     src << kPrelude;
-    // register budget: 128 per thread in fp32 (four CTAs per SM), 255 in fp64 (measured on the hop expression)
-    src << "extern \"C\" __global__ void __launch_bounds__(128, " << (f32 ? 6 : 3) << ") lqx_jit(const JGeo g";
+    // register budget from the estimated live reals (+ fp64 reduction accumulators, + 16 for indices and
+    // pointers): at most six CTAs of 128 threads per SM (85 registers) in fp32 and three (170) in fp64, at least two
+    const int nacc = reduce == 1 ? 1 : (reduce == 2 ? 2 * dst_kind : 0);
+    const int regs = live_reals(tree, (int)tree.size() - 1) * (f32 ? 1 : 2) + 2 * nacc + 16;
+    const int min_blocks = std::max(2, std::min(f32 ? 6 : 3, 65536 / (128 * regs)));
+    src << "extern \"C\" __global__ void __launch_bounds__(128, " << min_blocks << ") lqx_jit(const JGeo g";
     for (int k = 0; k < nscalars; ++k) src << ", const T k" << k;
     for (int l = 0; l < nleaves; ++l) src << ", const T* __restrict__ p" << l;
     const int nc = reduce == 1 ? 1 : 2 * dst_kind;

@@ -3,6 +3,7 @@ the evaluator must reduce to the already pinned oracle routines on the expressio
 (form i, form iii, the paper's hop written exactly as Listing 1 lines 25/27, the staple sum written with
 nested shifts), and the CUDA source generated for those expressions must compile for sm_100a."""
 import os
+import re
 import shutil
 import subprocess
 
@@ -70,6 +71,13 @@ def test_evaluator_reduces_to_the_pinned_routines(dims):
     tr = orc.eval_expr(dims, [(L, 0, 0, 0), (L, 1, 0, 0), (MUL, 0, 0, 0), (TRACE, 0, 0, 0)], [a, b])
     want = orc.trace_mm(dims, a, b, "t64")
     assert tr.shape == want.shape and np.abs(tr - want).max() < 1e-13
+    # the plaquette written as an expression: Re of its per-site value is the pinned per-site plaquette integrand
+    pl = orc.eval_expr(dims, plaquette_nodes(), u)
+    v = int(np.prod(dims))
+    want = orc.plaquette_sites(dims, u, np.arange(v, dtype=np.int64), "t64")
+    got = np.asarray(pl).reshape(v, -1)
+    re = got[:, 0].real if np.iscomplexobj(got) else got[:, 0]
+    assert np.abs(re - want).max() < 1e-12
 
 
 def test_evaluator_rejects_malformed_sequences():
@@ -81,6 +89,19 @@ def test_evaluator_rejects_malformed_sequences():
 
 
 # ------------------------------------------------------------------ the code generator, without a GPU
+def plaquette_nodes():
+    """trace( sum_{mu<nu} (u[mu]*shift(u[nu],F,mu)) * adj(u[nu]*shift(u[mu],F,nu)) ); leaves u0..u3"""
+    n, first = [], True
+    for mu in range(3):
+        for nu in range(mu + 1, 4):
+            n += [(L, mu, 0, 0), (L, nu, 0, 0), (SHIFT, +1, mu, 0), (MUL, 0, 0, 0)]
+            n += [(L, nu, 0, 0), (L, mu, 0, 0), (SHIFT, +1, nu, 0), (MUL, 0, 0, 0), (ADJ, 0, 0, 0), (MUL, 0, 0, 0)]
+            if not first:
+                n += [(ADD, 0, 0, 0)]
+            first = False
+    return n + [(TRACE, 0, 0, 0)]
+
+
 def _source(nodes, leaf_kinds, dst_kind, prec, accumulate=False):
     import paper_1105_2279_b200 as lqx
 
@@ -136,10 +157,29 @@ def test_generated_source_compiles_for_sm_100a(tmp_path, prec):
     sources["trace_mm"] = lqx.expr_source(None, lqx.COMPLEX, pc, e)
     sources["norm2_hop"] = lqx.expr_source(None, lqx.FERMION, pc, lqx.Expr(hop_nodes(), [lqx.COLORMAT] * 4 + [lqx.FERMION]), reduce=1)
     sources["sum_form_i"] = lqx.expr_source(None, lqx.COLORMAT, pc, lqx.Expr(list(FORM_I), [lqx.COLORMAT] * 4), reduce=2)
+    sources["sum_plaquette"] = lqx.expr_source(None, lqx.COMPLEX, pc, lqx.Expr(plaquette_nodes(), [lqx.COLORMAT] * 4), reduce=2)
     assert "jreduce<1>" in sources["norm2_hop"] and "jreduce<18>" in sources["sum_form_i"] and "jstore" not in sources["norm2_hop"].split("lqx_jit")[1]
     for name, text in sources.items():
         f = tmp_path / f"{name}_{prec}.cu"
         f.write_text(text)
-        r = subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-std=c++17", "-cubin", "-o", str(f) + ".cubin", str(f)],
-                           capture_output=True, text=True)
+        r = subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-std=c++17", "-Xptxas", "-v", "-cubin", "-o",
+                            str(f) + ".cubin", str(f)], capture_output=True, text=True)
         assert r.returncode == 0, r.stderr[-3000:]
+        # the CTAs-per-SM bound follows the expression's register need: nothing beyond a few spilled words
+        spill = [int(x) for x in re.findall(r"(\d+) bytes spill stores", r.stderr)]
+        assert spill and max(spill) <= 64, (name, r.stderr[-600:])
+
+
+def test_launch_bounds_follow_the_register_need():
+    import paper_1105_2279_b200 as lqx
+
+    def blocks(src):
+        return int(re.search(r"__launch_bounds__\(128, (\d+)\)", src).group(1))
+
+    cm4, f = [lqx.COLORMAT] * 4, lqx.FERMION
+    # accumulator + one matrix + one fermion: six CTAs of 128 threads per SM in fp32 (85 registers), three in fp64
+    assert blocks(_source(hop_nodes(), cm4 + [f], f, lqx.F32)) == 6
+    assert blocks(_source(hop_nodes(), cm4 + [f], f, lqx.F64)) == 3
+    # a product of products under a sum needs four matrices and the accumulator live: fewer CTAs, no spills
+    assert blocks(lqx.expr_source(None, lqx.COMPLEX, lqx.F32, lqx.Expr(plaquette_nodes(), cm4), reduce=2)) <= 4
+    assert blocks(lqx.expr_source(None, lqx.COMPLEX, lqx.F64, lqx.Expr(plaquette_nodes(), cm4), reduce=2)) == 2
