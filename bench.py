@@ -325,6 +325,24 @@ def _extras(torch, lqx, li, hbm_gbs):
         add("hop c2, 20 launches back to back (per 20; ramp-up and drain overlap as in the iterated Jacobi routine)", "f32", v * 20, 120, 2280,
             hop20, reps=10)
         out[-1]["l2"] = "warm: 63 MB working set fits the 126 MB L2"
+        # "CUDA-graph-amortised" -- the same 20 launches captured once and replayed as one graph
+        try:
+            side = torch.cuda.Stream()
+            lat.set_stream(side)
+            with torch.cuda.stream(side):
+                lqx.hop(chi, u, psi)
+                side.synchronize()
+                graph = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(graph, stream=side):
+                    hop20()
+                add("hop c2, 20 launches replayed as ONE CUDA graph (per 20)", "f32", v * 20, 120, 2280, graph.replay, reps=10)
+                out[-1]["l2"] = "warm: 63 MB working set fits the 126 MB L2"
+                del graph
+        except Exception as e:  # a failed capture must not take the bench line down
+            out.append({"kernel": "hop c2, CUDA graph", "error": repr(e)[:200]})
+        finally:
+            torch.cuda.synchronize()
+            lat.set_stream(torch.cuda.current_stream())
         add("hop+norm2 fused c2 (L2-cold, incl. sync)", "f32", v, 120, 2328, lambda: lqx.hop_norm2(chi, u, psi), reps=20, cold=True,
             lat=lat, kclass=lqx.K_HOP)
     # ---- the same hop kernel on a lattice 16x larger (32^3x64: 1 GB moved), where launch ramp-up and

@@ -215,6 +215,12 @@ class Lattice:
         _check(_lib.lqx_neighbor_table(self.ctx, direction, mu, out.ctypes.data_as(C.c_void_p)), self.ctx)
         return out
 
+    def set_stream(self, stream):
+        """lqx_set_stream: later calls are enqueued on `stream` (a torch.cuda.Stream); the old one is synchronised
+        first.  With a non-default stream the asynchronous calls can be captured into a CUDA graph."""
+        _check(_lib.lqx_set_stream(self.ctx, C.c_void_p(stream.cuda_stream)), self.ctx)
+        self.stream = stream
+
     def set_option(self, key: str, value: int):
         _check(_lib.lqx_set_option(self.ctx, key.encode(), int(value)), self.ctx)
 

@@ -237,6 +237,50 @@ def test_hop(lqx, dims, prec):
             assert abs(n2 - lqx.norm2(chi)) / want_n2 < 1e-13  # fused == two-call up to summation order
 
 
+def test_hop_and_smear_step_captured_in_a_cuda_graph(lqx):
+    """The asynchronous calls do nothing but enqueue kernels on the context's stream, so a user can capture them
+    into a CUDA graph (graph-amortised launches).  The replayed graph must reproduce the direct
+    calls bit for bit -- and those are checked against the oracle here as well."""
+    import torch
+
+    dims, prec = DIMS_RAGGED, "f32"
+    u = _links(2, dims, prec)
+    psi = _gauss(2, 10, dims, "f", prec)
+    with lqx.Lattice(dims) as lat:
+        fu = [lat.from_host(t) for t in u]
+        fo = [lat.alloc(lqx.COLORMAT, lqx.F32) for _ in range(4)]
+        fp = lat.from_host(psi)
+        chi = lat.alloc(fp.kind, fp.prec)
+        lqx.hop(chi, fu, fp)
+        lqx.smear_step(fo, fu, 0.5)
+        direct_chi = chi.pop()
+        direct_u = [f.pop() for f in fo]
+        assert site_rel_err(direct_chi, orc.hop(dims, u, psi, "t32")) < TOL[prec]
+        side = torch.cuda.Stream()
+        lat.set_stream(side)
+        try:
+            with torch.cuda.stream(side):
+                lqx.copy(chi, fp)            # overwrite the results so that only the replay can restore them
+                for f, g in zip(fo, fu):
+                    lqx.copy(f, g)
+                n0 = lat.launch_count()
+                graph = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(graph, stream=side):
+                    lqx.hop(chi, fu, fp)
+                    lqx.smear_step(fo, fu, 0.5)
+                assert lat.launch_count() - n0 == 2
+                side.synchronize()
+                assert not np.array_equal(chi.pop(), direct_chi)  # capture enqueued nothing
+                graph.replay()
+                side.synchronize()
+            assert np.array_equal(chi.pop(), direct_chi)
+            for f, d in zip(fo, direct_u):
+                assert np.array_equal(f.pop(), d)
+        finally:
+            torch.cuda.synchronize()
+            lat.set_stream(torch.cuda.current_stream())
+
+
 def test_c2_hop_full_size(lqx):
     """BASELINE.json configs[1]: 16^3x32 fp32, Haar links, Gaussian fermion; hop then norm2."""
     cfg = li.CONFIGS["c2"]
