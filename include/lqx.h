@@ -263,6 +263,8 @@ int64_t lqx_launch_count(const lqx_ctx* ctx);
  * lattice.  "jacobi_block" (32, 64, 128, 256) and "jacobi_sites" (1, 2, 4): the paper's launch
  * geometry parameters N_threads and N_site for lqx_jacobi_smear; 0 = tuned default.
  * "host_slabs": see lqx_smear_iterate_host.
+ * "plaq_variant" 0 = automatic (fp32: the site's four links held in registers, 16 matrix loads per site;
+ * fp64: rolled plane loops, 21 loads at half the registers -- each the faster one measured), 1 = rolled, 2 = held.
  * "time_kernels" 0/1 (see above).  All variants agree within rounding; DESIGN.md sec.6. */
 int lqx_set_option(lqx_ctx* ctx, const char* key, int value);
 

@@ -51,6 +51,7 @@ struct lqx_ctx {
     int64_t launches;
     int num_sms;
     int opt_smear_variant;
+    int opt_plaq_variant;                 // plaquette kernel: 0 = automatic, 1 = rolled loops, 2 = the site's four links held in registers
     int opt_block;
     int opt_jacobi_block, opt_jacobi_sites;  // launch geometry of the Jacobi step (0 = default 128 x 1)
     int opt_tile;  // -1 = automatic, 0 = Linear, 1..3 = TileA..TileC (lqx_smear.cuh)

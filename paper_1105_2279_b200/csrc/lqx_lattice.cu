@@ -148,6 +148,39 @@ __global__ void __launch_bounds__(MAP::THREADS) k_plaquette(const __grid_constan
     block_reduce_partial<1>(p, partials);
 }
 
+// The same sum with the four links of the site held in registers and the plane loops unrolled: 16 instead of
+// 21 matrix loads per site for about twice the registers (fp32: 165, three CTAs per SM).  The kernel is bound by
+// the L1 data pipe rather than by latency -- spreading the six planes of a site over six warps (more loads in
+// flight, 24 loads per site) ran 30-50 % slower -- so in fp32 the saved loads outweigh the lost occupancy
+// (0.94 -> 0.86 ms at 48^3x96); in fp64 (254 registers) they do not (0.37 -> 0.39 ms at 32^3x64).
+template <typename T, int MINB>
+__global__ void __launch_bounds__(128, MINB) k_plaquette_held(const __grid_constant__ Geo g, const __grid_constant__ Links<T> u,
+                                                              double* __restrict__ partials) {
+    const int s = blockIdx.x * 128 + threadIdx.x;
+    double p[1] = {0.0};
+    if (s < g.V) {
+        int x[4];
+        site_coords(g, s, x);
+        Mat3<T> own[4];
+#pragma unroll
+        for (int mu = 0; mu < 4; ++mu) own[mu] = load_mat(u.u[mu], s);
+        T acc = T(0);
+#pragma unroll
+        for (int mu = 0; mu < 3; ++mu) {
+            const int xpmu = nbr_fwd(g, s, x, mu);
+#pragma unroll
+            for (int nu = mu + 1; nu < 4; ++nu) {
+                const int xpnu = nbr_fwd(g, s, x, nu);
+                const Mat3<T> q1 = mul_nn(own[mu], load_mat(u.u[nu], xpmu));
+                const Mat3<T> q2 = mul_nn(own[nu], load_mat(u.u[mu], xpnu));
+                acc += re_tr_na(q1, q2);
+            }
+        }
+        p[0] = (double)acc;
+    }
+    block_reduce_partial<1>(p, partials);
+}
+
 int check_links(lqx_ctx** ctx_out, const lqx_field* const u[4]) {
     if (!u) return LQX_EINVAL;
     lqx_ctx* ctx = nullptr;
@@ -168,6 +201,19 @@ int plaquette_launch(lqx_ctx* ctx, const lqx_field* const u[4], double* out) {
     const Geo& g = ctx->geo;
     const int choice = lqx_pick_tile(ctx, 0);  // measured: linear 128-site blocks beat every tile shape here
     int nblocks = 0;
+    // option plaq_variant: 0 = automatic (held links in fp32, rolled loops in fp64: measured), 1 = rolled, 2 = held
+    const bool held = ctx->opt_plaq_variant == 2 || (ctx->opt_plaq_variant == 0 && sizeof(T) == 4 && choice == 0);
+    if (held) {
+        nblocks = (g.V + 127) / 128;
+        int rc = lqx_ensure_partials(ctx, (size_t)nblocks);
+        if (rc) return rc;
+        {
+            LqxTimed timed(ctx, LQX_K_PLAQUETTE);
+            k_plaquette_held<T, sizeof(T) == 4 ? 3 : 1><<<nblocks, 128, 0, ctx->stream>>>(g, make_links<T>(u), ctx->d_partials);
+        }
+        LQX_LAUNCH_CHECK(ctx);
+        return lqx_sum_partials(ctx, nblocks, 1, out);
+    }
     LQX_WITH_MAP(choice, {
         const int grid = MAP::grid(g);
         nblocks = grid;

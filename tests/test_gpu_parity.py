@@ -325,9 +325,12 @@ def test_staple_smear_plaquette(lqx, dims, prec):
                 assert site_rel_err(out[mu].pop(), want[mu]) < TOL[prec], (mu, want_plaq)
             if want_plaq:
                 assert abs(p - psum_want) / max(abs(psum_want), scale) < RTOL[prec]
-        ps, pa = lqx.plaquette(fu)
-        assert abs(ps - psum_want) / max(abs(psum_want), scale) < RTOL[prec]
-        assert abs(pa - psum_want / (18.0 * lat.volume)) < RTOL[prec]
+        for variant in (0, 1, 2):  # option plaq_variant: automatic, rolled loops, the site's links held in registers
+            lat.set_option("plaq_variant", variant)
+            ps, pa = lqx.plaquette(fu)
+            assert abs(ps - psum_want) / max(abs(psum_want), scale) < RTOL[prec], variant
+            assert abs(pa - psum_want / (18.0 * lat.volume)) < RTOL[prec], variant
+        lat.set_option("plaq_variant", 0)
         # plaquette of the smeared field (A11)
         ps2, _ = lqx.plaquette(out)
         w2 = orc.plaquette_sum(dims, want, "t64" if prec == "f64" else "n64")
