@@ -112,11 +112,15 @@ __device__ __forceinline__ Mat3<T> smear_update(T c0, T c1, const Mat3<T>& umu, 
 // variant 3: the literal evaluation with the loops kept rolled (so that only one staple's operands are
 // live: 80 registers, three 256-thread CTAs per SM in fp32), the eight neighbour site indices of the
 // thread parked in shared memory and looked up by the run-time direction, and U_mu(x) fetched only
-// when it is needed instead of being held across the nu loop.  Per link: first the three upper
-// staples with nu DEscending, so that after the nu > mu ones the accumulator is exactly
-// sum_{nu>mu} upper_{mu,nu} and the plaquette terms of this link cost ONE trace
-//   sum_{nu>mu} Re tr[U_mu U_nu(x+mu) adj(U_mu(x+nu)) adj(U_nu)] = Re tr[U_mu(x) adj(acc)],
-// then the three lower staples.
+// when it is needed instead of being held across the nu loop.  Per link: the three upper staples (nu
+// DEscending, the order every variant sums in), then the three lower staples, then U_mu(x) is loaded
+// once for the update -- and for the plaquette of the input field, which costs no load of its own:
+// every staple of link mu closes one plaquette with U_mu(x) (an upper one P_munu(x), a lower one
+// P_munu(x-nu^)), and over the whole periodic lattice every plaquette is met four times, so
+//   sum_x sum_{mu<nu} Re tr P_munu(x) = (1/4) sum_x sum_mu Re tr[U_mu(x) adj(S_mu(x))]
+// (SURVEY 8(c) staple pin; exact for the GLOBAL sum only, which is all a launch reports: the ranged
+// launches of the streamed host path run with PLAQ = false).  An extra trace after the nu > mu staples, as before, re-read
+// U_mu(x) for three links: +4 % on a kernel that is bound by the L1 data pipe.
 template <typename T, bool PLAQ, typename MAP, int MINB>
 __global__ void __launch_bounds__(MAP::THREADS, MINB) k_smear_rolled(const __grid_constant__ Geo g, const __grid_constant__ TileMap tm,
                                                                      const __grid_constant__ Links<T> u, const __grid_constant__ LinksOut<T> out,
@@ -140,10 +144,7 @@ __global__ void __launch_bounds__(MAP::THREADS, MINB) k_smear_rolled(const __gri
             Mat3<T> acc = zero_mat<T>();
 #pragma unroll 1
             for (int nu = 3; nu >= 0; --nu) {  // upper: U_nu(x) U_mu(x+nu^) adj(U_nu(x+mu^))
-                if (nu == mu) {
-                    if (PLAQ && mu < 3) pl += re_tr_na(load_mat(umu_p, s), acc);
-                    continue;
-                }
+                if (nu == mu) continue;
                 const T* __restrict__ unu_p = u.u[nu];
                 const Mat3<T> t = mul_nn(load_mat(unu_p, s), load_mat(umu_p, nb[nu][tid]));
                 mac_na(acc, t, load_mat(unu_p, xpmu));
@@ -156,9 +157,11 @@ __global__ void __launch_bounds__(MAP::THREADS, MINB) k_smear_rolled(const __gri
                 const Mat3<T> t = mul_an(load_mat(unu_p, xmnu), load_mat(umu_p, xmnu));
                 mac_nn(acc, t, load_mat(unu_p, xmnu + (xpmu - s)));
             }
-            store_mat(out.u[mu], s, smear_update(c0, c1, load_mat(umu_p, s), acc));
+            const Mat3<T> umu = load_mat(umu_p, s);
+            if (PLAQ) pl += re_tr_na(umu, acc);
+            store_mat(out.u[mu], s, smear_update(c0, c1, umu, acc));
         }
-        p[0] = (double)pl;
+        p[0] = 0.25 * (double)pl;
     }
     if (PLAQ) block_reduce_partial<1>(p, partials);
 }
