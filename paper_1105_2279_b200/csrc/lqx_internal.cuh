@@ -427,6 +427,114 @@ __device__ __forceinline__ void mac_an(Mat3<T>& c, const Mat3<T>& a, const Mat3<
             c.im[i][j] = im;
         }
 }
+// --------------------------------------------------------------------------------------------
+// fp32: the same products on packed (re, im) pairs.  sm_100a has FFMA2 (PTX fma.rn.f32x2): two fp32
+// FMAs per issue slot on a 64-bit register pair, and its SASS operand forms cover a complex
+// multiply-accumulate without any data movement: a 32-bit register broadcast to both lanes (.F32),
+// the pair swapped (.LO_HI) and a per-lane sign (.NP / .PN) -- ptxas folds mov.b64 {x, x},
+// {y, x} and {-y, x} into them as long as the signed pair is the FIRST multiplicand.  So
+//     c += a*b :  c = fma2((b.re, b.im), a.re, c);  c = fma2((-b.im, b.re), a.im, c)
+// is two instructions instead of four, with the operands exactly as the 128-bit loads deliver them.
+// Same lane throughput as scalar FFMA, half the issue slots (profiles/r02a).  Every lane is an IEEE
+// fma in the order of the generic code above except that in mac_na the two im terms swap.
+// --------------------------------------------------------------------------------------------
+typedef unsigned long long f32x2_t;
+__device__ __forceinline__ f32x2_t pk2(float lo, float hi) {
+    f32x2_t d;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(d) : "f"(lo), "f"(hi));
+    return d;
+}
+__device__ __forceinline__ void upk2(f32x2_t d, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(d)); }
+__device__ __forceinline__ f32x2_t fma2(f32x2_t a, f32x2_t b, f32x2_t c) {
+    f32x2_t d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ f32x2_t mul2(f32x2_t a, f32x2_t b) {
+    f32x2_t d;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+// c += a*b, c += a*conj(b), c += conj(a)*b on c = (re, im)
+__device__ __forceinline__ f32x2_t cmac_nn(f32x2_t c, float ar, float ai, float br, float bi) {
+    c = fma2(pk2(br, bi), pk2(ar, ar), c);
+    return fma2(pk2(-bi, br), pk2(ai, ai), c);
+}
+__device__ __forceinline__ f32x2_t cmac_nc(f32x2_t c, float ar, float ai, float br, float bi) {
+    c = fma2(pk2(br, -bi), pk2(ar, ar), c);
+    return fma2(pk2(bi, br), pk2(ai, ai), c);
+}
+__device__ __forceinline__ f32x2_t cmac_cn(f32x2_t c, float ar, float ai, float br, float bi) {
+    c = fma2(pk2(br, bi), pk2(ar, ar), c);
+    return fma2(pk2(bi, -br), pk2(ai, ai), c);
+}
+// non-template overloads: chosen over the templates above for T = float
+__device__ __forceinline__ Mat3<float> mul_nn(const Mat3<float>& a, const Mat3<float>& b) {
+    Mat3<float> c;
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            f32x2_t t = mul2(pk2(b.re[0][j], b.im[0][j]), pk2(a.re[i][0], a.re[i][0]));
+            t = fma2(pk2(-b.im[0][j], b.re[0][j]), pk2(a.im[i][0], a.im[i][0]), t);
+#pragma unroll
+            for (int k = 1; k < 3; ++k) t = cmac_nn(t, a.re[i][k], a.im[i][k], b.re[k][j], b.im[k][j]);
+            upk2(t, c.re[i][j], c.im[i][j]);
+        }
+    return c;
+}
+__device__ __forceinline__ void mac_nn(Mat3<float>& c, const Mat3<float>& a, const Mat3<float>& b) {
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            f32x2_t t = pk2(c.re[i][j], c.im[i][j]);
+#pragma unroll
+            for (int k = 0; k < 3; ++k) t = cmac_nn(t, a.re[i][k], a.im[i][k], b.re[k][j], b.im[k][j]);
+            upk2(t, c.re[i][j], c.im[i][j]);
+        }
+}
+__device__ __forceinline__ void mac_na(Mat3<float>& c, const Mat3<float>& a, const Mat3<float>& b) {
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            f32x2_t t = pk2(c.re[i][j], c.im[i][j]);
+#pragma unroll
+            for (int k = 0; k < 3; ++k) t = cmac_nc(t, a.re[i][k], a.im[i][k], b.re[j][k], b.im[j][k]);
+            upk2(t, c.re[i][j], c.im[i][j]);
+        }
+}
+__device__ __forceinline__ void mac_an(Mat3<float>& c, const Mat3<float>& a, const Mat3<float>& b) {
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            f32x2_t t = pk2(c.re[i][j], c.im[i][j]);
+#pragma unroll
+            for (int k = 0; k < 3; ++k) t = cmac_cn(t, a.re[k][i], a.im[k][i], b.re[k][j], b.im[k][j]);
+            upk2(t, c.re[i][j], c.im[i][j]);
+        }
+}
+__device__ __forceinline__ void mac_mv(Vec3<float>& w, const Mat3<float>& m, const Vec3<float>& v) {
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+        f32x2_t t = pk2(w.re[i], w.im[i]);
+#pragma unroll
+        for (int j = 0; j < 3; ++j) t = cmac_nn(t, m.re[i][j], m.im[i][j], v.re[j], v.im[j]);
+        upk2(t, w.re[i], w.im[i]);
+    }
+}
+__device__ __forceinline__ void mac_adj_mv(Vec3<float>& w, const Mat3<float>& m, const Vec3<float>& v) {
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+        f32x2_t t = pk2(w.re[i], w.im[i]);
+#pragma unroll
+        for (int j = 0; j < 3; ++j) t = cmac_cn(t, m.re[j][i], m.im[j][i], v.re[j], v.im[j]);
+        upk2(t, w.re[i], w.im[i]);
+    }
+}
+
 template <typename T>
 __device__ __forceinline__ Mat3<T> zero_mat() {
     Mat3<T> c;
