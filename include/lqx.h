@@ -254,10 +254,13 @@ enum { LQX_K_SMEAR = 0, LQX_K_PLAQUETTE = 1, LQX_K_HOP = 2, LQX_K_CATALOGUE = 3,
 int lqx_kernel_time(lqx_ctx* ctx, int kernel_class, double* total_ms, int* count);
 /* Number of kernels this context has launched since init (for bench.py's gpu_launches). */
 int64_t lqx_launch_count(const lqx_ctx* ctx);
-/* Options: "smear_variant" 0 or 3 = default (rolled literal kernel), 1 = first-cut literal kernel,
+/* Options: "smear_variant" 0 = default (fp32: 9, fp64: 3), 3 = rolled literal kernel, 1 = first-cut literal kernel,
  * 2 = shared-corner kernel (36 products, lower staples exchanged through shared memory), 4 = four
- * threads per site, 6 = operands staged in shared memory with cp.async (fp32); variants fall back to 3 where
- * none of their tile shapes divides the lattice.
+ * threads per site, 6 = operands staged in shared memory with cp.async (fp32), 7 = the CTA tile's own links in
+ * shared memory and the halo through L1, 8 = plane-ordered 42-product evaluation on whole-x-row tiles, persistent
+ * double-buffered CTAs (fp32), 9 = the literal evaluation of 3 on whole-x-row tiles whose own links sit in shared
+ * memory (fp32; same summation order as 3, bit-identical); variants fall back to 3 where their tiles do not fit
+ * the lattice.
  * "tile" -1 = automatic, 0 = linear 128-site blocks, 1..6 = CTA tile shape (8x4x4x2, 8x4x2x2,
  * 4x4x4x2, 16x4x2x2, 16x2x2x2, 32x2x2x2) of the nearest-neighbour kernels, used if it divides the
  * lattice.  "jacobi_block" (32, 64, 128, 256) and "jacobi_sites" (1, 2, 4): the paper's launch

@@ -433,8 +433,26 @@ int smear_launch_t(lqx_ctx* ctx, lqx_field* const uout[4], const lqx_field* cons
     const Links<T> in = make_links<T>(uin);
     const T c0 = (T)(1.0 - alpha), c1 = (T)(alpha / 6.0);
     int variant = ctx->opt_smear_variant;
-    if (variant != 1 && variant != 2 && variant != 4 && variant != 6) variant = 3;
+    if (variant == 0 && sizeof(T) == 4) variant = 9;  // fp32 default: literal evaluation on row tiles (falls back to 3)
+    if (variant != 1 && variant != 2 && variant != 4 && variant != 6 && variant != 7 && variant != 8 && variant != 9) variant = 3;
     if (only_mu >= 0) variant = 1;
+    if (variant == 9) {
+        int rc = 1;
+        if (sizeof(T) == 4) rc = lqx_smear_rowlit_launch(ctx, reinterpret_cast<const Links<float>&>(in), reinterpret_cast<const LinksOut<float>&>(o), (float)c0, (float)c1, plaq);
+        if (rc <= 0) return rc;
+        variant = 3;
+    }
+    if (variant == 8) {
+        int rc = 1;
+        if (sizeof(T) == 4) rc = lqx_smear_rows_launch(ctx, reinterpret_cast<const Links<float>&>(in), reinterpret_cast<const LinksOut<float>&>(o), (float)c0, (float)c1, plaq);
+        if (rc <= 0) return rc;
+        variant = 3;  // fp64, or the lattice does not fit the row tiles
+    }
+    if (variant == 7) {
+        const int rc = lqx_smear_tile_launch(ctx, in, o, c0, c1, plaq);
+        if (rc <= 0) return rc;
+        variant = 3;  // no tile of this kernel divides the lattice
+    }
     if (variant == 6) {
         int rc = 1;
         if (sizeof(T) == 4) rc = lqx_smear_staged_launch(ctx, reinterpret_cast<const Links<float>&>(in), reinterpret_cast<const LinksOut<float>&>(o), (float)c0, (float)c1, plaq);

@@ -63,3 +63,15 @@ int lqx_smear_launch_range(lqx_ctx* ctx, lqx_field* const uout[4], const lqx_fie
 // lattice is not a multiple of its 8x2x2x2 tile
 int lqx_smear_staged_launch(lqx_ctx* ctx, const Links<float>& in, const LinksOut<float>& out, float c0, float c1, double* plaq);
 void lqx_staged_release(lqx_ctx* ctx);
+
+// smear step with the tile's own links in shared memory (lqx_smear_tile.cu, option "smear_variant" = 7):
+// LQX_OK, a negative status, or 1 if no tile shape of this kernel divides the lattice
+int lqx_smear_tile_launch(lqx_ctx* ctx, const Links<float>& in, const LinksOut<float>& out, float c0, float c1, double* plaq);
+int lqx_smear_tile_launch(lqx_ctx* ctx, const Links<double>& in, const LinksOut<double>& out, double c0, double c1, double* plaq);
+
+// fp32 smear step, plane-ordered 42-product evaluation on whole-x-row tiles in shared memory, persistent
+// double-buffered CTAs (lqx_smear_rows.cu, option "smear_variant" = 8): LQX_OK, a negative status, or 1 if
+// the lattice does not fit
+int lqx_smear_rows_launch(lqx_ctx* ctx, const Links<float>& in, const LinksOut<float>& out, float c0, float c1, double* plaq);
+// the literal evaluation on the same row tiles, two CTAs per SM (option "smear_variant" = 9)
+int lqx_smear_rowlit_launch(lqx_ctx* ctx, const Links<float>& in, const LinksOut<float>& out, float c0, float c1, double* plaq);

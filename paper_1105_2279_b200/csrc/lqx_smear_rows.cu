@@ -1,0 +1,491 @@
+// lqx staple sum + smear step, fp32, plane-ordered evaluation on whole-x-row tiles held in shared memory
+// (option "smear_variant" = 8, formula of BASELINE.json configs[0]).
+//
+// What bounds the literal kernel (profiles/r02b): 76 operand matrices per site through the 128 B/clk L1
+// data pipe (1986 wavefronts per warp, pipe 75 % busy: x-shifted rows of an 8-site-wide tile straddle two
+// lines, +24 %) and 39 GB per launch from L2 (12.7 TB/s, the fabric's limit).  This kernel attacks both:
+//
+//  * evaluation order: the six planes (mu < nu) one after the other with all four staple sums S_mu live.
+//    With B = U_nu(x+mu^), C = U_mu(x+nu^) the product Z = B adj(C) serves BOTH upper staples of the plane,
+//    S_nu += U_mu(x) Z and S_mu += U_nu(x) adj(Z): 3 products instead of 4, and 42 products / 64 operand
+//    fetches per site instead of 48 / 76.  (Algebra of DESIGN.md sec.6.1; the oracle stays literal.)
+//  * tile = ROWS whole x-rows (L0 x 2 x 2 x 2 sites, one thread per site), the tile's own links copied to
+//    shared memory in the blocked field layout.  x-neighbours wrap around inside the row, so they are
+//    ALWAYS in the tile and come out of shared memory at any alignment for 4 wavefronts per 128-bit chunk;
+//    y/z/t-neighbours are in the tile for half of the rows.  Each operand is fetched by a predicated pair
+//    ld.shared / ld.global.nc into the same registers: the lanes inside the tile cost shared wavefronts,
+//    the others read whole aligned rows through L1 -- no lane pays twice and nothing diverges.
+//  * persistent CTAs, one per SM, double-buffered: while tile k is multiplied the own links of tile k+1
+//    arrive by cp.async, so the fill never idles the FMA pipe and one barrier per tile suffices.
+//
+// Sums the staples of a link in plane order (not the oracle's nu-ascending order): agrees with the other
+// variants to rounding, not bit for bit.
+#include <cuda_pipeline.h>
+
+#include "lqx_smear.cuh"
+
+namespace {
+
+struct RowMap {
+    int ny, nz, nt;  // tiles per direction
+    int zs;          // z-tiles per slab: tiles are visited y, z fastest inside a slab, then t, then the next slab,
+                     // so that the +-t neighbour rows of a tile are still in L2 (as Tiled<>::site does)
+    int ntiles;
+};
+
+// One colour matrix from the tile in shared memory (in) or from the field in global memory, by GENERIC loads from a
+// selected address.  Two facts shape this: (1) a predicated pair ld.shared / ld.global into the same registers --
+// written by hand or produced by ptxas if-converting a branch -- never ends a live range, and ptxas then keeps the
+// destination registers of all 64 fetches alive at once (5.5 KB of spills per thread); (2) x-neighbours are always in
+// the tile, so a warp mixes the two spaces only where it straddles two rows with different y/z/t position.
+__device__ __forceinline__ Mat3<float> fetch_mat(unsigned long long s_link, const float* g_link, bool in, int li, int gi) {
+    const int idx = in ? li : gi;
+    const unsigned off = (unsigned)(idx >> 5) * (32u * 18u * 4u) + (unsigned)(idx & 31) * 16u;
+    const unsigned long long a = (in ? s_link : (unsigned long long)g_link) + off;
+    const unsigned half = 2048u - (unsigned)(idx & 31) * 8u;
+    float r[18];
+#pragma unroll
+    for (int q = 0; q < 4; ++q)
+        asm volatile("ld.v4.f32 {%0,%1,%2,%3}, [%4];"
+                     : "=f"(r[4 * q]), "=f"(r[4 * q + 1]), "=f"(r[4 * q + 2]), "=f"(r[4 * q + 3])
+                     : "l"(a + q * 512u));
+    asm volatile("ld.v2.f32 {%0,%1}, [%2];" : "=f"(r[16]), "=f"(r[17]) : "l"(a + half));
+    Mat3<float> m;
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            m.re[i][j] = r[2 * (3 * i + j)];
+            m.im[i][j] = r[2 * (3 * i + j) + 1];
+        }
+    return m;
+}
+// a matrix of the tile itself (always shared memory)
+__device__ __forceinline__ Mat3<float> fetch_own(unsigned long long s_link_generic, int li) {
+    const unsigned sa = (unsigned)__cvta_generic_to_shared(reinterpret_cast<const void*>(s_link_generic)) + (unsigned)(li >> 5) * (32u * 18u * 4u) + (unsigned)(li & 31) * 16u;
+    const unsigned half = 2048u - (unsigned)(li & 31) * 8u;
+    float r[18];
+#pragma unroll
+    for (int q = 0; q < 4; ++q)
+        asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];"
+                     : "=f"(r[4 * q]), "=f"(r[4 * q + 1]), "=f"(r[4 * q + 2]), "=f"(r[4 * q + 3])
+                     : "r"(sa + q * 512u));
+    asm volatile("ld.shared.v2.f32 {%0,%1}, [%2];" : "=f"(r[16]), "=f"(r[17]) : "r"(sa + half));
+    Mat3<float> m;
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            m.re[i][j] = r[2 * (3 * i + j)];
+            m.im[i][j] = r[2 * (3 * i + j) + 1];
+        }
+    return m;
+}
+
+// the four links of site s -> shared buffer slot li, asynchronously (4 x 16 B + 8 B per link)
+__device__ __forceinline__ void fill_async(float* buf, int link_floats, const Links<float>& u, int s, int li) {
+    const size_t goff = (size_t)(s >> 5) * (32 * 18) + (size_t)(s & 31) * 4;
+    const int soff = (li >> 5) * (32 * 18) + (li & 31) * 4;
+#pragma unroll
+    for (int mu = 0; mu < 4; ++mu) {
+        const float* g = u.u[mu] + goff;
+        float* d = buf + mu * link_floats + soff;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) __pipeline_memcpy_async(d + q * 128, g + q * 128, 16);
+        __pipeline_memcpy_async(d + 512 - (li & 31) * 2, g + 512 - (s & 31) * 2, 8);
+    }
+}
+
+// scheduling fence: every element of m must exist before any later (volatile) load is issued.  Without it the
+// compiler hoists the independent operand loads of all six planes to the top and spills kilobytes per thread.
+__device__ __forceinline__ void fence_mat(const Mat3<float>& m) {
+    asm volatile("" ::"f"(m.re[0][0]), "f"(m.re[0][1]), "f"(m.re[0][2]), "f"(m.re[1][0]), "f"(m.re[1][1]), "f"(m.re[1][2]),
+                 "f"(m.re[2][0]), "f"(m.re[2][1]), "f"(m.re[2][2]), "f"(m.im[0][0]), "f"(m.im[0][1]), "f"(m.im[0][2]),
+                 "f"(m.im[1][0]), "f"(m.im[1][1]), "f"(m.im[1][2]), "f"(m.im[2][0]), "f"(m.im[2][1]), "f"(m.im[2][2]));
+}
+
+
+// What a thread knows about its site, packed so that it costs four registers and not twenty-four (the kernel runs
+// at the 168-register limit of twelve warps per SM): everything else is re-derived per fetch from uniform values.
+//   mask bit d      : x+d^ is in the tile          bit 4+d  : x-d^ is in the tile
+//        bit 8+d    : x_d + 1 == L_d (x+d^ wraps)  bit 12+d : x_d == 0 (x-d^ wraps)
+struct SiteCtx {
+    int s;         // global site index
+    unsigned mask;
+    int dpx, dmx;  // tile-local index delta of x+0^ / x-0^ (the row wraps around inside the tile)
+    int row_y, row_z, row_t;  // tile-local index delta of one step in y, z, t (uniform)
+    template <int D>
+    __device__ __forceinline__ bool ip() const { return D == 0 ? true : (mask >> D) & 1u; }
+    template <int D>
+    __device__ __forceinline__ bool im() const { return D == 0 ? true : (mask >> (4 + D)) & 1u; }
+    template <int D>
+    __device__ __forceinline__ int dp() const { return D == 0 ? dpx : (D == 1 ? row_y : (D == 2 ? row_z : row_t)); }
+    template <int D>
+    __device__ __forceinline__ int dm() const { return D == 0 ? dmx : -(D == 1 ? row_y : (D == 2 ? row_z : row_t)); }
+    // global site index of x+d^ / x-d^
+    template <int D>
+    __device__ __forceinline__ int gp(const Geo& g) const {
+        return ((mask >> (8 + D)) & 1u) ? s - (g.L[D] - 1) * g.stride_site[D] : s + g.stride_site[D];
+    }
+    template <int D>
+    __device__ __forceinline__ int gm(const Geo& g) const {
+        return ((mask >> (12 + D)) & 1u) ? s + (g.L[D] - 1) * g.stride_site[D] : s - g.stride_site[D];
+    }
+};
+
+// the operands of one plane mu < nu, in the order they are consumed:
+//   B = U_nu(x+mu), C = U_mu(x+nu)                      Z = B adj(C)
+//   U_mu(x)                                             S_nu += U_mu(x) Z        upper staple of link nu
+//   U_nu(x)                                             S_mu += U_nu(x) adj(Z)   upper staple of link mu
+//   E = U_nu(x-nu), F = U_mu(x-nu), G = U_nu(x-nu+mu)   S_mu += (adj(E) F) G     lower staple of link mu
+//   E' = U_mu(x-mu), F' = U_nu(x-mu), G' = U_mu(x-mu+nu) S_nu += (adj(E') F') G' lower staple of link nu
+// The loads of every product are issued BEFORE the FMAs of the product in front of it (one product of
+// prefetch); fence_mat pins that order.  B and C of the next plane are fetched during this plane's last product.
+template <int MU, int NU>
+__device__ __forceinline__ void fetch_BC(Mat3<float>& B, Mat3<float>& C, const SiteCtx& c, int li, const unsigned long long (&sl)[4],
+                                         const Links<float>& u, const Geo& g) {
+    B = fetch_mat(sl[NU], u.u[NU], c.ip<MU>(), li + c.dp<MU>(), c.gp<MU>(g));
+    C = fetch_mat(sl[MU], u.u[MU], c.ip<NU>(), li + c.dp<NU>(), c.gp<NU>(g));
+}
+
+template <int MU, int NU, int MU2, int NU2>
+__device__ __forceinline__ void plane(Mat3<float> (&S)[4], Mat3<float>& B, Mat3<float>& C, const SiteCtx& c, int li,
+                                      const unsigned long long (&sl)[4], const Links<float>& u, const Geo& g) {
+    // Software pipeline, one product deep: the operand(s) of the next product are requested, then __syncwarp() --
+    // a memory-ordering point ptxas will not sink loads across (left alone it moves every load down to its first
+    // use to save registers, and twelve warps per SM cannot cover an L2 round trip per operand) -- then the FMAs of
+    // the current product.  Four operand matrices live beside the four staple sums at the widest point.
+    const Mat3<float> Amu = fetch_own(sl[MU], li);
+    __syncwarp();
+    const Mat3<float> Z = mul_na(B, C);
+    fence_mat(Z);
+    const Mat3<float> Anu = fetch_own(sl[NU], li);
+    __syncwarp();
+    mac_nn(S[NU], Amu, Z);
+    fence_mat(S[NU]);
+    const Mat3<float> E = fetch_mat(sl[NU], u.u[NU], c.im<NU>(), li + c.dm<NU>(), c.gm<NU>(g));
+    const Mat3<float> F = fetch_mat(sl[MU], u.u[MU], c.im<NU>(), li + c.dm<NU>(), c.gm<NU>(g));
+    __syncwarp();
+    mac_na(S[MU], Anu, Z);
+    fence_mat(S[MU]);
+    const Mat3<float> G = fetch_mat(sl[NU], u.u[NU], c.im<NU>() && c.ip<MU>(), li + c.dm<NU>() + c.dp<MU>(), c.gm<NU>(g) + (c.gp<MU>(g) - c.s));
+    __syncwarp();
+    const Mat3<float> t = mul_an(E, F);
+    fence_mat(t);
+    const Mat3<float> E2 = fetch_mat(sl[MU], u.u[MU], c.im<MU>(), li + c.dm<MU>(), c.gm<MU>(g));
+    const Mat3<float> F2 = fetch_mat(sl[NU], u.u[NU], c.im<MU>(), li + c.dm<MU>(), c.gm<MU>(g));
+    __syncwarp();
+    mac_nn(S[MU], t, G);
+    fence_mat(S[MU]);
+    const Mat3<float> G2 = fetch_mat(sl[MU], u.u[MU], c.im<MU>() && c.ip<NU>(), li + c.dm<MU>() + c.dp<NU>(), c.gm<MU>(g) + (c.gp<NU>(g) - c.s));
+    __syncwarp();
+    const Mat3<float> t2 = mul_an(E2, F2);
+    fence_mat(t2);
+    constexpr int M2 = MU2 >= 0 ? MU2 : 0, N2 = NU2 >= 0 ? NU2 : 1;
+    if (MU2 >= 0) {
+        B = fetch_mat(sl[N2], u.u[N2], c.ip<M2>(), li + c.dp<M2>(), c.gp<M2>(g));
+        C = fetch_mat(sl[M2], u.u[M2], c.ip<N2>(), li + c.dp<N2>(), c.gp<N2>(g));
+        __syncwarp();
+    }
+    mac_nn(S[NU], t2, G2);
+    fence_mat(S[NU]);
+}
+
+template <bool PLAQ, int RY, int RZ, int RT, int MAXT>
+__global__ void __launch_bounds__(MAXT, 1) k_smear_rows(const __grid_constant__ Geo g, const __grid_constant__ RowMap rm,
+                                                        const __grid_constant__ Links<float> u, const __grid_constant__ LinksOut<float> out,
+                                                        float c0, float c1, double* __restrict__ partials) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int L0 = g.L[0];
+    const int nthr = blockDim.x;  // L0 * RY * RZ * RT
+    const int npad = (nthr + 31) & ~31;
+    const int link_floats = 18 * npad;
+    float* const buf0 = reinterpret_cast<float*>(smem_raw);
+    const int li = threadIdx.x;
+    const int lx = li % L0, row = li / L0;
+    const int ly = row % RY, lz = (row / RY) % RZ, lt = row / (RY * RZ);
+
+    SiteCtx c;
+    // tile-local deltas and in-tile flags do not depend on the tile; x-neighbours wrap around inside the row
+    c.dpx = (lx + 1 == L0) ? -(L0 - 1) : 1;
+    c.dmx = (lx == 0) ? (L0 - 1) : -1;
+    c.row_y = L0, c.row_z = RY * L0, c.row_t = RY * RZ * L0;
+    const unsigned tile_mask = (ly + 1 < RY ? 2u : 0u) | (lz + 1 < RZ ? 4u : 0u) | (lt + 1 < RT ? 8u : 0u) | (ly > 0 ? 32u : 0u) |
+                               (lz > 0 ? 64u : 0u) | (lt > 0 ? 128u : 0u);
+
+    const int per_slab = rm.ny * rm.zs * rm.nt;
+    auto site_of = [&](int tile, int (&x)[4]) {
+        const int k = tile / per_slab;
+        int rem = tile - k * per_slab;
+        const int bt = rem / (rm.ny * rm.zs);
+        rem -= bt * (rm.ny * rm.zs);
+        const int bz = rem / rm.ny + k * rm.zs, by = rem % rm.ny;
+        x[0] = lx, x[1] = RY * by + ly, x[2] = RZ * bz + lz, x[3] = RT * bt + lt;
+        return x[0] + g.L[0] * (x[1] + g.L[1] * (x[2] + g.L[2] * x[3]));
+    };
+
+    float pl = 0.f;
+    int tile = blockIdx.x;
+    int cur = 0;
+    if (tile < rm.ntiles) {
+        int x[4];
+        const int s = site_of(tile, x);
+        fill_async(buf0, link_floats, u, s, li);
+    }
+    __pipeline_commit();
+    for (; tile < rm.ntiles; tile += gridDim.x, cur ^= 1) {
+        int x[4];
+        c.s = site_of(tile, x);
+        c.mask = tile_mask;
+#pragma unroll
+        for (int d = 0; d < 4; ++d) {
+            if (x[d] + 1 == g.L[d]) c.mask |= 1u << (8 + d);
+            if (x[d] == 0) c.mask |= 1u << (12 + d);
+        }
+        __pipeline_wait_prior(0);
+        __syncthreads();  // buffer `cur` is complete, and every thread is done with buffer cur^1
+        {
+            const int next = tile + gridDim.x;
+            if (next < rm.ntiles) {
+                int xn[4];
+                const int sn = site_of(next, xn);
+                fill_async(buf0 + (cur ^ 1) * 4 * link_floats, link_floats, u, sn, li);
+            }
+            __pipeline_commit();
+        }
+        unsigned long long sl[4];  // generic addresses of the four links of the current buffer
+#pragma unroll
+        for (int mu = 0; mu < 4; ++mu) sl[mu] = (unsigned long long)(buf0 + (cur * 4 + mu) * link_floats);
+
+        Mat3<float> S[4];
+#pragma unroll
+        for (int mu = 0; mu < 4; ++mu) S[mu] = zero_mat<float>();
+        Mat3<float> B, C;
+        fetch_BC<0, 1>(B, C, c, li, sl, u, g);
+        plane<0, 1, 0, 2>(S, B, C, c, li, sl, u, g);
+        plane<0, 2, 0, 3>(S, B, C, c, li, sl, u, g);
+        plane<0, 3, 1, 2>(S, B, C, c, li, sl, u, g);
+        plane<1, 2, 1, 3>(S, B, C, c, li, sl, u, g);
+        plane<1, 3, 2, 3>(S, B, C, c, li, sl, u, g);
+        plane<2, 3, -1, -1>(S, B, C, c, li, sl, u, g);
+#pragma unroll
+        for (int mu = 0; mu < 4; ++mu) {
+            const Mat3<float> umu = fetch_own(sl[mu], li);
+            if (PLAQ) pl += re_tr_na(umu, S[mu]);
+            Mat3<float> r;
+#pragma unroll
+            for (int i = 0; i < 3; ++i)
+#pragma unroll
+                for (int j = 0; j < 3; ++j) {
+                    r.re[i][j] = fmaf(c1, S[mu].re[i][j], c0 * umu.re[i][j]);
+                    r.im[i][j] = fmaf(c1, S[mu].im[i][j], c0 * umu.im[i][j]);
+                }
+            store_mat(out.u[mu], c.s, r);
+        }
+    }
+    __pipeline_wait_prior(0);
+    if (PLAQ) {
+        double p[1] = {0.25 * (double)pl};
+        block_reduce_partial<1>(p, partials);
+    }
+}
+
+// --------------------------------------------------------------------------------------------------------------
+// Variant 9: the LITERAL evaluation (rolled loops, 48 products, the summation order of k_smear_rolled -- bit-identical
+// to it) on the same whole-x-row tiles: 80 registers, two 384-thread CTAs per SM (24 warps, each CTA's fill overlaps the
+// other's products), the tile's own links in shared memory, the halo through L2.
+// --------------------------------------------------------------------------------------------------------------
+template <bool PLAQ, int RY, int RZ, int RT, int MAXT, int MINB>
+__global__ void __launch_bounds__(MAXT, MINB) k_smear_rowlit(const __grid_constant__ Geo g, const __grid_constant__ RowMap rm,
+                                                          const __grid_constant__ Links<float> u, const __grid_constant__ LinksOut<float> out,
+                                                          float c0, float c1, double* __restrict__ partials) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int L0 = g.L[0];
+    const int nthr = blockDim.x;
+    const int npad = (nthr + 31) & ~31;
+    const int link_floats = 18 * npad;
+    float* const buf0 = reinterpret_cast<float*>(smem_raw);
+    const int li = threadIdx.x;
+    const int lx = li % L0, row = li / L0;
+    const int ly = row % RY, lz = (row / RY) % RZ, lt = row / (RY * RZ);
+    int x[4];
+    int s;
+    {
+        const int tile = blockIdx.x;
+        const int per_slab = rm.ny * rm.zs * rm.nt;
+        const int k = tile / per_slab;
+        int rem = tile - k * per_slab;
+        const int bt = rem / (rm.ny * rm.zs);
+        rem -= bt * (rm.ny * rm.zs);
+        const int bz = rem / rm.ny + k * rm.zs, by = rem % rm.ny;
+        x[0] = lx, x[1] = RY * by + ly, x[2] = RZ * bz + lz, x[3] = RT * bt + lt;
+        s = x[0] + g.L[0] * (x[1] + g.L[1] * (x[2] + g.L[2] * x[3]));
+    }
+    fill_async(buf0, link_floats, u, s, li);
+    __pipeline_commit();
+    unsigned mask = (ly + 1 < RY ? 2u : 0u) | (lz + 1 < RZ ? 4u : 0u) | (lt + 1 < RT ? 8u : 0u) | (ly > 0 ? 32u : 0u) |
+                    (lz > 0 ? 64u : 0u) | (lt > 0 ? 128u : 0u) | 17u;  // x-neighbours are always in the tile
+#pragma unroll
+    for (int d = 0; d < 4; ++d) {
+        if (x[d] + 1 == g.L[d]) mask |= 1u << (8 + d);
+        if (x[d] == 0) mask |= 1u << (12 + d);
+    }
+    const int dpx = (lx + 1 == L0) ? -(L0 - 1) : 1, dmx = (lx == 0) ? (L0 - 1) : -1;
+    // tile-local index delta, global site index of a neighbour, for a run-time direction
+    auto dloc = [&](int d, bool fwd) {
+        const int r = d == 1 ? L0 : (d == 2 ? RY * L0 : RY * RZ * L0);
+        return d == 0 ? (fwd ? dpx : dmx) : (fwd ? r : -r);
+    };
+    auto gnb = [&](int d, bool fwd) {
+        const int wrap = (g.L[d] - 1) * g.stride_site[d];
+        if (fwd) return ((mask >> (8 + d)) & 1u) ? s - wrap : s + g.stride_site[d];
+        return ((mask >> (12 + d)) & 1u) ? s + wrap : s - g.stride_site[d];
+    };
+    __pipeline_wait_prior(0);
+    __syncthreads();
+
+    float pl = 0.f;
+#pragma unroll 1
+    for (int mu = 0; mu < 4; ++mu) {
+        const float* umu_g = u.u[mu];
+        const unsigned long long umu_t = (unsigned long long)(buf0 + mu * link_floats);
+        const int xpmu = gnb(mu, true);
+        const bool in_pmu = (mask >> mu) & 1u;
+        const int d_pmu = dloc(mu, true);
+        Mat3<float> acc = zero_mat<float>();
+#pragma unroll 1
+        for (int nu = 3; nu >= 0; --nu) {  // upper: U_nu(x) U_mu(x+nu^) adj(U_nu(x+mu^))
+            if (nu == mu) continue;
+            const float* unu_g = u.u[nu];
+            const unsigned long long unu_t = (unsigned long long)(buf0 + nu * link_floats);
+            const bool in_pnu = (mask >> nu) & 1u;
+            const Mat3<float> t = mul_nn(fetch_own(unu_t, li), fetch_mat(umu_t, umu_g, in_pnu, li + dloc(nu, true), gnb(nu, true)));
+            mac_na(acc, t, fetch_mat(unu_t, unu_g, in_pmu, li + d_pmu, xpmu));
+        }
+#pragma unroll 1
+        for (int nu = 0; nu < 4; ++nu) {  // lower: adj(U_nu(x-nu^)) U_mu(x-nu^) U_nu(x-nu^+mu^)
+            if (nu == mu) continue;
+            const float* unu_g = u.u[nu];
+            const unsigned long long unu_t = (unsigned long long)(buf0 + nu * link_floats);
+            const bool in_mnu = (mask >> (4 + nu)) & 1u;
+            const int xmnu = gnb(nu, false);
+            const int l1 = li + dloc(nu, false);
+            const Mat3<float> t = mul_an(fetch_mat(unu_t, unu_g, in_mnu, l1, xmnu), fetch_mat(umu_t, umu_g, in_mnu, l1, xmnu));
+            mac_nn(acc, t, fetch_mat(unu_t, unu_g, in_mnu && in_pmu, l1 + d_pmu, xmnu + (xpmu - s)));
+        }
+        const Mat3<float> umu = fetch_own(umu_t, li);
+        if (PLAQ) pl += re_tr_na(umu, acc);
+        Mat3<float> r;
+#pragma unroll
+        for (int i = 0; i < 3; ++i)
+#pragma unroll
+            for (int j = 0; j < 3; ++j) {
+                r.re[i][j] = fmaf(c1, acc.re[i][j], c0 * umu.re[i][j]);
+                r.im[i][j] = fmaf(c1, acc.im[i][j], c0 * umu.im[i][j]);
+            }
+        store_mat(out.u[mu], s, r);
+    }
+    if (PLAQ) {
+        double p[1] = {0.25 * (double)pl};
+        block_reduce_partial<1>(p, partials);
+    }
+}
+
+template <int RY, int RZ, int RT, int MAXT, int MINB>
+int rowlit_launch(lqx_ctx* ctx, const Links<float>& in, const LinksOut<float>& out, float c0, float c1, double* plaq) {
+    const Geo& g = ctx->geo;
+    const int nthr = g.L[0] * RY * RZ * RT;
+    if (nthr > MAXT || g.L[1] % RY || g.L[2] % RZ || g.L[3] % RT || (size_t)g.Vpad * 72 >= ((size_t)1 << 32)) return 1;
+    RowMap rm;
+    rm.ny = g.L[1] / RY, rm.nz = g.L[2] / RZ, rm.nt = g.L[3] / RT;
+    rm.ntiles = rm.ny * rm.nz * rm.nt;
+    int target = ctx->opt_block > 0 ? ctx->opt_block : kSlabZ;
+    rm.zs = 1;
+    for (int z = 1; z <= rm.nz; ++z)
+        if (rm.nz % z == 0 && z * RZ <= target) rm.zs = z;
+    const int npad = (nthr + 31) & ~31;
+    const size_t smem = (size_t)4 * 18 * npad * sizeof(float);
+    const int grid = rm.ntiles;
+    if (plaq) LQX_CUDA(ctx, cudaFuncSetAttribute(k_smear_rowlit<true, RY, RZ, RT, MAXT, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    else LQX_CUDA(ctx, cudaFuncSetAttribute(k_smear_rowlit<false, RY, RZ, RT, MAXT, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    if (plaq) {
+        int rc = lqx_ensure_partials(ctx, (size_t)grid);
+        if (rc) return rc;
+    }
+    {
+        LqxTimed timed(ctx, LQX_K_SMEAR);
+        if (plaq) k_smear_rowlit<true, RY, RZ, RT, MAXT, MINB><<<grid, nthr, smem, ctx->stream>>>(g, rm, in, out, c0, c1, ctx->d_partials);
+        else k_smear_rowlit<false, RY, RZ, RT, MAXT, MINB><<<grid, nthr, smem, ctx->stream>>>(g, rm, in, out, c0, c1, nullptr);
+    }
+    LQX_LAUNCH_CHECK(ctx);
+    return plaq ? lqx_sum_partials(ctx, grid, 1, plaq) : LQX_OK;
+}
+
+template <int RY, int RZ, int RT, int MAXT>
+int rows_launch(lqx_ctx* ctx, const Links<float>& in, const LinksOut<float>& out, float c0, float c1, double* plaq) {
+    const Geo& g = ctx->geo;
+    const int nthr = g.L[0] * RY * RZ * RT;
+    if (nthr > MAXT || g.L[1] % RY || g.L[2] % RZ || g.L[3] % RT || (size_t)g.Vpad * 72 >= ((size_t)1 << 32)) return 1;
+    RowMap rm;
+    rm.ny = g.L[1] / RY, rm.nz = g.L[2] / RZ, rm.nt = g.L[3] / RT;
+    rm.ntiles = rm.ny * rm.nz * rm.nt;
+    // slab thickness in z: the largest divisor of nz that keeps a slab at most kSlabZ sites thick
+    int target = ctx->opt_block > 0 ? ctx->opt_block : kSlabZ;
+    rm.zs = 1;
+    for (int z = 1; z <= rm.nz; ++z)
+        if (rm.nz % z == 0 && z * RZ <= target) rm.zs = z;
+    const int npad = (nthr + 31) & ~31;
+    const size_t smem = 2 * (size_t)4 * 18 * npad * sizeof(float);
+    if (smem > 227 * 1024) return 1;
+    const int grid = std::min(rm.ntiles, ctx->num_sms);
+    if (plaq) LQX_CUDA(ctx, cudaFuncSetAttribute(k_smear_rows<true, RY, RZ, RT, MAXT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    else LQX_CUDA(ctx, cudaFuncSetAttribute(k_smear_rows<false, RY, RZ, RT, MAXT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    if (plaq) {
+        int rc = lqx_ensure_partials(ctx, (size_t)grid);
+        if (rc) return rc;
+    }
+    {
+        LqxTimed timed(ctx, LQX_K_SMEAR);
+        if (plaq) k_smear_rows<true, RY, RZ, RT, MAXT><<<grid, nthr, smem, ctx->stream>>>(g, rm, in, out, c0, c1, ctx->d_partials);
+        else k_smear_rows<false, RY, RZ, RT, MAXT><<<grid, nthr, smem, ctx->stream>>>(g, rm, in, out, c0, c1, nullptr);
+    }
+    LQX_LAUNCH_CHECK(ctx);
+    return plaq ? lqx_sum_partials(ctx, grid, 1, plaq) : LQX_OK;
+}
+
+}  // namespace
+
+// LQX_OK, a negative status, or 1 if the lattice does not fit this kernel.  Option "tile" picks the rows of a tile:
+// 1 = 2x3x1 (y, z, t; 6 rows), 2 = 3x2x1, 3 = 2x2x2 (8 rows), 4 = 2x1x3, 5 = 1x2x3; automatic = the first that fits
+int lqx_smear_rows_launch(lqx_ctx* ctx, const Links<float>& in, const LinksOut<float>& out, float c0, float c1, double* plaq) {
+    const int t = ctx->opt_tile;
+    int rc = 1;
+    if (t == 1 || t <= 0) rc = rows_launch<2, 3, 1, 288>(ctx, in, out, c0, c1, plaq);
+    if (rc != 1) return rc;
+    if (t == 2 || t <= 0) rc = rows_launch<3, 2, 1, 288>(ctx, in, out, c0, c1, plaq);
+    if (rc != 1) return rc;
+    if (t == 3 || t <= 0) rc = rows_launch<2, 2, 2, 384>(ctx, in, out, c0, c1, plaq);
+    if (rc != 1) return rc;
+    if (t == 4) rc = rows_launch<2, 1, 3, 288>(ctx, in, out, c0, c1, plaq);
+    if (rc != 1) return rc;
+    if (t == 5) rc = rows_launch<1, 2, 3, 288>(ctx, in, out, c0, c1, plaq);
+    return rc;
+}
+
+// variant 9 (literal evaluation on row tiles).  Option "tile": 1 = 2x2x2 rows (8), 2 = 2x2x1 (4 rows), 3 = 2x1x2, 4 = 1x2x2
+int lqx_smear_rowlit_launch(lqx_ctx* ctx, const Links<float>& in, const LinksOut<float>& out, float c0, float c1, double* plaq) {
+    const int t = ctx->opt_tile;
+    int rc = 1;
+    if (t == 1 || t <= 0) rc = rowlit_launch<2, 2, 2, 384, 2>(ctx, in, out, c0, c1, plaq);
+    if (rc != 1) return rc;
+    if (t == 2 || t <= 0) rc = rowlit_launch<2, 2, 1, 192, 4>(ctx, in, out, c0, c1, plaq);
+    if (rc != 1) return rc;
+    if (t == 3) rc = rowlit_launch<2, 2, 1, 192, 3>(ctx, in, out, c0, c1, plaq);
+    if (rc != 1) return rc;
+    if (t == 4) rc = rowlit_launch<2, 3, 1, 288, 2>(ctx, in, out, c0, c1, plaq);
+    if (rc != 1) return rc;
+    if (t == 5) rc = rowlit_launch<3, 2, 1, 288, 2>(ctx, in, out, c0, c1, plaq);
+    if (rc != 1) return rc;
+    if (t == 6) rc = rowlit_launch<2, 2, 2, 384, 1>(ctx, in, out, c0, c1, plaq);
+    return rc;
+}

@@ -339,12 +339,13 @@ def test_staple_smear_plaquette(lqx, dims, prec):
 
 # every smear kernel variant (option "smear_variant": 1 literal gather, 2 shared-corner with the lower
 # staples exchanged through shared memory, 3 rolled literal = default, 4 four threads per site, 6 operands
-# staged in shared memory) and every
+# staged in shared memory, 7 the tile's own links in shared memory and the halo through L1, 8 plane-ordered 42-product evaluation on
+# whole-x-row tiles in shared memory with persistent double-buffered CTAs) and every
 # CTA tile shape that divides the lattice, against the truth oracle; 16x8x4x4 spans several tiles in every
 # direction for all shapes, 8x4x4x2 is exactly one 8x4x4x2 tile (every neighbour wraps into the same tile)
 @pytest.mark.parametrize("dims", [(16, 8, 4, 4), (8, 4, 4, 2), (4, 4, 4, 4)])
 @pytest.mark.parametrize("prec", ["f32", "f64"])
-@pytest.mark.parametrize("variant", [1, 2, 3, 4, 6])
+@pytest.mark.parametrize("variant", [1, 2, 3, 4, 6, 7, 8, 9])
 def test_smear_variants_and_tiles(lqx, dims, prec, variant):
     tv = orc.truth_variant(prec)
     u = _links(5, dims, prec)
@@ -369,7 +370,7 @@ def test_smear_variants_and_tiles(lqx, dims, prec, variant):
             lqx.smear_step(out, fu, 0.5, want_plaq_in=True)
             for mu in range(4):
                 assert np.array_equal(out[mu].pop(), got[mu]), (variant, tile, mu)
-            if variant in (1, 3, 6):  # variant 6 adds its staples in variant 3's order; variant 2 sums in an order that depends on the tile faces; 2 and 4 fall back to 3 for tiles they lack
+            if variant in (1, 3, 6, 7, 9):  # variants 6 and 7 add their staples in variant 3's order; variant 2 sums in an order that depends on the tile faces; 2 and 4 fall back to 3 for tiles they lack
                 if first is None:
                     first = got
                 for mu in range(4):
