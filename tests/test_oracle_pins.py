@@ -479,14 +479,125 @@ def test_sum_of_constant_field():
 
 # ------------------------------------------------------------------------------- E0/E3/E4 pieces
 @pytest.mark.parametrize("variant", ["n32", "n64"])
-def test_axpy_scale_divide_elementwise(variant):
-    dims = (2, 4, 2, 4)
+@pytest.mark.parametrize("kind", ["f", "cv"])
+def test_axpy_and_divide_compose_to_one_jacobi_iteration(variant, kind):
+    """Two code paths of the oracle: Listing 1 with iter = 1 (orc_jacobi_smear) is, line by line, E1/E2 (the hop),
+    E3 `chi = s_0 + kappa*h` and E4 `chi /= norm`.  Built from the separate routines hop, axpy
+    and divide it must give the same numbers BIT FOR BIT in the native variants; a wrong operand order or sign in
+    axpy (s_0 and h swapped, kappa on the wrong term) or a multiply in divide misses by O(1)."""
+    dims = (4, 2, 6, 2)
     dt = np.float32 if variant == "n32" else np.float64
-    a, b = gauss(8, 0, dims, "f").astype(dt), gauss(8, 1, dims, "f").astype(dt)
-    k = dt(0.17)
-    assert np.array_equal(orc.axpy(dims, a, 0.17, b, variant), a + k * b)
-    assert np.array_equal(orc.scale(dims, 0.17, a, variant), k * a)
-    assert np.array_equal(orc.divide(dims, 0.17, a, variant), a / k)
+    u = [t.astype(dt) for t in links(6, dims)]
+    chi = gauss(6, 3, dims, kind).astype(dt)
+    kappa, norm = 0.23, 1.9
+    whole = orc.jacobi_smear(dims, u, chi, kappa, 1, -1, norm, variant)
+    pieces = orc.divide(dims, norm, orc.axpy(dims, chi, kappa, orc.hop(dims, u, chi, variant), variant), variant)
+    assert np.array_equal(whole, pieces)
+    # iter = 0 is E4 alone
+    assert np.array_equal(orc.jacobi_smear(dims, u, chi, kappa, 0, -1, norm, variant), orc.divide(dims, norm, chi, variant))
+
+
+@pytest.mark.parametrize("variant", ["n32", "n64", "t32", "t64"])
+def test_scale_against_divide_and_linearity(variant):
+    """scale(1/n) and divide(n) are the same map up to one rounding of 1/n and one of the product (reading A22);
+    divide by a power of two is exact; axpy is linear in kappa: axpy(a, 2k, b) - axpy(a, k, b) = k*b up to rounding,
+    axpy(a, 0, b) = a exactly, axpy(0, 1, b) = b exactly."""
+    dims = (2, 4, 2, 4)
+    a, b = (gauss(8, k, dims, "f").astype(np.float32 if variant.endswith("32") else np.float64) for k in (0, 1))
+    # scalars are rounded once to the FIELD precision in every variant, so 1/n and n carry fp32 roundings in t32 too
+    eps = 2.0 ** -23 if variant.endswith("32") else 2.0 ** -52
+    n = 1.7
+    s, d = orc.scale(dims, 1.0 / n, a, variant).astype(np.float64), orc.divide(dims, n, a, variant).astype(np.float64)
+    assert np.abs(s - d).max() <= 2.5 * eps * np.abs(d).max()
+    assert np.array_equal(orc.divide(dims, 4.0, a, variant), orc.scale(dims, 0.25, a, variant))
+    assert np.array_equal(orc.divide(dims, 4.0, a, variant).astype(np.float64), a.astype(np.float64) / 4.0)
+    assert np.array_equal(orc.axpy(dims, a, 0.0, b, variant).astype(np.float64), a.astype(np.float64))
+    assert np.array_equal(orc.axpy(dims, np.zeros_like(a), 1.0, b, variant).astype(np.float64), b.astype(np.float64))
+    k = 0.375  # exactly representable, so k*b is one rounding
+    diff = orc.axpy(dims, a, 2 * k, b, variant).astype(np.float64) - orc.axpy(dims, a, k, b, variant).astype(np.float64)
+    assert np.abs(diff - k * b.astype(np.float64)).max() <= 4 * eps * (np.abs(a).max() + np.abs(b).max())
+
+
+# ------------------------------------------------------------------------------- a10: the trajectory driver
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+def test_smear_iterate_on_unit_links_is_constant(prec):
+    """unit links are a fixed point of the step (S = 6, U' = U): every plaquette average is exactly 1 and the
+    field never changes, however many steps."""
+    dims = (4, 2, 4, 2)
+    u = links(0, dims, prec, "unit")
+    out, plaqs = orc.smear_iterate(dims, u, 0.5, 4, prec)
+    if prec == "f64":
+        assert plaqs == [1.0, 1.0, 1.0, 1.0]
+        for mu in range(4):
+            assert np.array_equal(out[mu], u[mu])
+    else:
+        # Step 1 runs in the truth variant of fp32, whose a/6 is rounded to fp32 (reading A10): 6 * c1 = 0.5 (1 + 3e-8),
+        # so the links become 1 + d with d = 6 c1 - 0.5.  The later steps run in fp64 with the exact coefficient (A23),
+        # where U = 1 + d maps to 1 + 2 d (the fixed point has eigenvalue 2): d doubles per step.  This pins the
+        # driver's switch of variant after the first step -- without it d would grow as 2^k - 1.
+        d1 = 6.0 * float(np.float32(0.5 / 6.0)) - 0.5
+        for k, p in enumerate(plaqs):
+            assert abs(p - (1.0 + d1 * 2 ** k) ** 4) < 1e-12, k
+        for mu in range(4):
+            assert np.abs(out[mu] - (1.0 + d1 * 8) * u[mu]).max() < 1e-12
+
+
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+def test_smear_iterate_with_alpha_zero_is_constant(prec):
+    """alpha = 0: U' = U, so the trajectory is constant and every reported plaquette is the input's."""
+    dims = (2, 4, 2, 4)
+    u = links(3, dims, prec)
+    out, plaqs = orc.smear_iterate(dims, u, 0.0, 3, prec)
+    p0 = orc.plaquette_avg(dims, u, orc.truth_variant(prec))
+    assert all(abs(p - p0) < 1e-14 for p in plaqs)
+    for mu in range(4):
+        assert np.array_equal(out[mu].astype(np.float64), u[mu].astype(np.float64))
+
+
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+def test_smear_iterate_equals_explicit_steps(prec):
+    """The driver is n explicit smear_step calls with the plaquette of each OUTPUT (reading A11 for configs[3]):
+    the plaquette reported for step k is that of the field AFTER step k, not before it, and the links returned are
+    those after the last step.  Rebuilt here from smear_step / plaquette_avg calls written out one by one; the first
+    step starts from the storage-precision field with wide arithmetic, the later ones stay in fp64 (A23)."""
+    dims = (4, 4, 2, 6)
+    u0 = links(4, dims, prec, "near_unit")
+    out, plaqs = orc.smear_iterate(dims, u0, 0.5, 3, prec)
+    tv = orc.truth_variant(prec)
+    later = "t64" if prec == "f64" else "n64"
+    u1 = orc.smear_step(dims, u0, 0.5, tv)
+    u2 = orc.smear_step(dims, u1, 0.5, later)
+    u3 = orc.smear_step(dims, u2, 0.5, later)
+    want = [orc.plaquette_avg(dims, u1, later), orc.plaquette_avg(dims, u2, later), orc.plaquette_avg(dims, u3, later)]
+    assert plaqs == want
+    for mu in range(4):
+        assert np.array_equal(out[mu], u3[mu])
+    # and none of the reported values is the plaquette BEFORE its step
+    before = [orc.plaquette_avg(dims, u0, tv), want[0], want[1]]
+    assert all(abs(p - b) > 1e-3 for p, b in zip(plaqs, before))
+    # one step of the driver = smear_step + plaquette_avg of its output
+    out1, p1 = orc.smear_iterate(dims, u0, 0.5, 1, prec)
+    assert p1 == [want[0]] and all(np.array_equal(a, b) for a, b in zip(out1, u1))
+
+
+def test_smear_iterate_plaquette_is_gauge_invariant_and_matches_numpy():
+    """the whole trajectory of plaquettes is invariant under a gauge transformation of the start (the step is gauge
+    covariant), and the first value equals a numpy-roll evaluation of the plaquette of smear_step's output."""
+    dims = (4, 2, 2, 4)
+    u = links(5, dims, "f64", "near_unit")
+    g = cplx(li.gauge_field(9, dims, "f64", "haar")[0].numpy())
+    ug = [real2(t) for t in gauge_transform_links([cplx(t) for t in u], g, dims)]
+    _, p = orc.smear_iterate(dims, u, 0.5, 3, "f64")
+    _, pg = orc.smear_iterate(dims, ug, 0.5, 3, "f64")
+    assert np.allclose(p, pg, rtol=0, atol=1e-13)
+    u1 = [cplx(t) for t in orc.smear_step(dims, u, 0.5, "t64")]
+    tot = 0.0
+    for mu in range(4):
+        for nu in range(mu + 1, 4):
+            a = np.einsum("xij,xjk->xik", u1[mu], roll_site(u1[nu], dims, +1, mu))
+            b = np.einsum("xij,xjk->xik", u1[nu], roll_site(u1[mu], dims, +1, nu))
+            tot += np.einsum("xij,xij->", a, b.conj()).real
+    assert abs(p[0] - tot / (18.0 * vol(dims))) < 1e-13
 
 
 # ------------------------------------------------------------------------------- variants agree
