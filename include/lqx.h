@@ -107,7 +107,8 @@ int lqx_field_prec(const lqx_field* f);
 int lqx_field_push(lqx_field* f, const void* host_qdp_order);
 /* device blocked SoA -> host QDP order.  Synchronises.  Bit-exact.  Does not free (reading A4). */
 int lqx_field_pop(const lqx_field* f, void* host_qdp_order);
-/* Same converters between two DEVICE buffers (dev_qdp_order: V*2*kind reals, AoS). Asynchronous. */
+/* Same converters between two DEVICE buffers (dev_qdp_order: V*2*kind reals, AoS, 16-byte aligned -- LQX_EINVAL
+ * otherwise: the converter moves 128-bit words). Asynchronous. */
 int lqx_field_import_dev(lqx_field* f, const void* dev_qdp_order);
 int lqx_field_export_dev(const lqx_field* f, void* dev_qdp_order);
 

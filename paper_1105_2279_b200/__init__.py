@@ -36,9 +36,19 @@ def _load():
     if not os.path.exists(path) or _build._stale(path, [os.path.join(_build.CSRC, s) for s in _build.SOURCES] + _build.HEADERS):
         try:
             path = _build.build()
-        except Exception as e:  # no nvcc on this machine: use the shipped .so if there is one
+        except Exception as e:
+            # never run kernels that do not match the sources under review without saying so: a stale library is
+            # loaded only on explicit request (LQX_ALLOW_STALE=1), and then loudly
             if not os.path.exists(_build.LIB):
                 raise ImportError(f"liblqx.so is missing and could not be built: {e}") from e
+            if os.environ.get("LQX_ALLOW_STALE") != "1":
+                raise ImportError(f"liblqx.so is older than csrc/ and could not be rebuilt ({e}); "
+                                  "set LQX_ALLOW_STALE=1 to load it anyway") from e
+            import time
+            import warnings
+
+            warnings.warn("loading a STALE liblqx.so (built %s) although csrc/ is newer: %s"
+                          % (time.ctime(os.path.getmtime(_build.LIB)), e))
             path = _build.LIB
     return C.CDLL(path)
 

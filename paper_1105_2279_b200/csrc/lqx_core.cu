@@ -421,11 +421,14 @@ int lqx_transpose_range(lqx_ctx* ctx, lqx_kind kind, lqx_prec prec, const void* 
 
 extern "C" int lqx_field_import_dev(lqx_field* f, const void* dev_qdp_order) {
     if (!f || !dev_qdp_order) return LQX_EINVAL;
+    // the converter moves 128-bit words on both sides: a misaligned view would fault (a sticky context error)
+    if (((uintptr_t)dev_qdp_order & 15) != 0) return lqx_fail(f->ctx, LQX_EINVAL, "import_dev: the device buffer must be 16-byte aligned");
     LQX_CUDA(f->ctx, cudaSetDevice(f->ctx->device));
     return transpose_launch(f->ctx, f, dev_qdp_order, f->data, true);
 }
 extern "C" int lqx_field_export_dev(const lqx_field* f, void* dev_qdp_order) {
     if (!f || !dev_qdp_order) return LQX_EINVAL;
+    if (((uintptr_t)dev_qdp_order & 15) != 0) return lqx_fail(f->ctx, LQX_EINVAL, "export_dev: the device buffer must be 16-byte aligned");
     LQX_CUDA(f->ctx, cudaSetDevice(f->ctx->device));
     return transpose_launch(f->ctx, f, f->data, dev_qdp_order, false);
 }

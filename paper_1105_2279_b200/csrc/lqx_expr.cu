@@ -31,8 +31,9 @@ int check_same(lqx_ctx** ctx_out, std::initializer_list<const lqx_field*> fs) {
 // flat elementwise kernels over the raw storage (layout-agnostic; pad lanes included, they are
 // never read for results).  mode 0: r = a ; 1: r = a + k*b ; 2: r = k*a ; 3: r = a / k
 // ---------------------------------------------------------------------------------------------
-template <typename T, int MODE>
-__global__ void __launch_bounds__(256) k_flat(size_t nvec, T k, const T* __restrict__ a, const T* __restrict__ b, T* __restrict__ r) {
+template <typename T, int MODE, bool INPLACE>
+__global__ void __launch_bounds__(256) k_flat(size_t nvec, T k, typename KPtr<T, INPLACE>::in a, typename KPtr<T, INPLACE>::in b,
+                                              typename KPtr<T, INPLACE>::out r) {
     typedef typename Vec128<T>::type V;
     constexpr int W = Vec128<T>::W;
     const size_t step = (size_t)gridDim.x * blockDim.x;
@@ -59,9 +60,11 @@ int flat_launch(lqx_ctx* ctx, lqx_field* r, const lqx_field* a, const lqx_field*
     size_t want = (nvec + block - 1) / block;
     int grid = (int)std::min<size_t>(want, (size_t)ctx->num_sms * 16);
     if (grid < 1) grid = 1;
+    // in place (r is a or b, reading A21): the instantiation without __restrict__ / read-only loads
+    const bool inplace = lqx_identical(r, a) || (b && lqx_identical(r, b));
     LqxTimed timed(ctx, LQX_K_CATALOGUE);
-    k_flat<T, MODE><<<grid, block, 0, ctx->stream>>>(nvec, (T)k, (const T*)a->data, b ? (const T*)b->data : nullptr,
-                                                      (T*)r->data);
+    if (inplace) k_flat<T, MODE, true><<<grid, block, 0, ctx->stream>>>(nvec, (T)k, (const T*)a->data, b ? (const T*)b->data : nullptr, (T*)r->data);
+    else k_flat<T, MODE, false><<<grid, block, 0, ctx->stream>>>(nvec, (T)k, (const T*)a->data, b ? (const T*)b->data : nullptr, (T*)r->data);
     LQX_LAUNCH_CHECK(ctx);
     return LQX_OK;
 }
@@ -72,6 +75,8 @@ int flat_dispatch(lqx_field* r, const lqx_field* a, const lqx_field* b, double k
     int rc = b ? check_same(&ctx, {r, a, b}) : check_same(&ctx, {r, a});
     if (rc) return rc;
     if (r->kind != a->kind || (b && b->kind != a->kind)) return lqx_fail(ctx, LQX_ETYPE, "field kinds differ");
+    if ((lqx_same(r, a) && !lqx_identical(r, a)) || (b && lqx_same(r, b) && !lqx_identical(r, b)))
+        return lqx_fail(ctx, LQX_EALIAS, "destination partially overlaps an operand");
     LQX_CUDA(ctx, cudaSetDevice(ctx->device));
     return r->prec == LQX_F32 ? flat_launch<float, MODE>(ctx, r, a, b, k) : flat_launch<double, MODE>(ctx, r, a, b, k);
 }
@@ -81,9 +86,9 @@ int flat_dispatch(lqx_field* r, const lqx_field* a, const lqx_field* b, double k
 // periodic neighbour ("shift ... reads its operand through a site table" -- here the
 // index is computed).  AX = false: r = shift(b);  AX = true: r = alpha*a - shift(b)
 // ---------------------------------------------------------------------------------------------
-template <typename T, int NREAL, bool AX>
-__global__ void __launch_bounds__(128) k_shift(const __grid_constant__ Geo g, int dir, int mu, T alpha, const T* __restrict__ a,
-                                               const T* __restrict__ b, T* __restrict__ r) {
+template <typename T, int NREAL, bool AX, bool INPLACE>
+__global__ void __launch_bounds__(128) k_shift(const __grid_constant__ Geo g, int dir, int mu, T alpha, typename KPtr<T, INPLACE>::in a,
+                                               const T* __restrict__ b, typename KPtr<T, INPLACE>::out r) {
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= g.V) return;
     int x[4];
@@ -93,7 +98,7 @@ __global__ void __launch_bounds__(128) k_shift(const __grid_constant__ Geo g, in
     load_site<T, NREAL>(b, n, vb);
     if (AX) {
         T va[NREAL];
-        load_site<T, NREAL>(a, s, va);
+        load_site<T, NREAL, INPLACE>(a, s, va);
 #pragma unroll
         for (int j = 0; j < NREAL; ++j) vb[j] = mul_rn(alpha, va[j]) - vb[j];  // alpha*A rounded once, as written
     }
@@ -107,13 +112,18 @@ int shift_launch(lqx_ctx* ctx, lqx_field* r, double alpha, const lqx_field* a, c
     const T* pa = a ? (const T*)a->data : nullptr;
     const T* pb = (const T*)b->data;
     T* pr = (T*)r->data;
+    const bool inplace = AX && a && lqx_identical(r, a);  // form iii may overwrite its UNshifted operand (A21)
     LqxTimed timed(ctx, LQX_K_CATALOGUE);
+#define LQX_SHIFT_LAUNCH(NREAL)                                                                                   \
+    if (inplace) k_shift<T, NREAL, AX, AX><<<grid, block, 0, ctx->stream>>>(g, dir, mu, (T)alpha, pa, pb, pr);     \
+    else k_shift<T, NREAL, AX, false><<<grid, block, 0, ctx->stream>>>(g, dir, mu, (T)alpha, pa, pb, pr);
     switch ((int)r->kind) {
-        case LQX_COMPLEX: k_shift<T, 2, AX><<<grid, block, 0, ctx->stream>>>(g, dir, mu, (T)alpha, pa, pb, pr); break;
-        case LQX_COLORVEC: k_shift<T, 6, AX><<<grid, block, 0, ctx->stream>>>(g, dir, mu, (T)alpha, pa, pb, pr); break;
-        case LQX_COLORMAT: k_shift<T, 18, AX><<<grid, block, 0, ctx->stream>>>(g, dir, mu, (T)alpha, pa, pb, pr); break;
-        default: k_shift<T, 24, AX><<<grid, block, 0, ctx->stream>>>(g, dir, mu, (T)alpha, pa, pb, pr); break;
+        case LQX_COMPLEX: LQX_SHIFT_LAUNCH(2) break;
+        case LQX_COLORVEC: LQX_SHIFT_LAUNCH(6) break;
+        case LQX_COLORMAT: LQX_SHIFT_LAUNCH(18) break;
+        default: LQX_SHIFT_LAUNCH(24) break;
     }
+#undef LQX_SHIFT_LAUNCH
     LQX_LAUNCH_CHECK(ctx);
     return LQX_OK;
 }
@@ -122,13 +132,14 @@ int shift_launch(lqx_ctx* ctx, lqx_field* r, double alpha, const lqx_field* a, c
 // site-local matrix forms: one thread per site, all operands of the site in registers
 // ---------------------------------------------------------------------------------------------
 // form (i) R = A*B + C*adj(D)
-template <typename T>
-__global__ void __launch_bounds__(128) k_mm_plus_madj(int V, const T* __restrict__ a, const T* __restrict__ b, const T* __restrict__ c,
-                                                      const T* __restrict__ d, T* __restrict__ r) {
+template <typename T, bool INPLACE>
+__global__ void __launch_bounds__(128) k_mm_plus_madj(int V, typename KPtr<T, INPLACE>::in a, typename KPtr<T, INPLACE>::in b,
+                                                      typename KPtr<T, INPLACE>::in c, typename KPtr<T, INPLACE>::in d,
+                                                      typename KPtr<T, INPLACE>::out r) {
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= V) return;
-    const Mat3<T> ma = load_mat(a, s), mb = load_mat(b, s);
-    const Mat3<T> mc = load_mat(c, s), md = load_mat(d, s);
+    const Mat3<T> ma = load_mat<T, INPLACE>(a, s), mb = load_mat<T, INPLACE>(b, s);
+    const Mat3<T> mc = load_mat<T, INPLACE>(c, s), md = load_mat<T, INPLACE>(d, s);
     Mat3<T> acc = mul_nn(ma, mb);
     mac_na(acc, mc, md);
     store_mat(r, s, acc);
@@ -153,13 +164,14 @@ __global__ void __launch_bounds__(128) k_trace_mm(int V, const T* __restrict__ a
     store_site<T, 2>(c, s, out);
 }
 // form (iv) w = M*v per spin component
-template <typename T, int NSPIN>
-__global__ void __launch_bounds__(128) k_mat_vec(int V, const T* __restrict__ m, const T* __restrict__ v, T* __restrict__ w) {
+template <typename T, int NSPIN, bool INPLACE>
+__global__ void __launch_bounds__(128) k_mat_vec(int V, const T* __restrict__ m, typename KPtr<T, INPLACE>::in v,
+                                                 typename KPtr<T, INPLACE>::out w) {
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= V) return;
     const Mat3<T> mm = load_mat(m, s);
     Vec3<T> vv[NSPIN], ww[NSPIN];
-    load_vecs<T, NSPIN>(v, s, vv);
+    load_vecs<T, NSPIN, INPLACE>(v, s, vv);
 #pragma unroll
     for (int a = 0; a < NSPIN; ++a) {
 #pragma unroll
@@ -287,6 +299,7 @@ extern "C" int lqx_ax_minus_shift(lqx_field* r, double alpha, const lqx_field* a
     if (mu < 0 || mu > 3 || (dir != LQX_FORWARD && dir != LQX_BACKWARD)) return lqx_fail(ctx, LQX_EINVAL, "mu/dir");
     if (r->kind != a->kind || r->kind != b->kind) return lqx_fail(ctx, LQX_ETYPE, "ax_minus_shift: kinds differ");
     if (lqx_same(r, b)) return lqx_fail(ctx, LQX_EALIAS, "ax_minus_shift: destination is the shifted operand");
+    if (lqx_same(r, a) && !lqx_identical(r, a)) return lqx_fail(ctx, LQX_EALIAS, "ax_minus_shift: destination partially overlaps A");
     LQX_CUDA(ctx, cudaSetDevice(ctx->device));
     return r->prec == LQX_F32 ? shift_launch<float, true>(ctx, r, alpha, a, b, (int)dir, mu)
                               : shift_launch<double, true>(ctx, r, alpha, a, b, (int)dir, mu);
@@ -299,15 +312,23 @@ extern "C" int lqx_mm_plus_madj(lqx_field* r, const lqx_field* a, const lqx_fiel
     if (rc) return rc;
     for (const lqx_field* f : {(const lqx_field*)r, a, b, c, d})
         if (f->kind != LQX_COLORMAT) return lqx_fail(ctx, LQX_ETYPE, "mm_plus_madj wants colour matrices");
+    bool inplace = false;  // site-local: r may BE one of the operands (A21), never overlap one partially
+    for (const lqx_field* f : {a, b, c, d}) {
+        if (lqx_identical(r, f)) inplace = true;
+        else if (lqx_same(r, f)) return lqx_fail(ctx, LQX_EALIAS, "mm_plus_madj: destination partially overlaps an operand");
+    }
     LQX_CUDA(ctx, cudaSetDevice(ctx->device));
     const int V = ctx->geo.V, grid = (V + 127) / 128;
     LqxTimed timed(ctx, LQX_K_CATALOGUE);
-    if (r->prec == LQX_F32)
-        k_mm_plus_madj<float><<<grid, 128, 0, ctx->stream>>>(V, (const float*)a->data, (const float*)b->data,
-                                                            (const float*)c->data, (const float*)d->data, (float*)r->data);
-    else
-        k_mm_plus_madj<double><<<grid, 128, 0, ctx->stream>>>(V, (const double*)a->data, (const double*)b->data,
-                                                             (const double*)c->data, (const double*)d->data, (double*)r->data);
+#define LQX_FORM1(T, IP) k_mm_plus_madj<T, IP><<<grid, 128, 0, ctx->stream>>>(V, (const T*)a->data, (const T*)b->data, (const T*)c->data, (const T*)d->data, (T*)r->data)
+    if (r->prec == LQX_F32) {
+        if (inplace) LQX_FORM1(float, true);
+        else LQX_FORM1(float, false);
+    } else {
+        if (inplace) LQX_FORM1(double, true);
+        else LQX_FORM1(double, false);
+    }
+#undef LQX_FORM1
     LQX_LAUNCH_CHECK(ctx);
     return LQX_OK;
 }
@@ -318,6 +339,7 @@ extern "C" int lqx_trace_mm(lqx_field* c, const lqx_field* a, const lqx_field* b
     if (rc) return rc;
     if (c->kind != LQX_COMPLEX || a->kind != LQX_COLORMAT || b->kind != LQX_COLORMAT)
         return lqx_fail(ctx, LQX_ETYPE, "trace_mm: complex = trace(matrix*matrix)");
+    if (lqx_same(c, a) || lqx_same(c, b)) return lqx_fail(ctx, LQX_EALIAS, "trace_mm: destination overlaps an operand");
     LQX_CUDA(ctx, cudaSetDevice(ctx->device));
     const int V = ctx->geo.V, grid = (V + 127) / 128;
     LqxTimed timed(ctx, LQX_K_CATALOGUE);
@@ -335,17 +357,28 @@ extern "C" int lqx_mat_vec(lqx_field* w, const lqx_field* m, const lqx_field* v)
     if (rc) return rc;
     if (m->kind != LQX_COLORMAT || w->kind != v->kind || (v->kind != LQX_COLORVEC && v->kind != LQX_FERMION))
         return lqx_fail(ctx, LQX_ETYPE, "mat_vec: matrix * (colour vector | fermion)");
+    if (lqx_same(w, m) || (lqx_same(w, v) && !lqx_identical(w, v))) return lqx_fail(ctx, LQX_EALIAS, "mat_vec: destination overlaps an operand");
+    const bool inplace = lqx_identical(w, v);  // v = M*v in place (A21)
     LQX_CUDA(ctx, cudaSetDevice(ctx->device));
     const int V = ctx->geo.V, grid = (V + 127) / 128;
     LqxTimed timed(ctx, LQX_K_CATALOGUE);
     const bool ferm = v->kind == LQX_FERMION;
-    if (w->prec == LQX_F32) {
-        if (ferm) k_mat_vec<float, 4><<<grid, 128, 0, ctx->stream>>>(V, (const float*)m->data, (const float*)v->data, (float*)w->data);
-        else k_mat_vec<float, 1><<<grid, 128, 0, ctx->stream>>>(V, (const float*)m->data, (const float*)v->data, (float*)w->data);
-    } else {
-        if (ferm) k_mat_vec<double, 4><<<grid, 128, 0, ctx->stream>>>(V, (const double*)m->data, (const double*)v->data, (double*)w->data);
-        else k_mat_vec<double, 1><<<grid, 128, 0, ctx->stream>>>(V, (const double*)m->data, (const double*)v->data, (double*)w->data);
+#define LQX_FORM4(T, NS, IP) k_mat_vec<T, NS, IP><<<grid, 128, 0, ctx->stream>>>(V, (const T*)m->data, (const T*)v->data, (T*)w->data)
+#define LQX_FORM4_T(T)                          \
+    if (ferm) {                                 \
+        if (inplace) LQX_FORM4(T, 4, true);     \
+        else LQX_FORM4(T, 4, false);            \
+    } else {                                    \
+        if (inplace) LQX_FORM4(T, 1, true);     \
+        else LQX_FORM4(T, 1, false);            \
     }
+    if (w->prec == LQX_F32) {
+        LQX_FORM4_T(float)
+    } else {
+        LQX_FORM4_T(double)
+    }
+#undef LQX_FORM4_T
+#undef LQX_FORM4
     LQX_LAUNCH_CHECK(ctx);
     return LQX_OK;
 }

@@ -113,7 +113,33 @@ int lqx_fetch_result(lqx_ctx* ctx, int n, double* out);
         if (e__ != cudaSuccess) return lqx_cuda_fail((ctx), e__, "kernel launch"); \
     } while (0)
 
-static inline bool lqx_same(const lqx_field* a, const lqx_field* b) { return a->data == b->data; }
+// Aliasing between two fields is decided on BYTE RANGES (two lqx_field_attach views may overlap without sharing
+// a base pointer).  lqx_same: any overlap -- what the shifted forms reject with LQX_EALIAS.  lqx_identical: the same
+// storage exactly -- the only aliasing a site-local form may run with (in place, reading A21); those launches use
+// the plain-load, non-__restrict__ instantiation of their kernel (ld.global.nc is defined only for memory the
+// kernel never writes).
+static inline size_t lqx_field_nbytes(const lqx_field* f) {
+    return (size_t)f->ctx->geo.Vpad * 2 * (size_t)(int)f->kind * (size_t)(int)f->prec;
+}
+static inline bool lqx_same(const lqx_field* a, const lqx_field* b) {
+    const char* pa = (const char*)a->data;
+    const char* pb = (const char*)b->data;
+    return pa < pb + lqx_field_nbytes(b) && pb < pa + lqx_field_nbytes(a);
+}
+static inline bool lqx_identical(const lqx_field* a, const lqx_field* b) {
+    return a->data == b->data && lqx_field_nbytes(a) == lqx_field_nbytes(b);
+}
+// kernel parameter types: read-only / restrict for out-of-place launches, plain for in-place ones
+template <typename T, bool INPLACE>
+struct KPtr {
+    typedef const T* __restrict__ in;
+    typedef T* __restrict__ out;
+};
+template <typename T>
+struct KPtr<T, true> {
+    typedef const T* in;
+    typedef T* out;
+};
 
 // --------------------------------------------------------------------------------------------
 // device side: geometry
@@ -202,18 +228,20 @@ __device__ __forceinline__ float2 ldg_pinned(const float2* p) {
     return v;
 }
 
-// all NREAL reals of site s (read-only path)
-template <typename T, int NREAL>
-__device__ __forceinline__ void load_site(const T* __restrict__ base, int s, T (&r)[NREAL]) {
+// all NREAL reals of site s: through the read-only path (ld.global.nc), or with plain loads (PLAIN) where the same
+// kernel writes the field (in-place site-local forms)
+template <typename T, int NREAL, bool PLAIN = false>
+__device__ __forceinline__ void load_site(const T* base, int s, T (&r)[NREAL]) {
     typedef typename Vec128<T>::type V;
     constexpr int W = Vec128<T>::W, NFULL = NREAL / W;
     const T* blk = base + (size_t)(s >> 5) * (32 * NREAL);
     const int lane = s & 31;
     const V* p = reinterpret_cast<const V*>(blk) + lane;
 #pragma unroll
-    for (int q = 0; q < NFULL; ++q) unpack(__ldg(p + q * 32), &r[q * W]);
+    for (int q = 0; q < NFULL; ++q) unpack(PLAIN ? p[q * 32] : __ldg(p + q * 32), &r[q * W]);
     if (NREAL % W != 0) {  // fp32 only: trailing (re,im) pair
-        const float2 t = __ldg(reinterpret_cast<const float2*>(blk + NFULL * 32 * W) + lane);
+        const float2* ph = reinterpret_cast<const float2*>(blk + NFULL * 32 * W) + lane;
+        const float2 t = PLAIN ? *ph : __ldg(ph);
         r[NFULL * W] = (T)t.x;
         r[NFULL * W + 1] = (T)t.y;
     }
@@ -234,7 +262,7 @@ __device__ __forceinline__ void load_site_pinned(const T* __restrict__ base, int
     }
 }
 template <typename T, int NREAL>
-__device__ __forceinline__ void store_site(T* __restrict__ base, int s, const T (&r)[NREAL]) {
+__device__ __forceinline__ void store_site(T* base, int s, const T (&r)[NREAL]) {
     typedef typename Vec128<T>::type V;
     constexpr int W = Vec128<T>::W, NFULL = NREAL / W;
     T* blk = base + (size_t)(s >> 5) * (32 * NREAL);
@@ -280,10 +308,10 @@ struct Vec3 {
     T re[3], im[3];
 };
 
-template <typename T>
-__device__ __forceinline__ Mat3<T> load_mat(const T* __restrict__ p, int s) {
+template <typename T, bool PLAIN = false>
+__device__ __forceinline__ Mat3<T> load_mat(const T* p, int s) {
     T r[18];
-    load_site<T, 18>(p, s, r);
+    load_site<T, 18, PLAIN>(p, s, r);
     Mat3<T> m;
 #pragma unroll
     for (int i = 0; i < 3; ++i)
@@ -309,7 +337,7 @@ __device__ __forceinline__ Mat3<T> load_mat_pinned(const T* __restrict__ p, int 
     return m;
 }
 template <typename T>
-__device__ __forceinline__ void store_mat(T* __restrict__ p, int s, const Mat3<T>& m) {
+__device__ __forceinline__ void store_mat(T* p, int s, const Mat3<T>& m) {
     T r[18];
 #pragma unroll
     for (int i = 0; i < 3; ++i)
@@ -321,10 +349,10 @@ __device__ __forceinline__ void store_mat(T* __restrict__ p, int s, const Mat3<T
     store_site<T, 18>(p, s, r);
 }
 // NSPIN colour vectors of one site (NSPIN = 1: LatticeColorVector, 4: LatticeFermion)
-template <typename T, int NSPIN>
-__device__ __forceinline__ void load_vecs(const T* __restrict__ p, int s, Vec3<T> (&v)[NSPIN]) {
+template <typename T, int NSPIN, bool PLAIN = false>
+__device__ __forceinline__ void load_vecs(const T* p, int s, Vec3<T> (&v)[NSPIN]) {
     T r[6 * NSPIN];
-    load_site<T, 6 * NSPIN>(p, s, r);
+    load_site<T, 6 * NSPIN, PLAIN>(p, s, r);
 #pragma unroll
     for (int a = 0; a < NSPIN; ++a)
 #pragma unroll
@@ -334,7 +362,7 @@ __device__ __forceinline__ void load_vecs(const T* __restrict__ p, int s, Vec3<T
         }
 }
 template <typename T, int NSPIN>
-__device__ __forceinline__ void store_vecs(T* __restrict__ p, int s, const Vec3<T> (&v)[NSPIN]) {
+__device__ __forceinline__ void store_vecs(T* p, int s, const Vec3<T> (&v)[NSPIN]) {
     T r[6 * NSPIN];
 #pragma unroll
     for (int a = 0; a < NSPIN; ++a)

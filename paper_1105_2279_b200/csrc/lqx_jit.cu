@@ -59,8 +59,11 @@ Nvrtc g_nvrtc;
 const char* kPrelude = R"SRC(
 struct JGeo { int L[4]; int st[4]; int V; };
 template <int N> struct Obj { T re[N], im[N]; };   // N complex numbers in QDP order
-template <int N>
-__device__ __forceinline__ Obj<N> jload(const T* __restrict__ base, int s) {
+// PLAIN: ordinary loads instead of the read-only path -- for the destination of `+=` and for every leaf of a kernel
+// whose destination IS one of its leaves (in place, site-local): ld.global.nc is defined only for memory the kernel
+// never writes
+template <int N, bool PLAIN = kAllPlain>
+__device__ __forceinline__ Obj<N> jload(const T* base, int s) {
     constexpr int NREAL = 2 * N, NFULL = NREAL / W;
     T r[NREAL];
     const T* blk = base + (size_t)(s >> 5) * (32 * NREAL);
@@ -68,13 +71,14 @@ __device__ __forceinline__ Obj<N> jload(const T* __restrict__ base, int s) {
     const VEC* p = reinterpret_cast<const VEC*>(blk) + lane;
 #pragma unroll
     for (int q = 0; q < NFULL; ++q) {
-        const VEC v = __ldg(p + q * 32);
+        const VEC v = PLAIN ? p[q * 32] : __ldg(p + q * 32);
         const T* e = reinterpret_cast<const T*>(&v);
 #pragma unroll
         for (int k = 0; k < W; ++k) r[q * W + k] = e[k];
     }
     if (NREAL % W != 0) {
-        const float2 t = __ldg(reinterpret_cast<const float2*>(blk + NFULL * 32 * W) + lane);
+        const float2* ph = reinterpret_cast<const float2*>(blk + NFULL * 32 * W) + lane;
+        const float2 t = PLAIN ? *ph : __ldg(ph);
         r[NFULL * W] = (T)t.x;
         r[NFULL * W + 1] = (T)t.y;
     }
@@ -84,7 +88,7 @@ __device__ __forceinline__ Obj<N> jload(const T* __restrict__ base, int s) {
     return o;
 }
 template <int N>
-__device__ __forceinline__ void jstore(T* __restrict__ base, int s, const Obj<N>& o) {
+__device__ __forceinline__ void jstore(T* base, int s, const Obj<N>& o) {
     constexpr int NREAL = 2 * N, NFULL = NREAL / W;
     T r[NREAL];
 #pragma unroll
@@ -525,10 +529,11 @@ static int live_reals(const std::vector<XNode>& n, int i) {
 // reduce: 0 = dst (=|+=) expr ; 1 = norm2(expr) ; 2 = sum(expr).  For the reductions every thread walks a
 // grid-stride loop of sites with fp64 accumulators and the CTA leaves one partial per component.
 std::string make_source(const std::vector<XNode>& tree, int nleaves, int nscalars, int dst_kind, bool f32, bool accumulate,
-                        int reduce) {
+                        int reduce, bool inplace) {
     std::ostringstream src;
     if (f32) src << "typedef float T;\ntypedef float4 VEC;\nconstexpr int W = 4;\n";
     else src << "typedef double T;\ntypedef double2 VEC;\nconstexpr int W = 2;\n";
+    src << "constexpr bool kAllPlain = " << (inplace ? "true" : "false") << ";\n";
     src << kPrelude;
     // register budget from the estimated live reals (+ fp64 reduction accumulators, + 16 for indices and
     // pointers): at most six CTAs of 128 threads per SM (85 registers) in fp32 and three (170) in fp64, at least two
@@ -537,7 +542,7 @@ std::string make_source(const std::vector<XNode>& tree, int nleaves, int nscalar
     const int min_blocks = std::max(2, std::min(f32 ? 6 : 3, 65536 / (128 * regs)));
     src << "extern \"C\" __global__ void __launch_bounds__(128, " << min_blocks << ") lqx_jit(const JGeo g";
     for (int k = 0; k < nscalars; ++k) src << ", const T k" << k;
-    for (int l = 0; l < nleaves; ++l) src << ", const T* __restrict__ p" << l;
+    for (int l = 0; l < nleaves; ++l) src << (inplace ? ", const T* p" : ", const T* __restrict__ p") << l;
     const int nc = reduce == 1 ? 1 : 2 * dst_kind;
     if (reduce) {
         src << ", double* __restrict__ partials) {\n    double acc[" << nc << "];\n";
@@ -563,7 +568,7 @@ std::string make_source(const std::vector<XNode>& tree, int nleaves, int nscalar
             << ".re[i];\n        acc[2 * i + 1] += (double)" << r << ".im[i];\n    }\n    }\n";
         src << "    jreduce<" << nc << ">(acc, partials);\n";
     } else if (accumulate) {
-        src << "    jstore<" << dst_kind << ">(dst, s0, jadd(jload<" << dst_kind << ">(dst, s0), " << r << "));\n";
+        src << "    jstore<" << dst_kind << ">(dst, s0, jadd(jload<" << dst_kind << ", true>(dst, s0), " << r << "));\n";
     } else {
         src << "    jstore<" << dst_kind << ">(dst, s0, " << r << ");\n";
     }
@@ -633,7 +638,7 @@ extern "C" int lqx_expr_source(lqx_ctx* ctx, lqx_kind dst_kind, lqx_prec prec, i
     if (rc) return rc;
     if (tree.back().kind != (int)dst_kind) return lqx_fail(ctx, LQX_ETYPE, "expr: destination kind differs from the expression's");
     const int reduce = accumulate >= 2 ? accumulate - 1 : 0;  // 2, 3: the kernels of lqx_expr_reduce (norm2, sum)
-    const std::string src = make_source(tree, nleaves, (int)scalars.size(), (int)dst_kind, prec == LQX_F32, accumulate == 1, reduce);
+    const std::string src = make_source(tree, nleaves, (int)scalars.size(), (int)dst_kind, prec == LQX_F32, accumulate == 1, reduce, false);
     strncpy(buf, src.c_str(), buflen - 1);
     buf[buflen - 1] = '\0';
     return (int)src.size();
@@ -655,14 +660,18 @@ static int run_expr(lqx_ctx* ctx, lqx_prec prec, lqx_field* dst, int accumulate,
     if (rc) return rc;
     if (scalars.size() > 16) return lqx_fail(ctx, LQX_EINVAL, "expr: at most 16 scalars");
     const int kind = tree.back().kind;
+    bool inplace = false;
     if (dst) {
         if (kind != (int)dst->kind) return lqx_fail(ctx, LQX_ETYPE, "expr: destination kind differs from the expression's");
-        for (int l = 0; l < nleaves; ++l)
+        for (int l = 0; l < nleaves; ++l) {
             if (shifted[l] && lqx_same(dst, leaves[l])) return lqx_fail(ctx, LQX_EALIAS, "expr: destination is read through a shift");
+            if (lqx_identical(dst, leaves[l])) inplace = true;  // site-local use of the destination (A21)
+            else if (lqx_same(dst, leaves[l])) return lqx_fail(ctx, LQX_EALIAS, "expr: destination partially overlaps a leaf");
+        }
     }
     LQX_CUDA(ctx, cudaSetDevice(ctx->device));
     const bool f32 = prec == LQX_F32;
-    const std::string src = make_source(tree, nleaves, (int)scalars.size(), kind, f32, accumulate != 0, reduce);
+    const std::string src = make_source(tree, nleaves, (int)scalars.size(), kind, f32, accumulate != 0, reduce, inplace);
     cudaKernel_t fn;
     {
         std::lock_guard<std::mutex> lock(g_caches_mutex);

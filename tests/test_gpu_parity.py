@@ -529,6 +529,124 @@ def test_error_codes(lqx):
             lqx.Lattice((4, 0, 4, 4))
 
 
+# Reading A21: a site-local form may overwrite one of its operands.  Those launches run the plain-load,
+# non-__restrict__ instantiation of the kernel (ld.global.nc is undefined for memory the kernel writes): every in-place
+# form, twice, on a ragged lattice, bit for bit against its out-of-place result.
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+def test_in_place_forms_equal_out_of_place_bit_for_bit(lqx, prec):
+    dims = DIMS_RAGGED
+    a, b, c, d = (_gauss(7, k, dims, "cm", prec) for k in range(4))
+    v = _gauss(7, 4, dims, "cv", prec)
+    psi = _gauss(7, 5, dims, "f", prec)
+    with lqx.Lattice(dims) as lat:
+        P = _prec(lqx, prec)
+        fa, fb, fc, fd = (lat.from_host(t) for t in (a, b, c, d))
+
+        def fresh(t):
+            return lat.from_host(t)
+
+        for rep in range(2):
+            # form i with the destination in each operand slot
+            want = lat.alloc(lqx.COLORMAT, P)
+            lqx.mm_plus_madj(want, fa, fb, fc, fd)
+            w = want.pop()
+            for slot in range(4):
+                ops = [fa, fb, fc, fd]
+                ops[slot] = fresh((a, b, c, d)[slot])
+                lqx.mm_plus_madj(ops[slot], *ops)
+                assert np.array_equal(ops[slot].pop(), w), ("form i", slot, rep)
+            # the same matrix in two slots and as the destination
+            x = fresh(a)
+            lqx.mm_plus_madj(want, fa, fa, fc, fa)
+            lqx.mm_plus_madj(x, x, x, fc, x)
+            assert np.array_equal(x.pop(), want.pop())
+            # E3 / E4 / scale / copy
+            for fn, args in ((lqx.axpy, (1, 0.37, 2)), (lqx.axpy, (2, 0.37, 1))):
+                r = lat.alloc(lqx.COLORMAT, P)
+                fn(r, fa, args[1], fb)
+                x = fresh(a if args[0] == 1 else b)
+                fn(x, x if args[0] == 1 else fa, args[1], fb if args[0] == 1 else x)
+                assert np.array_equal(x.pop(), r.pop()), ("axpy", args, rep)
+            r = lat.alloc(lqx.COLORMAT, P)
+            x = fresh(a)
+            lqx.scale(r, -1.75, fa), lqx.scale(x, -1.75, x)
+            assert np.array_equal(x.pop(), r.pop())
+            x = fresh(a)
+            lqx.divide(r, fa, 1.3), lqx.divide(x, x, 1.3)
+            assert np.array_equal(x.pop(), r.pop())
+            x = fresh(a)
+            lqx.copy(x, x)
+            assert np.array_equal(x.pop(), a)
+            # form iv: v = M v
+            for vec, kind in ((v, lqx.COLORVEC), (psi, lqx.FERMION)):
+                r = lat.alloc(kind, P)
+                x = fresh(vec)
+                lqx.mat_vec(r, fa, x), lqx.mat_vec(x, fa, x)
+                assert np.array_equal(x.pop(), r.pop()), ("form iv", kind, rep)
+            # form iii may overwrite its UNshifted operand
+            r = lat.alloc(lqx.COLORMAT, P)
+            x = fresh(a)
+            lqx.ax_minus_shift(r, 2.5, fa, fb, lqx.BACKWARD, 2), lqx.ax_minus_shift(x, 2.5, x, fb, lqx.BACKWARD, 2)
+            assert np.array_equal(x.pop(), r.pop())
+            # run-time expressions: dst as a leaf (site-local), and dst += e
+            X = lqx.Expr.leaf
+            r = lat.alloc(lqx.COLORMAT, P)
+            x = fresh(a)
+            lqx.expr_eval(r, X(fa) * X(fb) + X(fc) * lqx.adj(X(fa)))
+            lqx.expr_eval(x, X(x) * X(fb) + X(fc) * lqx.adj(X(x)))
+            assert np.array_equal(x.pop(), r.pop())
+            r, x = fresh(d), fresh(d)
+            lqx.expr_eval(r, X(fa) * lqx.shifted(X(fb), lqx.FORWARD, 1), accumulate=True)
+            y = fresh(a)
+            lqx.expr_eval(x, X(y) * lqx.shifted(X(fb), lqx.FORWARD, 1), accumulate=True)
+            assert np.array_equal(x.pop(), r.pop())
+
+
+def test_partial_overlap_and_misalignment_are_errors(lqx):
+    """two attached views that overlap without sharing a base pointer are aliases too (byte ranges, not pointers);
+    the device-to-device converters want 16-byte aligned buffers"""
+    import ctypes as C
+
+    import torch
+
+    dims = (4, 4, 4, 4)
+    with lqx.Lattice(dims) as lat:
+        nbytes = lat.field_bytes(lqx.COLORMAT, lqx.F32)
+        mem = torch.zeros(2 * nbytes, dtype=torch.uint8, device="cuda")
+
+        def view(off):
+            h = C.c_void_p()
+            rc = lqx._lib.lqx_field_attach(lat.ctx, lqx.COLORMAT, lqx.F32, C.c_void_p(mem.data_ptr() + off), nbytes, C.byref(h))
+            assert rc == 0
+            return lqx.Field(lat, h, lqx.COLORMAT, lqx.F32, mem)
+
+        f0, f1, f2 = view(0), view(256), view(nbytes)
+        other = lat.alloc(lqx.COLORMAT, lqx.F32)
+
+        def code(fn, *args):
+            with pytest.raises(lqx.LqxError) as e:
+                fn(*args)
+            return e.value.code
+
+        assert code(lqx.shift, f0, f1, +1, 0) == -4
+        assert code(lqx.copy, f0, f1) == -4
+        assert code(lqx.mm_plus_madj, f1, f0, other, other, other) == -4
+        assert code(lqx.ax_minus_shift, f1, 2.5, f0, other, -1, 2) == -4
+        u = [f1, other, lat.alloc(lqx.COLORMAT, lqx.F32), lat.alloc(lqx.COLORMAT, lqx.F32)]
+        o = [f0] + [lat.alloc(lqx.COLORMAT, lqx.F32) for _ in range(3)]
+        assert code(lqx.smear_step, o, u, 0.5) == -4
+        lqx.copy(f0, f2)  # adjacent, not overlapping: fine
+        lqx.shift(f0, f2, +1, 0)
+        buf = torch.zeros(lat.volume * 18 + 4, dtype=torch.float32, device="cuda")
+        with pytest.raises(lqx.LqxError) as e:
+            other.import_dev(buf[1:])
+        assert e.value.code == -1
+        with pytest.raises(lqx.LqxError) as e:
+            other.export_dev(buf[1:])
+        assert e.value.code == -1
+        other.import_dev(buf[4:])
+
+
 # ------------------------------------------------------------------------------------------------
 # NEXT-1: the paper's complete Jacobi smearing routine (Listing 1)
 # ------------------------------------------------------------------------------------------------
