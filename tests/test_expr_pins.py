@@ -122,7 +122,7 @@ def test_generated_source_is_one_fused_kernel():
                  lqx.COLORMAT, lqx.F64)
     assert s1 == s2 and "2.5" not in s1
     # accumulate ('+=', E2 of the Listing) reads the destination
-    assert "jload<12>(dst, s0)" in _source(hop_nodes(), [lqx.COLORMAT] * 4 + [lqx.FERMION], lqx.FERMION, lqx.F32, True)
+    assert "jload<12, true>(dst, s0)" in _source(hop_nodes(), [lqx.COLORMAT] * 4 + [lqx.FERMION], lqx.FERMION, lqx.F32, True)
 
 
 def test_generator_type_and_shape_errors():
