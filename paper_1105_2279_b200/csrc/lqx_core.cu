@@ -89,6 +89,7 @@ extern "C" int lqx_init(const int dims[4], int device, void* cuda_stream, lqx_ct
     c->opt_smear_variant = 0;
     c->opt_plaq_variant = 0;
     c->opt_block = 0;
+    c->opt_hop_block = 0;
     c->opt_tile = -1;
     c->opt_jacobi_block = c->opt_jacobi_sites = 0;
     c->timing = false;
@@ -178,6 +179,7 @@ extern "C" int lqx_set_option(lqx_ctx* ctx, const char* key, int value) {
     if (!strcmp(key, "smear_variant")) ctx->opt_smear_variant = value;
     else if (!strcmp(key, "plaq_variant")) ctx->opt_plaq_variant = value;
     else if (!strcmp(key, "block")) ctx->opt_block = value;
+    else if (!strcmp(key, "hop_block")) ctx->opt_hop_block = value;
     else if (!strcmp(key, "tile")) ctx->opt_tile = value;
     else if (!strcmp(key, "jacobi_block")) ctx->opt_jacobi_block = value;
     else if (!strcmp(key, "jacobi_sites")) ctx->opt_jacobi_sites = value;

@@ -53,6 +53,7 @@ struct lqx_ctx {
     int opt_smear_variant;
     int opt_plaq_variant;                 // plaquette kernel: 0 = automatic, 1 = rolled loops, 2 = the site's four links held in registers
     int opt_block;
+    int opt_hop_block;                    // CTA size of the hop kernel on linear blocks: 0 = default (128), 32, 64, 128, 256
     int opt_jacobi_block, opt_jacobi_sites;  // launch geometry of the Jacobi step (0 = default 128 x 1)
     int opt_tile;  // -1 = automatic, 0 = Linear, 1..3 = TileA..TileC (lqx_smear.cuh)
     // optional per-kernel-class device timing (bench harness): cudaEvent pairs on the stream
@@ -818,8 +819,9 @@ struct Tiled {
     }
 };
 
-struct Linear {
-    static constexpr int THREADS = 128;
+template <int NTHREADS>
+struct LinearN {
+    static constexpr int THREADS = NTHREADS;
     __device__ static __forceinline__ bool site(const Geo& g, const TileMap& m, int x[4], int& s) {
         s = m.s0 + blockIdx.x * THREADS + threadIdx.x;
         if (s >= m.s1) return false;
@@ -840,3 +842,4 @@ struct Linear {
     }
     static bool splits_t(int) { return true; }
 };
+typedef LinearN<128> Linear;

@@ -72,12 +72,23 @@ template <typename T, int NSPIN, bool DIV, int NSITE, int MASK>
 __global__ void __launch_bounds__(256, sizeof(T) == 4 ? 3 : 2) k_jacobi_step(const __grid_constant__ Geo g, const __grid_constant__ Links<T> u,
                                                                              int dirmask, const T* __restrict__ psi, const T* __restrict__ s0,
                                                                              T kappa, T nrm, T* __restrict__ chi) {
+    // Programmatic dependent launch (sm_90+): the iterations of the routine are launched with programmatic stream
+    // serialisation, so the CTAs of iteration k+1 are scheduled -- and do their index arithmetic -- while iteration
+    // k drains; they touch memory only after griddepcontrol.wait, which returns when iteration k is complete and
+    // visible.  16^3x32, 20 iterations: 0.302 -> 0.268 ms.  (Requesting the first direction's links before the wait,
+    // which do not depend on the previous iteration, changed nothing.)
+    asm volatile("griddepcontrol.launch_dependents;");
+    bool waited = false;
 #pragma unroll 1
     for (int k = 0; k < NSITE; ++k) {
         const int s = (k * gridDim.x + blockIdx.x) * blockDim.x + threadIdx.x;
         if (s >= g.V) return;
         int x[4];
         site_coords(g, s, x);
+        if (!waited) {
+            asm volatile("griddepcontrol.wait;" ::: "memory");
+            waited = true;
+        }
         Vec3<T> acc[NSPIN];
 #pragma unroll
         for (int a = 0; a < NSPIN; ++a)
@@ -271,22 +282,30 @@ static int hop_impl(lqx_field* chi, const lqx_field* const u[4], const lqx_field
 #define LQX_HOP(T, NSPIN, N2)                                                                                      \
     k_hop<T, NSPIN, N2, MAP><<<grid, MAP::THREADS, 0, ctx->stream>>>(g, tm, make_links<T>(u), (const T*)psi->data, \
                                                                     (T*)chi->data, ctx->d_partials, ctx->d_ticket, ctx->h_result)
-    LQX_WITH_MAP(choice, {
-        const int grid = MAP::grid(g);
-        if (n2) {
-            rc = lqx_ensure_partials(ctx, (size_t)grid);
-            if (rc) return rc;
-        }
-        const TileMap tm = MAP::map(g, kSlabZ);
-        LqxTimed timed(ctx, LQX_K_HOP);
-        if (psi->prec == LQX_F32) {
-            if (ferm) { if (n2) LQX_HOP(float, 4, true); else LQX_HOP(float, 4, false); }
-            else      { if (n2) LQX_HOP(float, 1, true); else LQX_HOP(float, 1, false); }
-        } else {
-            if (ferm) { if (n2) LQX_HOP(double, 4, true); else LQX_HOP(double, 4, false); }
-            else      { if (n2) LQX_HOP(double, 1, true); else LQX_HOP(double, 1, false); }
-        }
-    })
+#define LQX_HOP_BODY                                                                                  \
+    {                                                                                                 \
+        const int grid = MAP::grid(g);                                                                \
+        if (n2) {                                                                                     \
+            rc = lqx_ensure_partials(ctx, (size_t)grid);                                              \
+            if (rc) return rc;                                                                        \
+        }                                                                                             \
+        const TileMap tm = MAP::map(g, kSlabZ);                                                       \
+        LqxTimed timed(ctx, LQX_K_HOP);                                                               \
+        if (psi->prec == LQX_F32) {                                                                   \
+            if (ferm) { if (n2) LQX_HOP(float, 4, true); else LQX_HOP(float, 4, false); }             \
+            else      { if (n2) LQX_HOP(float, 1, true); else LQX_HOP(float, 1, false); }             \
+        } else {                                                                                      \
+            if (ferm) { if (n2) LQX_HOP(double, 4, true); else LQX_HOP(double, 4, false); }           \
+            else      { if (n2) LQX_HOP(double, 1, true); else LQX_HOP(double, 1, false); }           \
+        }                                                                                             \
+    }
+    // linear blocks: the CTA size is a launch-geometry knob (option "hop_block", the auto-tuner's choice)
+    const int hb = ctx->opt_hop_block;
+    if (choice == 0 && hb == 32) { typedef LinearN<32> MAP; LQX_HOP_BODY }
+    else if (choice == 0 && hb == 64) { typedef LinearN<64> MAP; LQX_HOP_BODY }
+    else if (choice == 0 && hb == 256) { typedef LinearN<256> MAP; LQX_HOP_BODY }
+    else LQX_WITH_MAP(choice, LQX_HOP_BODY)
+#undef LQX_HOP_BODY
 #undef LQX_HOP
     LQX_LAUNCH_CHECK(ctx);
     if (n2) return lqx_fetch_result(ctx, 1, norm2_out);
@@ -601,9 +620,17 @@ extern "C" int lqx_jacobi_smear(lqx_field* chi, const lqx_field* const u[4], dou
         const bool last = it == iter - 1;
         {
             LqxTimed timed(ctx, LQX_K_HOP);
-#define LQX_JAC3(T, NSPIN, DIV, NS, MASK)                                                                                          \
-    k_jacobi_step<T, NSPIN, DIV, NS, MASK><<<grid, bs, 0, ctx->stream>>>(g, make_links<T>(u), dirmask, (const T*)cur->data,         \
-                                                                         (const T*)tmp[0]->data, (T)kappa, (T)norm, (T*)nxt->data)
+#define LQX_JAC3(T, NSPIN, DIV, NS, MASK)                                                                                  \
+    do {                                                                                                                   \
+        cudaLaunchConfig_t cfg = {};                                                                                       \
+        cfg.gridDim = dim3(grid), cfg.blockDim = dim3(bs), cfg.dynamicSmemBytes = 0, cfg.stream = ctx->stream;             \
+        cudaLaunchAttribute attr[1];                                                                                       \
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;                                                   \
+        attr[0].val.programmaticStreamSerializationAllowed = 1;                                                            \
+        cfg.attrs = attr, cfg.numAttrs = 1;                                                                                \
+        LQX_CUDA(ctx, cudaLaunchKernelEx(&cfg, k_jacobi_step<T, NSPIN, DIV, NS, MASK>, g, make_links<T>(u), dirmask,       \
+                                         (const T*)cur->data, (const T*)tmp[0]->data, (T)kappa, (T)norm, (T*)nxt->data)); \
+    } while (0)
 #define LQX_JAC(T, NSPIN, DIV)                                          \
     do {                                                                \
         if (nsite == 1 && dirmask == 0xF) LQX_JAC3(T, NSPIN, DIV, 1, 0xF); \
