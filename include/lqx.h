@@ -255,6 +255,32 @@ enum { LQX_K_SMEAR = 0, LQX_K_PLAQUETTE = 1, LQX_K_HOP = 2, LQX_K_CATALOGUE = 3,
 int lqx_kernel_time(lqx_ctx* ctx, int kernel_class, double* total_ms, int* count);
 /* Number of kernels this context has launched since init (for bench.py's gpu_launches). */
 int64_t lqx_launch_count(const lqx_ctx* ctx);
+/* What the last lqx_smear_step / lqx_smear_iterate launch of this context ran: the variant in effect after options,
+ * tuned choice and fall-backs, the FMA lane-operations it executes per site (48 products x 108 + 144 for the literal
+ * evaluation), and the kernel's name (truncated to name_len - 1 characters).  Any out pointer may be NULL. */
+int lqx_smear_info(const lqx_ctx* ctx, int* variant, int* lane_ops_per_site, char* kernel_name, int name_len);
+
+/* ---------------------------------------------------------------------------------------------
+ * Auto-tuning of the launch geometry -- the paper's to-do (sec.5.4 "auto-tuning ... geometry
+ * parameters ... stored for later inclusion"; sec.9), its sweeps PAPER.md:242-262 (Figs. 1-2).
+ * lqx_autotune times, on the context's lattice and stream (it synchronises), every geometry the library can select for
+ * one kernel class and precision and keeps the fastest in the context; later calls use it unless an explicit
+ * lqx_set_option overrides it.  kernel_class: LQX_K_SMEAR (param = smear_variant, tile), LQX_K_PLAQUETTE
+ * (param = plaq_variant), LQX_K_HOP (param[0] > 0: CTA size of lqx_hop; param[0] < 0: N_threads = -param[0] and
+ * N_site = param[1] of one lqx_jacobi_smear iteration).  rows (caller-owned, may be NULL) receives up to max_rows
+ * table rows: ms = median of `reps` launches, chosen = 1 for the kept geometry; *nrows = rows measured.
+ * It allocates and frees its own scratch fields (eight link fields, or four links and four fermions).
+ * lqx_tuned reads back what is kept (0 / -1 = nothing): smear {variant, tile}, plaquette {variant},
+ * hop {hop_block, jacobi_block, jacobi_sites}. */
+typedef struct {
+    int kernel_class;
+    int prec;
+    int param[2];
+    double ms;
+    int chosen;
+} lqx_tune_row;
+int lqx_autotune(lqx_ctx* ctx, int kernel_class, lqx_prec prec, int reps, lqx_tune_row* rows, int max_rows, int* nrows);
+int lqx_tuned(const lqx_ctx* ctx, int kernel_class, lqx_prec prec, int out[4]);
 /* Options: "smear_variant" 0 = default (fp32: 9, fp64: 3), 3 = rolled literal kernel, 1 = first-cut literal kernel,
  * 2 = shared-corner kernel (36 products, lower staples exchanged through shared memory), 4 = four
  * threads per site, 6 = operands staged in shared memory with cp.async (fp32), 7 = the CTA tile's own links in
@@ -266,7 +292,8 @@ int64_t lqx_launch_count(const lqx_ctx* ctx);
  * 4x4x4x2, 16x4x2x2, 16x2x2x2, 32x2x2x2) of the nearest-neighbour kernels, used if it divides the
  * lattice.  "jacobi_block" (32, 64, 128, 256) and "jacobi_sites" (1, 2, 4): the paper's launch
  * geometry parameters N_threads and N_site for lqx_jacobi_smear; 0 = tuned default.
- * "host_slabs": see lqx_smear_iterate_host.
+ * "hop_block" (32, 64, 128, 256): CTA size of lqx_hop on
+ * linear blocks; 0 = tuned or default (128).  "host_slabs": see lqx_smear_iterate_host.
  * "plaq_variant" 0 = automatic (fp32: the site's four links held in registers, 16 matrix loads per site;
  * fp64: rolled plane loops, 21 loads at half the registers -- each the faster one measured), 1 = rolled, 2 = held.
  * "time_kernels" 0/1 (see above).  All variants agree within rounding; DESIGN.md sec.6. */

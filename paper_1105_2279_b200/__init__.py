@@ -24,6 +24,10 @@ KIND_SHAPE = {COMPLEX: (), COLORVEC: (3,), COLORMAT: (3, 3), FERMION: (4, 3)}
 _NP = {F32: np.float32, F64: np.float64}
 
 
+class TuneRow(C.Structure):
+    _fields_ = [("kernel_class", C.c_int), ("prec", C.c_int), ("param", C.c_int * 2), ("ms", C.c_double), ("chosen", C.c_int)]
+
+
 class LqxError(RuntimeError):
     def __init__(self, code, detail=""):
         self.code = int(code)
@@ -106,6 +110,9 @@ SIGNATURES = {
     "lqx_bench_copy_peak": (_i, [_vp, C.c_size_t, _pd]),
     "lqx_kernel_time": (_i, [_vp, _i, _pd, C.POINTER(C.c_int)]),
     "lqx_launch_count": (_i64, [_vp]),
+    "lqx_smear_info": (_i, [_vp, C.POINTER(C.c_int), C.POINTER(C.c_int), C.c_char_p, _i]),
+    "lqx_autotune": (_i, [_vp, _i, _i, _i, _vp, _i, C.POINTER(C.c_int)]),
+    "lqx_tuned": (_i, [_vp, _i, _i, C.POINTER(C.c_int)]),
     "lqx_set_option": (_i, [_vp, C.c_char_p, _i]),
     "lqx_strerror": (C.c_char_p, [_i]),
     "lqx_last_error": (C.c_char_p, [_vp]),
@@ -242,6 +249,26 @@ class Lattice:
 
     def expr_cache_size(self) -> int:
         return int(_lib.lqx_expr_cache_size(self.ctx))
+
+    def smear_info(self):
+        """(variant, FMA lane-ops per site, kernel name) of the last smear launch."""
+        v, n = C.c_int(), C.c_int()
+        name = C.create_string_buffer(64)
+        _check(_lib.lqx_smear_info(self.ctx, C.byref(v), C.byref(n), name, 64), self.ctx)
+        return v.value, n.value, name.value.decode()
+
+    def autotune(self, kernel_class, prec, reps=5):
+        """Time every launch geometry of a kernel class on this lattice, keep the fastest; returns the table rows."""
+        rows = (TuneRow * 64)()
+        n = C.c_int()
+        _check(_lib.lqx_autotune(self.ctx, kernel_class, prec, reps, C.cast(rows, C.c_void_p), 64, C.byref(n)), self.ctx)
+        return [{"kernel_class": r.kernel_class, "prec": r.prec, "param": [r.param[0], r.param[1]], "ms": r.ms, "chosen": bool(r.chosen)}
+                for r in rows[:min(n.value, 64)]]
+
+    def tuned(self, kernel_class, prec):
+        out = (C.c_int * 4)()
+        _check(_lib.lqx_tuned(self.ctx, kernel_class, prec, out), self.ctx)
+        return list(out)
 
     def launch_count(self) -> int:
         return int(_lib.lqx_launch_count(self.ctx))

@@ -90,6 +90,11 @@ extern "C" int lqx_init(const int dims[4], int device, void* cuda_stream, lqx_ct
     c->opt_plaq_variant = 0;
     c->opt_block = 0;
     c->opt_hop_block = 0;
+    for (int p = 0; p < 2; ++p) {
+        c->tuned_smear_variant[p] = 0, c->tuned_smear_tile[p] = -1, c->tuned_plaq_variant[p] = 0;
+        c->tuned_hop_block[p] = 0, c->tuned_jacobi_block[p] = 0, c->tuned_jacobi_sites[p] = 0;
+    }
+    c->last_smear_variant = 0, c->last_smear_lane_ops = 0, c->last_smear_kernel = "";
     c->opt_tile = -1;
     c->opt_jacobi_block = c->opt_jacobi_sites = 0;
     c->timing = false;
@@ -158,6 +163,16 @@ extern "C" int lqx_set_stream(lqx_ctx* ctx, void* cuda_stream) {
 extern "C" int64_t lqx_volume(const lqx_ctx* ctx) { return ctx ? ctx->geo.V : (int64_t)LQX_EINVAL; }
 extern "C" int64_t lqx_padded_volume(const lqx_ctx* ctx) { return ctx ? ctx->geo.Vpad : (int64_t)LQX_EINVAL; }
 extern "C" int64_t lqx_launch_count(const lqx_ctx* ctx) { return ctx ? ctx->launches : (int64_t)LQX_EINVAL; }
+extern "C" int lqx_smear_info(const lqx_ctx* ctx, int* variant, int* lane_ops_per_site, char* kernel_name, int name_len) {
+    if (!ctx) return LQX_EINVAL;
+    if (variant) *variant = ctx->last_smear_variant;
+    if (lane_ops_per_site) *lane_ops_per_site = ctx->last_smear_lane_ops;
+    if (kernel_name && name_len > 0) {
+        strncpy(kernel_name, ctx->last_smear_kernel ? ctx->last_smear_kernel : "", (size_t)name_len - 1);
+        kernel_name[name_len - 1] = '\0';
+    }
+    return LQX_OK;
+}
 
 static bool valid_kind(int k) { return k == LQX_COMPLEX || k == LQX_COLORVEC || k == LQX_COLORMAT || k == LQX_FERMION; }
 static bool valid_prec(int p) { return p == LQX_F32 || p == LQX_F64; }

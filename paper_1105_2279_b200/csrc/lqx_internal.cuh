@@ -56,6 +56,15 @@ struct lqx_ctx {
     int opt_hop_block;                    // CTA size of the hop kernel on linear blocks: 0 = default (128), 32, 64, 128, 256
     int opt_jacobi_block, opt_jacobi_sites;  // launch geometry of the Jacobi step (0 = default 128 x 1)
     int opt_tile;  // -1 = automatic, 0 = Linear, 1..3 = TileA..TileC (lqx_smear.cuh)
+    // launch geometries kept by lqx_autotune (lqx_tune.cu), per precision (0 = fp32, 1 = fp64); 0 / -1 = not tuned.
+    // An explicit option always wins over a tuned value, a tuned value over the built-in default.
+    int tuned_smear_variant[2], tuned_smear_tile[2];
+    int tuned_plaq_variant[2];
+    int tuned_hop_block[2];
+    int tuned_jacobi_block[2], tuned_jacobi_sites[2];
+    // what the last smear launch ran (bench.py reports the kernel and its executed lane-ops from here)
+    int last_smear_variant, last_smear_lane_ops;
+    const char* last_smear_kernel;
     // optional per-kernel-class device timing (bench harness): cudaEvent pairs on the stream
     bool timing;
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> timers[LQX_NUM_KERNEL_CLASSES];

@@ -213,7 +213,8 @@ int plaquette_launch(lqx_ctx* ctx, const lqx_field* const u[4], double* out) {
     const int choice = lqx_pick_tile(ctx, 0);  // measured: linear 128-site blocks beat every tile shape here
     int nblocks = 0;
     // option plaq_variant: 0 = automatic (held links in fp32, rolled loops in fp64: measured), 1 = rolled, 2 = held
-    const bool held = ctx->opt_plaq_variant == 2 || (ctx->opt_plaq_variant == 0 && sizeof(T) == 4 && choice == 0);
+    const int pv = ctx->opt_plaq_variant ? ctx->opt_plaq_variant : ctx->tuned_plaq_variant[sizeof(T) == 4 ? 0 : 1];
+    const bool held = pv == 2 || (pv == 0 && sizeof(T) == 4 && choice == 0);
     if (held) {
         nblocks = (g.V + 127) / 128;
         int rc = lqx_ensure_partials(ctx, (size_t)nblocks);
@@ -300,7 +301,7 @@ static int hop_impl(lqx_field* chi, const lqx_field* const u[4], const lqx_field
         }                                                                                             \
     }
     // linear blocks: the CTA size is a launch-geometry knob (option "hop_block", the auto-tuner's choice)
-    const int hb = ctx->opt_hop_block;
+    const int hb = ctx->opt_hop_block ? ctx->opt_hop_block : ctx->tuned_hop_block[psi->prec == LQX_F32 ? 0 : 1];
     if (choice == 0 && hb == 32) { typedef LinearN<32> MAP; LQX_HOP_BODY }
     else if (choice == 0 && hb == 64) { typedef LinearN<64> MAP; LQX_HOP_BODY }
     else if (choice == 0 && hb == 256) { typedef LinearN<256> MAP; LQX_HOP_BODY }
@@ -611,9 +612,11 @@ extern "C" int lqx_jacobi_smear(lqx_field* chi, const lqx_field* const u[4], dou
     // launch geometry: options "jacobi_block" (N_threads: 32, 64, 128, 256) and "jacobi_sites" (N_site: 1, 2, 4)
     // defaults from the sweep on B200 (bench.py --sweep-geometry): 32 x 1 in fp32 -- as on the
     // paper's GTX 480 --, 128 x 1 in fp64 (where the block size makes no measurable difference)
-    const int ob = ctx->opt_jacobi_block;
+    const int pi = chi->prec == LQX_F32 ? 0 : 1;
+    const int ob = ctx->opt_jacobi_block ? ctx->opt_jacobi_block : ctx->tuned_jacobi_block[pi];
+    const int os = ctx->opt_jacobi_sites ? ctx->opt_jacobi_sites : ctx->tuned_jacobi_sites[pi];
     const int bs = (ob == 32 || ob == 64 || ob == 128 || ob == 256) ? ob : (chi->prec == LQX_F32 ? 32 : 128);
-    const int nsite = (ctx->opt_jacobi_sites == 2 || ctx->opt_jacobi_sites == 4) ? ctx->opt_jacobi_sites : 1;
+    const int nsite = (os == 2 || os == 4) ? os : 1;
     const int grid = (g.V + bs * nsite - 1) / (bs * nsite);
     const bool ferm = chi->kind == LQX_FERMION;
     for (int it = 0; it < iter; ++it) {

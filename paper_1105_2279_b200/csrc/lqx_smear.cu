@@ -432,32 +432,59 @@ int smear_launch_t(lqx_ctx* ctx, lqx_field* const uout[4], const lqx_field* cons
     for (int mu = 0; mu < 4; ++mu) o.u[mu] = uout[mu] ? (T*)uout[mu]->data : nullptr;
     const Links<T> in = make_links<T>(uin);
     const T c0 = (T)(1.0 - alpha), c1 = (T)(alpha / 6.0);
+    constexpr int PI = sizeof(T) == 4 ? 0 : 1;
     int variant = ctx->opt_smear_variant;
+    const int tile_saved = ctx->opt_tile;
+    if (variant == 0 && ctx->tuned_smear_variant[PI]) {  // the auto-tuner's choice, tile included
+        variant = ctx->tuned_smear_variant[PI];
+        if (ctx->opt_tile < 0) ctx->opt_tile = ctx->tuned_smear_tile[PI];
+    }
+    struct Restore {
+        lqx_ctx* c;
+        int t;
+        ~Restore() { c->opt_tile = t; }
+    } restore = {ctx, tile_saved};
     if (variant == 0 && sizeof(T) == 4) variant = 9;  // fp32 default: literal evaluation on row tiles (falls back to 3)
+    // executed FMA lane-ops per site: 48 (variant 8: 42; variant 2: 36 + halo) products x 108 + update 4 x 36
+    ctx->last_smear_lane_ops = 48 * 108 + 144;
     if (variant != 1 && variant != 2 && variant != 4 && variant != 6 && variant != 7 && variant != 8 && variant != 9) variant = 3;
     if (only_mu >= 0) variant = 1;
+    ctx->last_smear_variant = variant;
+    ctx->last_smear_kernel = variant == 9 ? "k_smear_rowlit" : variant == 8 ? "k_smear_rows" : variant == 7 ? "k_smear_tile"
+                           : variant == 6 ? "k_smear_staged" : variant == 4 ? "k_smear_mu4" : variant == 2 ? "k_smear_shared"
+                           : variant == 1 ? "k_smear_gather" : "k_smear_rolled";
+    if (variant == 8) ctx->last_smear_lane_ops = 42 * 108 + 144;
+    if (variant == 2) ctx->last_smear_lane_ops = 36 * 108 + 144;  // + the halo products of the tile in use
+    struct Fallback {  // a variant whose tiles do not fit hands over to the rolled kernel
+        lqx_ctx* c;
+        void operator()() const { c->last_smear_variant = 3, c->last_smear_kernel = "k_smear_rolled", c->last_smear_lane_ops = 48 * 108 + 144; }
+    } fell_back = {ctx};
     if (variant == 9) {
         int rc = 1;
         if (sizeof(T) == 4) rc = lqx_smear_rowlit_launch(ctx, reinterpret_cast<const Links<float>&>(in), reinterpret_cast<const LinksOut<float>&>(o), (float)c0, (float)c1, plaq);
         if (rc <= 0) return rc;
         variant = 3;
+        fell_back();
     }
     if (variant == 8) {
         int rc = 1;
         if (sizeof(T) == 4) rc = lqx_smear_rows_launch(ctx, reinterpret_cast<const Links<float>&>(in), reinterpret_cast<const LinksOut<float>&>(o), (float)c0, (float)c1, plaq);
         if (rc <= 0) return rc;
         variant = 3;  // fp64, or the lattice does not fit the row tiles
+        fell_back();
     }
     if (variant == 7) {
         const int rc = lqx_smear_tile_launch(ctx, in, o, c0, c1, plaq);
         if (rc <= 0) return rc;
         variant = 3;  // no tile of this kernel divides the lattice
+        fell_back();
     }
     if (variant == 6) {
         int rc = 1;
         if (sizeof(T) == 4) rc = lqx_smear_staged_launch(ctx, reinterpret_cast<const Links<float>&>(in), reinterpret_cast<const LinksOut<float>&>(o), (float)c0, (float)c1, plaq);
         if (rc <= 0) return rc;
         variant = 3;  // fp64, or the lattice is not a multiple of the staged kernel's tile
+        fell_back();
     }
     if (variant == 2) {
         // option "tile": 1 = 8x4x4x2 (256 threads), 2 = 8x4x2x2, 3 = 4x4x4x2, 4 = 16x4x2x2 (256), 5 = 16x2x2x2
@@ -471,6 +498,7 @@ int smear_launch_t(lqx_ctx* ctx, lqx_field* const uout[4], const lqx_field* cons
         else if ((t == 3 || t < 0) && TileC::fits(g)) rc = smear_shared_launch<T, TileC, MB128>(ctx, in, o, c0, c1, plaq);
         if (rc <= 0) return rc;
         variant = 3;  // no tile of this kernel divides the lattice
+        fell_back();
     }
     if (variant == 4) {
         // option "tile": 1 = 8x2x2x2, 2 = 16x2x2x1, 3 = 4x4x2x2 (64 sites); 4 = 8x4x2x2, 5 = 16x2x2x2 (128 sites)
@@ -484,6 +512,7 @@ int smear_launch_t(lqx_ctx* ctx, lqx_field* const uout[4], const lqx_field* cons
         else if (t == 5 && TileE::fits(g)) rc = smear_mu4_launch<T, TileE, 1>(ctx, in, o, c0, c1, plaq);
         if (rc <= 0) return rc;
         variant = 3;  // no tile of this kernel divides the lattice
+        fell_back();
     }
     const int choice = lqx_pick_tile(ctx, sizeof(T) == 4 ? 1 : 0);  // measured best
     int nblocks = 0;

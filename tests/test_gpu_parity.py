@@ -706,6 +706,68 @@ def test_jacobi_smear_every_launch_geometry(lqx, prec, kind):
                     f.free()
 
 
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+@pytest.mark.parametrize("dims", [(16, 8, 4, 4), DIMS_RAGGED])
+def test_autotune_keeps_a_geometry_that_agrees_with_the_oracle(lqx, dims, prec):
+    """lqx_autotune: the table lists every candidate with a time, exactly one is kept per kernel, an
+    explicit option still overrides it, and the calls that follow -- now running the kept geometry -- agree with the oracle."""
+    tv = orc.truth_variant(prec)
+    P = _prec(lqx, prec)
+    u = _links(5, dims, prec)
+    psi = _gauss(5, 9, dims, "f", prec)
+    with lqx.Lattice(dims) as lat:
+        for cls, nkept in ((lqx.K_SMEAR, 1), (lqx.K_PLAQUETTE, 1), (lqx.K_HOP, 2)):
+            rows = lat.autotune(cls, P, reps=2)
+            assert rows and all(r["ms"] > 0 and r["kernel_class"] == cls and r["prec"] == P for r in rows)
+            assert sum(r["chosen"] for r in rows) == nkept
+        t = lat.tuned(lqx.K_SMEAR, P)
+        assert t[0] in (3, 9)
+        hb, jb, js = lat.tuned(lqx.K_HOP, P)[:3]
+        assert hb in (32, 64, 128, 256) and jb in (32, 64, 128, 256) and js in (1, 2, 4)
+        assert lat.tuned(lqx.K_PLAQUETTE, P)[0] in (1, 2)
+        fu = [lat.from_host(x) for x in u]
+        out = [lat.alloc(lqx.COLORMAT, P) for _ in range(4)]
+        p = lqx.smear_step(out, fu, 0.5, want_plaq_in=True)
+        assert lat.smear_info()[0] == t[0]
+        want = orc.smear_step(dims, u, 0.5, tv)
+        for mu in range(4):
+            assert site_rel_err(out[mu].pop(), want[mu]) < TOL[prec]
+        psum = orc.plaquette_sum(dims, u, tv)
+        scale = np.sqrt(18.0 * lat.volume)
+        assert abs(p - psum) / max(abs(psum), scale) < RTOL[prec]
+        assert abs(lqx.plaquette(fu)[0] - psum) / max(abs(psum), scale) < RTOL[prec]
+        fpsi, chi = lat.from_host(psi), lat.alloc(lqx.FERMION, P)
+        lqx.hop(chi, fu, fpsi)
+        assert site_rel_err(chi.pop(), orc.hop(dims, u, psi, tv)) < TOL[prec]
+        tmp = [lat.alloc(lqx.FERMION, P) for _ in range(2)]
+        lqx.jacobi_smear(fpsi, fu, 0.21, 3, 3, 1.7, tmp)
+        assert site_rel_err(fpsi.pop(), orc.jacobi_smear(dims, u, psi, 0.21, 3, 3, 1.7, tv)) < TOL[prec] * 3
+        # an explicit option wins over the tuned choice
+        lat.set_option("smear_variant", 1)
+        lqx.smear_step(out, fu, 0.5)
+        assert lat.smear_info()[0] == 1 and lat.smear_info()[2] == "k_smear_gather"
+
+
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+def test_hop_every_block_size(lqx, prec):
+    dims = DIMS_RAGGED
+    u = _links(2, dims, prec)
+    psi = _gauss(2, 10, dims, "f", prec)
+    want = orc.hop(dims, u, psi, orc.truth_variant(prec))
+    with lqx.Lattice(dims) as lat:
+        fu = [lat.from_host(t) for t in u]
+        fpsi, chi = lat.from_host(psi), lat.alloc(lqx.FERMION, _prec(lqx, prec))
+        first = None
+        for hb in (0, 32, 64, 128, 256):
+            lat.set_option("hop_block", hb)
+            lqx.scale(chi, 0.0, chi)
+            lqx.hop(chi, fu, fpsi)
+            got = chi.pop()
+            assert site_rel_err(got, want) < TOL[prec], hb
+            first = got if first is None else first
+            assert np.array_equal(got, first), hb
+
+
 def test_jacobi_smear_config2_size(lqx):
     """16^3x32 fp32 (the lattice of configs[1], a Table-1 size of the paper), 10 iterations, fermion."""
     cfg = li.CONFIGS["c2"]
