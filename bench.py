@@ -37,6 +37,8 @@ WORKLOADS = {
     "c4": dict(cfg="c4", recipe="near_unit", desc="BASELINE configs[3]: 48^3x96 fp32 near-unit SU(3) (exp(0.1iH) reunitarised), "
                "iterated smear steps a=0.5, plaquette after each"),
     "c3": dict(cfg="c3", recipe="haar", desc="BASELINE configs[2]: 32^3x64 fp64 Haar SU(3), smear steps a=0.5 + plaquette"),
+    # only with --kernel-only --only hop: the lattice of BASELINE configs[1] (16^3x32 fp32), for the ncu capture of k_hop
+    "c2": dict(cfg="c2", recipe="haar", desc="BASELINE configs[1]: 16^3x32 fp32 Haar SU(3) + Gaussian fermion, hop"),
 }
 
 
@@ -49,27 +51,35 @@ def _peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)", 1965.0
 
 
-def _ncu_traffic():
-    """DRAM bytes per launch of the dominant kernel from the newest committed ncu capture
-    (profiles/rNN?_smear*.md, rows dram__bytes_read.sum / dram__bytes_write.sum, last launch column).
-    bench.py never runs under ncu; this is the recorded figure, or (None, reason)."""
+def _ncu_capture(kernel_name, prec="f32"):
+    """Figures of the newest committed ncu capture OF THIS KERNEL: the profiles/r*.md file (newest round letter last)
+    whose `Kernel Name` row names `kernel_name`.  Returns (dict of metric -> value in base units, file) or
+    (None, reason).  bench.py never runs under ncu; these are recorded figures, used for `traffic` and for naming
+    the busiest unit -- a capture of another kernel is never attached to this line."""
     import glob
     import re
 
-    files = sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_smear*.md")))
-    if not files:
-        return None, "no ncu capture under profiles/"
-    vals = {}
-    for line in open(files[-1]):
-        m = re.match(r"\|\s*dram__bytes_(read|write)\.sum\s*\|\s*(\w+)\s*\|(.*)\|\s*$", line)
-        if m:
-            scale = {"Gbyte": 1e9, "Mbyte": 1e6, "Kbyte": 1e3, "byte": 1.0}.get(m.group(2))
-            cols = [c.strip() for c in m.group(3).split("|")]
-            if scale and cols:
-                vals[m.group(1)] = float(cols[-1]) * scale
-    if len(vals) != 2:
-        return None, "dram__bytes rows not found in " + os.path.basename(files[-1])
-    return vals["read"] + vals["write"], "profiles/" + os.path.basename(files[-1])
+    for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "r*.md")), reverse=True):
+        text = open(path).read()
+        m = re.search(r"^\|\s*Kernel Name\s*\|[^|]*\|(.*)\|\s*$", text, re.M)
+        if not m or not re.search(r"\b" + re.escape(kernel_name) + r"\b", m.group(1)):
+            continue
+        if ("<double" in m.group(1) and prec == "f32") or ("<float" in m.group(1) and prec == "f64"):
+            continue  # the other precision's instantiation of this kernel
+        vals = {}
+        for line in text.splitlines():
+            mm = re.match(r"\|\s*([a-z0-9_.]+)\s*\|\s*([\w/%]*)\s*\|(.*)\|\s*$", line)
+            if not mm:
+                continue
+            cols = [c.strip() for c in mm.group(3).split("|")]
+            try:
+                x = float(cols[-1])
+            except ValueError:
+                continue
+            vals[mm.group(1)] = x * {"Gbyte": 1e9, "Mbyte": 1e6, "Kbyte": 1e3}.get(mm.group(2), 1.0)
+        if "dram__bytes_read.sum" in vals and "dram__bytes_write.sum" in vals:
+            return vals, "profiles/" + os.path.basename(path)
+    return None, f"no committed ncu capture of {kernel_name} under profiles/"
 
 
 class ClockSampler(threading.Thread):
@@ -212,9 +222,20 @@ def _cpu_baseline(orc, dims, prec, host_links, target_s=12.0):
     while n == v and t < 0.75 * target_s:  # the whole field is a few seconds of CPU work: time several whole steps
         t += run(n)
         passes += 1
-    return {"value": passes * n / t, "unit": "site-updates/s", "cores": orc.num_threads(), "kind": "oracle",
-            "sample": f"{passes} pass(es) over the first {n} of {v} sites of the full-size field (all 4 directions + "
-                      f"plaquette), oracle variant {variant}, {t:.1f} s"}
+    out = {"value": passes * n / t, "unit": "site-updates/s", "cores": orc.num_threads(), "kind": "oracle",
+           "sample": f"{passes} pass(es) over the first {n} of {v} sites of the full-size field (all 4 directions + "
+                     f"plaquette), oracle variant {variant}, {t:.1f} s"}
+    # SURVEY 8(d) timing protocol: also ONE host thread, on a sample a tenth of the all-core budget
+    nthreads = orc.num_threads()
+    try:
+        orc.set_num_threads(1)
+        n1 = int(min(v, max(2000, out["value"] / max(nthreads, 1) * target_s * 0.25)))
+        t1 = run(n1)
+        out["single_thread"] = {"value": n1 / t1, "unit": "site-updates/s", "cores": 1,
+                                "sample": f"the first {n1} sites, {t1:.1f} s"}
+    finally:
+        orc.set_num_threads(nthreads)
+    return out
 
 
 def _time_kernel(torch, fn, reps, flush=None):
@@ -269,10 +290,12 @@ def jacobi_listing(lqx, chi, u, kappa, iters, no_smear_dir, norm, work, fused):
     lqx.expr_eval(chi, (1.0 / norm) * L(chi))                             # chi /= norm (E4; reciprocal multiply, A22)
 
 
-def _extras(torch, lqx, li, hbm_gbs):
+def _extras(torch, lqx, li, hbm_gbs, tune=None):
     """Per-kernel numbers for the other BASELINE configs (same JSON line, key "kernels"): device time
-    per launch, algorithmic GB/s (SURVEY 8(d) bytes/site) and its fraction of the measured HBM peak."""
+    per launch, algorithmic GB/s (SURVEY 8(d) bytes/site) and its fraction of the measured HBM peak.
+    tune: dict that receives the lqx_autotune tables of the hop / Jacobi geometries (Figs. 1-2 on B200)."""
     out = []
+    tune = {} if tune is None else tune
     flush = torch.zeros(64 * 1024 * 1024, dtype=torch.float32, device="cuda")  # 256 MB > L2
 
     def add(name, prec, sites, reals_per_site, flops_per_site, fn, reps=10, cold=False, lat=None, kclass=None):
@@ -314,8 +337,18 @@ def _extras(torch, lqx, li, hbm_gbs):
         psi = lat.alloc(lqx.FERMION, lqx.F32).import_dev(li.gaussian_field(2, 10, dims, "f", "f32", device="cuda"))
         chi = lat.alloc(lqx.FERMION, lqx.F32)
         v = lat.volume
+        tune["hop_and_jacobi_step_16^3x32_f32"] = lat.autotune(lqx.K_HOP, lqx.F32, 5)
+        # what a single L2-cold launch of this size can reach at all when timed by events: a plain copy moving the same
+        # 63 MB (31.5 MB read + 31.5 MB written), measured the same way -- the event pair alone costs ~6 us
+        ca = torch.empty(v * 120 // 2, dtype=torch.float32, device="cuda")
+        cb = torch.empty_like(ca)
+        add("copy of the same 63 MB, torch (L2-cold): the floor of one cold launch timed by events", "f32", v, 120, 0,
+            lambda: cb.copy_(ca), reps=20, cold=True)
+        copy_ms = out[-1]["ms"]
+        del ca, cb
         add("hop c2 (L2-cold)", "f32", v, 120, 2280, lambda: lqx.hop(chi, u, psi), reps=20, cold=True)
         out[-1]["l2"] = "flushed between launches"
+        out[-1]["frac_of_copy_same_bytes"] = copy_ms / out[-1]["ms"]
         add("hop c2 (L2-warm)", "f32", v, 120, 2280, lambda: lqx.hop(chi, u, psi), reps=20)
         out[-1]["l2"] = "warm: 63 MB working set fits the 126 MB L2"
         def hop20():
@@ -357,6 +390,7 @@ def _extras(torch, lqx, li, hbm_gbs):
                 del a
             psi = lat.alloc(lqx.FERMION, pcode).import_dev(li.gaussian_field(2, 10, dims, "f", prec, device="cuda"))
             chi = lat.alloc(lqx.FERMION, pcode)
+            tune[f"hop_and_jacobi_step_32^3x64_{prec} (the lattice of the paper's Figs. 1-2)"] = lat.autotune(lqx.K_HOP, pcode, 3)
             add("hop 32^3x64 (not a BASELINE config; size check)", prec, lat.volume, 120, 2280, lambda: lqx.hop(chi, u, psi), reps=10)
             eh = None
             for mu in range(4):  # the Listing's E1/E2 expression, summed over mu, as ONE run-time expression
@@ -491,6 +525,23 @@ def run_sweep(args):
                                                                 "slightly better than 1 (PAPER.md:248, :260)"}}))
 
 
+def _kernel_only_other(args, torch, lqx, li, lat, u):
+    """--kernel-only --only plaquette|hop: a few launches of that kernel on the workload's lattice (what ncu wraps)."""
+    P = u[0].prec
+    if args.only == "plaquette":
+        fn = lambda: lqx.plaquette(u)
+    else:
+        psi = lat.alloc(lqx.FERMION, P).import_dev(li.gaussian_field(2, 10, lat.dims, "f", "f32" if P == lqx.F32 else "f64", device="cuda"))
+        chi = lat.alloc(lqx.FERMION, P)
+        fn = lambda: lqx.hop(chi, u, psi)
+    for _ in range(3):
+        fn()
+    torch.cuda.synchronize()
+    med, best = _time_kernel(torch, fn, max(args.steps, 3))
+    print(json.dumps({"kernel_only": args.only, "workload": args.workload, "ms": med, "ms_best": best}))
+    lat.close()
+
+
 def run_ours(args):
     import torch
 
@@ -520,6 +571,20 @@ def run_ours(args):
     fma2_peak = lat.bench_fma_peak(1) if prec == "f32" else None
     copy_peak = lat.bench_copy_peak(1 << 30)
 
+    if args.smear_variant:
+        lat.set_option("smear_variant", args.smear_variant)
+    if args.tile >= 0:
+        lat.set_option("tile", args.tile)
+    if args.block:
+        lat.set_option("block", args.block)
+    tune_tables = None
+    if args.autotune or (world == 1 and not args.kernel_only and not args.smear_variant):
+        # NEXT-3: the library times its launch geometries on this lattice and keeps the winners;
+        # the tables go into the JSON line (the B200 counterpart of the paper's Figs. 1-2)
+        tune_tables = {"smear": lat.autotune(lqx.K_SMEAR, u[0].prec, 3), "plaquette": lat.autotune(lqx.K_PLAQUETTE, u[0].prec, 3)}
+    if args.kernel_only and args.only != "smear":
+        return _kernel_only_other(args, torch, lqx, li, lat, u)
+
     lqx.smear_iterate(u, tmp, ALPHA, W)  # warm-up (>= 3 steps)
     torch.cuda.synchronize()
     lat.set_option("time_kernels", 1)
@@ -545,26 +610,39 @@ def run_ours(args):
     value = replica_value(world, V, K, ms)
     k_ms = smear_ms / max(smear_n, 1)  # average duration of the dominant kernel inside the timed region
     alg_bytes = V * SMEAR_REALS_PER_SITE * esize
-    variant = "literal"
-    lane_ops = V * SMEAR_LANE_OPS[variant]
+    # the kernel that actually ran (options, tuned choice and fall-backs resolved by the library) and what it executes
+    variant, lane_ops_site, kname = lat.smear_info()
+    lane_ops = V * lane_ops_site
     # FP-pipe peak from unit counts and clocks: 148 SMs x 128 fp32 (64 fp64) FMA lanes x sm_max
     alu_peak_tflops = 148 * (128 if prec == "f32" else 64) * 2 * sm_max * 1e6 / 1e12
-    traffic, traffic_src = _ncu_traffic() if (args.workload == "c4") else (None, "no capture for this workload")
+    cap, cap_src = _ncu_capture(kname, prec)
+    traffic = (cap["dram__bytes_read.sum"] + cap["dram__bytes_write.sum"]) if cap else None
+    alu_frac = 2 * lane_ops / (k_ms * 1e-3) / 1e12 / alu_peak_tflops
+    hbm_frac = alg_bytes / (k_ms * 1e-3) / 1e9 / hbm_gbs
     roofline = {
-        "kernel": "k_smear_rolled (staple sum + smear update, fused input plaquette)",
+        "kernel": f"{kname} (staple sum + smear update of all four links, fused input plaquette; smear_variant {variant})",
         "bound": "alu", "achieved": 2 * lane_ops / (k_ms * 1e-3) / 1e12, "peak": alu_peak_tflops, "unit": "TFLOP/s",
-        "frac": 2 * lane_ops / (k_ms * 1e-3) / 1e12 / alu_peak_tflops,
+        "frac": alu_frac,
         "peak_source": f"148 SMs x {128 if prec == 'f32' else 64} FMA lanes x 2 x {sm_max:.0f} MHz (DESIGN.md sec.7); "
                        f"FMA-chain micro-benchmark in this run: {2 * fma_peak / 1e12:.1f} TFLOP/s"
                        + (f", packed f32x2: {2 * fma2_peak / 1e12:.1f}" if fma2_peak else ""),
-        "frac_at_measured_clock": (2 * lane_ops / (k_ms * 1e-3) / 1e12) / (alu_peak_tflops * clocks["sm_mhz"] / sm_max)
-        if clocks.get("sm_mhz") else None,
-        "flops_counted": f"executed FMA lane-ops x 2 ({SMEAR_LANE_OPS[variant]} lane-ops/site, {variant} evaluation)",
+        "frac_at_measured_clock": alu_frac / (clocks["sm_mhz"] / sm_max) if clocks.get("sm_mhz") else None,
+        "flops_counted": f"executed FMA lane-ops x 2 ({lane_ops_site} lane-ops/site as reported by lqx_smear_info for this kernel)",
         "traffic": traffic, "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum)",
-        "traffic_source": traffic_src, "ms_per_launch": k_ms, "launches": smear_n,
+        "traffic_source": cap_src, "ms_per_launch": k_ms, "launches": smear_n,
         "hbm": {"bound": "hbm", "achieved": alg_bytes / (k_ms * 1e-3) / 1e9, "peak": hbm_gbs, "unit": "GB/s",
-                "frac": alg_bytes / (k_ms * 1e-3) / 1e9 / hbm_gbs, "peak_source": hbm_src,
+                "frac": hbm_frac, "peak_source": hbm_src,
                 "copy_kernel_this_run_gbs": copy_peak / 1e9, "alg_bytes_per_launch": alg_bytes},
+        # neither roof is what the kernel runs into: ncu names the unit; from the committed capture
+        "busiest_units_ncu": ({k: cap[k] for k in ("l1tex__data_pipe_lsu_wavefronts.avg.pct_of_peak_sustained_elapsed",
+                                                   "smsp__issue_active.avg.pct_of_peak_sustained_active",
+                                                   "sm__pipe_fma_cycles_active.avg.pct_of_peak_sustained_active",
+                                                   "lts__throughput.avg.pct_of_peak_sustained_elapsed",
+                                                   "gpu__dram_throughput.avg.pct_of_peak_sustained_elapsed") if k in cap}
+                              if cap else None),
+        "l1_data_pipe_ceiling": "128 B/clk/SM = 32 fp32 operands per clock for 128 FMA lanes: the literal evaluation moves "
+                                "76 matrices x 72 B per site through it (42.8 clk/site) for 5328 lane-ops (41.6 clk/site)",
+        "north_star_target": {"text": "smear step >= 70 % of the HBM roofline", "hbm_frac": hbm_frac, "met": bool(hbm_frac >= 0.70)},
     }
     line = {
         "metric": "smear-step site-updates/s", "value": value, "unit": "site-updates/s", "n_gpus": world,
@@ -572,7 +650,7 @@ def run_ours(args):
         "vs_baseline": None, "dtype": prec, "data": "synthetic",
         "config": {"workload": wl["desc"], "dims": list(dims), "sites": V, "alpha": ALPHA, "l2": "inputs larger than L2 "
                    f"({2 * alg_bytes / 2 / 1e9:.2f} GB read+written per step)", "parallelism": "replicas only" if world > 1 else "1 GPU",
-                   "smear_variant": variant},
+                   "smear_variant": variant, "smear_kernel": kname},
         "gflops_canonical": world * V * K * SMEAR_CANONICAL_FLOPS / (ms * 1e-3) / 1e9,
         "hbm_gbs_algorithmic": world * (K * alg_bytes + V * PLAQ_REALS_PER_SITE * esize) / (ms * 1e-3) / 1e9,
         "plaquette_avg_after_each_step": plaqs,
@@ -581,6 +659,9 @@ def run_ours(args):
                               "plaquette_launches": plaq_n, "timed_region": ms},
     }
 
+    if tune_tables is not None:
+        line["autotune"] = {"what": "lqx_autotune on this lattice: ms per launch of every candidate geometry, chosen = kept "
+                                    "(param: smear = [smear_variant, tile], plaquette = [plaq_variant, 0])", **tune_tables}
     if not args.kernel_only:
         # ---- e2e: the public host-buffer call, H2D + D2H inside the timed region, every step; under torchrun every
         # rank runs its replica from its own pinned buffers and the job takes as long as the slowest rank
@@ -614,7 +695,11 @@ def run_ours(args):
     lat.close()
     torch.cuda.empty_cache()
     if world == 1 and not args.no_extras and not args.kernel_only:
-        line["kernels"] = _extras(torch, lqx, li, hbm_gbs)
+        more = {}
+        line["kernels"] = _extras(torch, lqx, li, hbm_gbs, more)
+        line.setdefault("autotune", {"what": "lqx_autotune"}).update(more)
+        line["autotune"]["what_hop"] = ("hop tables: param[0] > 0 = CTA size of lqx_hop; param[0] < 0 = N_threads = -param[0], "
+                                        "N_site = param[1] of one lqx_jacobi_smear iteration (PAPER.md:117-126), ms per iteration")
     if rank == 0:
         print(json.dumps(line))
     if world > 1:
@@ -690,6 +775,12 @@ def main():
     ap.add_argument("--extras-only", action="store_true",
                     help="only the per-kernel numbers of configs 2, 3, 5 and the Jacobi routine (one JSON line with key "
                          "'kernels'): the command ncu wraps for the catalogue / hop / Jacobi kernels")
+    ap.add_argument("--smear-variant", type=int, default=0, help="lqx option smear_variant (0 = library default / tuned)")
+    ap.add_argument("--tile", type=int, default=-1, help="lqx option tile (-1 = automatic)")
+    ap.add_argument("--block", type=int, default=0, help="lqx option block (slab thickness of the row-tile kernels)")
+    ap.add_argument("--only", default="smear", choices=["smear", "plaquette", "hop"],
+                    help="with --kernel-only: the kernel to run (the command ncu wraps for that kernel)")
+    ap.add_argument("--autotune", action="store_true", help="let lqx_autotune pick the launch geometries before timing")
     ap.add_argument("--kernel-only", action="store_true",
                     help="timed device region only (no e2e, no cpu_baseline, no extras): the command ncu wraps")
     ap.add_argument("--e2e-steps", type=int, default=5, help="cap on host-buffer steps timed for e2e")
