@@ -570,6 +570,9 @@ def run_ours(args):
     fma_peak = lat.bench_fma_peak(fma_kind)
     fma2_peak = lat.bench_fma_peak(1) if prec == "f32" else None
     copy_peak = lat.bench_copy_peak(1 << 30)
+    # the FMA pipe fed the way the kernel feeds it: 3x3 complex products on register operands (three distinct register
+    # operands per instruction, FFMA2 with broadcast / swapped operands in fp32) instead of one dependent chain
+    prod_peak = lat.bench_fma_peak(3 if prec == "f32" else 4)
 
     if args.smear_variant:
         lat.set_option("smear_variant", args.smear_variant)
@@ -627,6 +630,8 @@ def run_ours(args):
                        f"FMA-chain micro-benchmark in this run: {2 * fma_peak / 1e12:.1f} TFLOP/s"
                        + (f", packed f32x2: {2 * fma2_peak / 1e12:.1f}" if fma2_peak else ""),
         "frac_at_measured_clock": alu_frac / (clocks["sm_mhz"] / sm_max) if clocks.get("sm_mhz") else None,
+        "product_stream_peak_tflops": 2 * prod_peak / 1e12,
+        "frac_of_product_stream_peak": (2 * lane_ops / (k_ms * 1e-3)) / (2 * prod_peak),
         "flops_counted": f"executed FMA lane-ops x 2 ({lane_ops_site} lane-ops/site as reported by lqx_smear_info for this kernel)",
         "traffic": traffic, "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum)",
         "traffic_source": cap_src, "ms_per_launch": k_ms, "launches": smear_n,

@@ -241,8 +241,10 @@ int lqx_smear_iterate_host(lqx_ctx* ctx, lqx_prec prec, const void* const host_u
 /* ---------------------------------------------------------------------------------------------
  * Harness support: device micro-benchmarks that give the roofline denominators.
  * ------------------------------------------------------------------------------------------- */
-/* kind: 0 = fp32 FMA, 1 = packed fp32x2 FMA, 2 = fp64 FMA.  Returns achieved FMA lane-ops/s
- * (one fused multiply-add on one real = 1 lane-op = 2 flop) in *lane_ops_per_s. */
+/* kind: 0 = fp32 FMA, 1 = packed fp32x2 FMA, 2 = fp64 FMA (one dependent chain per accumulator, constant multiplicands);
+ * 3 = fp32, 4 = fp64: a stream of 3x3 complex products on register operands -- the instruction mix of the lattice
+ * kernels (fp32: FFMA2 with broadcast and swapped operands), three distinct register operands per instruction.
+ * Returns achieved FMA lane-ops/s (one fused multiply-add on one real = 1 lane-op = 2 flop) in *lane_ops_per_s. */
 int lqx_bench_fma_peak(lqx_ctx* ctx, int kind, double* lane_ops_per_s);
 /* Plain device copy of `bytes` bytes (read + write counted): achieved bytes/s. */
 int lqx_bench_copy_peak(lqx_ctx* ctx, size_t bytes, double* bytes_per_s);

@@ -68,6 +68,37 @@ __global__ void __launch_bounds__(256) k_fma_peak(int iters, float seed, double*
     }
 }
 
+// The same pipes fed the way the lattice kernels feed them: 3x3 complex products on matrices held in registers
+// (lqx_internal.cuh mac_nn / mac_na: 108 FMA lane-ops each; fp32 = 54 FFMA2 with broadcast and swapped operands), i.e.
+// three DISTINCT register operands per instruction instead of the chain benchmark's one.  What this reaches is the
+// FMA rate a product-shaped instruction stream can have at all (register-file ports included).
+template <typename T>
+__global__ void __launch_bounds__(256) k_product_peak(int iters, T seed, double* __restrict__ sink) {
+    Mat3<T> a, b, c;
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            a.re[i][j] = (i == j ? T(1) : T(0)) + seed * T(1e-3) * T(threadIdx.x % 7 + i);
+            a.im[i][j] = seed * T(1e-3) * T(j + 1);
+            b.re[i][j] = (i == j ? T(1) : T(0)) - seed * T(1e-3) * T(i + j);
+            b.im[i][j] = seed * T(2e-3) * T(i);
+            c.re[i][j] = c.im[i][j] = T(0);
+        }
+    for (int it = 0; it < iters; ++it) {
+        mac_nn(c, a, b);  // c += a b
+        mac_na(a, c, b);  // a += c adj(b)
+        mac_an(b, a, c);  // b += adj(a) c   (values grow; only the instruction stream matters)
+        mac_nn(c, b, a);
+    }
+    T t = T(0);
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+        for (int j = 0; j < 3; ++j) t += a.re[i][j] + b.im[i][j] + c.re[i][j];
+    if (t == T(123.456)) sink[0] = (double)t;
+}
+
 __global__ void __launch_bounds__(256) k_copy(size_t n16, const uint4* __restrict__ src, uint4* __restrict__ dst) {
     const size_t step = (size_t)gridDim.x * blockDim.x;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n16; i += step) dst[i] = src[i];
@@ -76,7 +107,7 @@ __global__ void __launch_bounds__(256) k_copy(size_t n16, const uint4* __restric
 }  // namespace
 
 extern "C" int lqx_bench_fma_peak(lqx_ctx* ctx, int kind, double* lane_ops_per_s) {
-    if (!ctx || !lane_ops_per_s || kind < 0 || kind > 2) return LQX_EINVAL;
+    if (!ctx || !lane_ops_per_s || kind < 0 || kind > 4) return LQX_EINVAL;
     LQX_CUDA(ctx, cudaSetDevice(ctx->device));
     const int grid = ctx->num_sms * 8, block = 256, iters = 2048;
     cudaEvent_t e0, e1;
@@ -87,13 +118,16 @@ extern "C" int lqx_bench_fma_peak(lqx_ctx* ctx, int kind, double* lane_ops_per_s
         LQX_CUDA(ctx, cudaEventRecord(e0, ctx->stream));
         if (kind == 0) k_fma_peak<0><<<grid, block, 0, ctx->stream>>>(iters, 1.0f, ctx->d_result + 63);
         else if (kind == 1) k_fma_peak<1><<<grid, block, 0, ctx->stream>>>(iters, 1.0f, ctx->d_result + 63);
-        else k_fma_peak<2><<<grid, block, 0, ctx->stream>>>(iters, 1.0f, ctx->d_result + 63);
+        else if (kind == 2) k_fma_peak<2><<<grid, block, 0, ctx->stream>>>(iters, 1.0f, ctx->d_result + 63);
+        else if (kind == 3) k_product_peak<float><<<grid, block, 0, ctx->stream>>>(iters, 1e-3f, ctx->d_result + 63);
+        else k_product_peak<double><<<grid, block, 0, ctx->stream>>>(iters, 1e-3, ctx->d_result + 63);
         LQX_LAUNCH_CHECK(ctx);
         LQX_CUDA(ctx, cudaEventRecord(e1, ctx->stream));
         LQX_CUDA(ctx, cudaEventSynchronize(e1));
         float ms = 0.f;
         LQX_CUDA(ctx, cudaEventElapsedTime(&ms, e0, e1));
-        const double lanes = (double)grid * block * (double)iters * 8.0 * 16.0 * (kind == 1 ? 2.0 : 1.0);
+        const double lanes = kind >= 3 ? (double)grid * block * (double)iters * 4.0 * 108.0
+                                       : (double)grid * block * (double)iters * 8.0 * 16.0 * (kind == 1 ? 2.0 : 1.0);
         if (rep > 0) best = std::max(best, lanes / (ms * 1e-3));
     }
     cudaEventDestroy(e0);
