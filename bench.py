@@ -542,6 +542,74 @@ def _kernel_only_other(args, torch, lqx, li, lat, u):
     lat.close()
 
 
+def run_tsplit(args):
+    """NEXT-4: ONE global lattice decomposed along t over the ranks, halo exchange over
+    torch.distributed (NCCL) overlapped with the interior launch (paper_1105_2279_b200/tsplit.py).  Not the contract
+    (BASELINE.json: replicas only) -- an extra mode: `torchrun ... bench.py --tsplit --gpus N`; with one GPU the halos
+    are the rank's own periodic images, which measures what the split formulation costs by itself."""
+    import torch
+
+    import lattice_inputs as li
+    import paper_1105_2279_b200 as lqx
+    from paper_1105_2279_b200 import tsplit
+
+    rank, world, local, barrier, vmax = _dist()
+    torch.cuda.set_device(local)
+    wl = WORKLOADS[args.workload]
+    cfg = li.CONFIGS[wl["cfg"]]
+    gdims, prec = cfg["dims"], cfg["prec"]
+    P = lqx.F32 if prec == "f32" else lqx.F64
+    K, W = args.steps, max(args.warmup, 3)
+    ldims = tsplit.local_dims(gdims, world)
+    lat = lqx.Lattice(ldims, device=local)
+    comm = tsplit.DistComm() if world > 1 else tsplit.SelfComm()
+    ts = tsplit.TSplit(tsplit.LqxBackend(lqx, lat), comm, gdims)
+    # synthetic links of the workload's recipe on the local lattice (own slices and halos alike; the first exchange
+    # overwrites the halos): timing does not depend on which slab of the global field a rank holds
+    u = []
+    for mu in range(4):
+        z = (li.near_unit_su3_complex(cfg["seed"] + 100 * rank, mu, lat.volume, 0.1, f"cuda:{local}") if wl["recipe"] == "near_unit"
+             else li.haar_su3_complex(cfg["seed"] + 100 * rank, mu, lat.volume, f"cuda:{local}"))
+        a = li._as_real(z, prec)
+        u.append(lat.alloc(lqx.COLORMAT, P).import_dev(a))
+        del z, a
+    tmp = [lat.alloc(lqx.COLORMAT, P) for _ in range(4)]
+    torch.cuda.synchronize()
+    for _ in range(W):
+        ts.smear_step(tmp, u, ALPHA)
+        u, tmp = tmp, u
+    torch.cuda.synchronize()
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(K):
+        ts.smear_step(tmp, u, ALPHA)
+        u, tmp = tmp, u
+    e1.record()
+    torch.cuda.synchronize()
+    barrier()
+    ms = vmax(e0.elapsed_time(e1))
+    plaq = ts.plaquette_sum(u) / (18.0 * li.volume(gdims))
+    V = li.volume(gdims)
+    esize = 4 if prec == "f32" else 8
+    if rank == 0:
+        print(json.dumps({
+            "metric": "smear-step site-updates/s", "value": V * K / (ms * 1e-3), "unit": "site-updates/s", "n_gpus": world,
+            "steps": K, "warmup": W, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+            "dtype": prec, "data": "synthetic", "mode": "tsplit",
+            "config": {"workload": wl["desc"] + " -- ONE lattice decomposed along t", "dims": list(gdims), "local_dims": list(ldims),
+                       "parallelism": f"t-split x{world}: per step and rank 2 x 4 halo slices = "
+                                      f"{2 * 4 * ldims[0] * ldims[1] * ldims[2] * 18 * esize / 1e6:.1f} MB exchanged "
+                                      + ("over NCCL" if world > 1 else "(one rank: its own periodic images, device copies)")
+                                      + ", overlapped with the interior launch", "l2": "inputs larger than L2"},
+            "plaquette_avg_after_last_step": plaq}))
+    lat.close()
+    if world > 1:
+        import torch.distributed as dist
+
+        dist.destroy_process_group()
+
+
 def run_ours(args):
     import torch
 
@@ -785,6 +853,8 @@ def main():
     ap.add_argument("--block", type=int, default=0, help="lqx option block (slab thickness of the row-tile kernels)")
     ap.add_argument("--only", default="smear", choices=["smear", "plaquette", "hop"],
                     help="with --kernel-only: the kernel to run (the command ncu wraps for that kernel)")
+    ap.add_argument("--tsplit", action="store_true",
+                    help="NEXT-4 extra mode: one global lattice decomposed along t over the ranks (halo exchange), not replicas")
     ap.add_argument("--autotune", action="store_true", help="let lqx_autotune pick the launch geometries before timing")
     ap.add_argument("--kernel-only", action="store_true",
                     help="timed device region only (no e2e, no cpu_baseline, no extras): the command ncu wraps")
@@ -802,6 +872,8 @@ def main():
         print(json.dumps({"kernels": _extras(torch, lqx, li, _peaks()[0])}))
     elif args.impl == "reference":
         run_reference(args)
+    elif args.tsplit:
+        run_tsplit(args)
     else:
         run_ours(args)
 

@@ -239,6 +239,22 @@ int lqx_smear_iterate_host(lqx_ctx* ctx, lqx_prec prec, const void* const host_u
                            double* plaq_avg_after_each);
 
 /* ---------------------------------------------------------------------------------------------
+ * NEXT-4 (sec.9 "parallelisation to multiple GPUs per host"): building blocks of a
+ * decomposition along t.  A rank's context is a t-slab with one halo slice on either side (local extent
+ * L3/ranks + 2); paper_1105_2279_b200/tsplit.py drives the halo exchange (torch.distributed or peer copies) and
+ * overlaps it with the interior launch.  Nothing here communicates.
+ *   lqx_smear_step_range : the smear step of the time slices [t0, t1) only (asynchronous).  The caller guarantees
+ *       that the input slices t0-1 .. t1 hold what the step should read.  Bit-identical to lqx_smear_step on those sites.
+ *   lqx_plaquette_range  : sum over the sites of [t0, t1) of the six plaquettes (synchronises, host double).
+ *   lqx_field_slice      : byte offset and size of time slice t inside a field's device storage.  A slice is one
+ *       contiguous range (sites are lexicographic with t slowest and blocks of 32 sites are contiguous) iff
+ *       L0*L1*L2 is a multiple of 32; otherwise LQX_EGEOM.
+ * ------------------------------------------------------------------------------------------- */
+int lqx_smear_step_range(lqx_field* const uout[4], const lqx_field* const uin[4], double alpha, int t0, int t1);
+int lqx_plaquette_range(const lqx_field* const u[4], int t0, int t1, double* plaq_sum);
+int lqx_field_slice(const lqx_field* f, int t, int64_t* offset_bytes, int64_t* nbytes);
+
+/* ---------------------------------------------------------------------------------------------
  * Harness support: device micro-benchmarks that give the roofline denominators.
  * ------------------------------------------------------------------------------------------- */
 /* kind: 0 = fp32 FMA, 1 = packed fp32x2 FMA, 2 = fp64 FMA (one dependent chain per accumulator, constant multiplicands);

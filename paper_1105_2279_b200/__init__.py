@@ -110,6 +110,9 @@ SIGNATURES = {
     "lqx_bench_copy_peak": (_i, [_vp, C.c_size_t, _pd]),
     "lqx_kernel_time": (_i, [_vp, _i, _pd, C.POINTER(C.c_int)]),
     "lqx_launch_count": (_i64, [_vp]),
+    "lqx_smear_step_range": (_i, [_pvp, _pvp, _d, _i, _i]),
+    "lqx_plaquette_range": (_i, [_pvp, _i, _i, _pd]),
+    "lqx_field_slice": (_i, [_vp, _i, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]),
     "lqx_smear_info": (_i, [_vp, C.POINTER(C.c_int), C.POINTER(C.c_int), C.c_char_p, _i]),
     "lqx_autotune": (_i, [_vp, _i, _i, _i, _vp, _i, C.POINTER(C.c_int)]),
     "lqx_tuned": (_i, [_vp, _i, _i, C.POINTER(C.c_int)]),
@@ -309,6 +312,20 @@ class Field:
         out = np.empty(self.host_shape, dtype=_NP[self.prec])
         _check(_lib.lqx_field_pop(self.handle, out.ctypes.data_as(C.c_void_p)), self.lat.ctx)
         return out
+
+    def slice_bytes(self, t):
+        """(offset, nbytes) of time slice t inside this field's device storage (lqx_field_slice)."""
+        off, n = C.c_int64(), C.c_int64()
+        _check(_lib.lqx_field_slice(self.handle, int(t), C.byref(off), C.byref(n)), self.lat.ctx)
+        return off.value, n.value
+
+    def slice_view(self, t):
+        """Time slice t of the device storage as a torch uint8 view (torch-owned fields only): what a halo
+        exchange sends and receives."""
+        if self._mem is None:
+            raise ValueError("slice_view needs a field whose memory torch owns (Lattice.alloc(torch_memory=True))")
+        off, n = self.slice_bytes(t)
+        return self._mem[off:off + n]
 
     def import_dev(self, dev_tensor):
         """AoS QDP-order torch CUDA tensor -> this field (device to device)."""
@@ -526,6 +543,18 @@ def smear_step(uout, uin, alpha, want_plaq_in: bool = False):
     p = C.c_double()
     _check(_lib.lqx_smear_step(_arr4(uout), _arr4(uin), float(alpha), C.byref(p) if want_plaq_in else None), _ctx_of(uin[0]))
     return p.value if want_plaq_in else None
+
+
+def smear_step_range(uout, uin, alpha, t0, t1):
+    """The smear step of the time slices [t0, t1) only (asynchronous); see lqx_smear_step_range."""
+    _check(_lib.lqx_smear_step_range(_arr4(uout), _arr4(uin), float(alpha), int(t0), int(t1)), _ctx_of(uin[0]))
+
+
+def plaquette_range(u, t0, t1):
+    """Plaquette SUM over the sites of the time slices [t0, t1)."""
+    s = C.c_double()
+    _check(_lib.lqx_plaquette_range(_arr4(u), int(t0), int(t1), C.byref(s)), _ctx_of(u[0]))
+    return s.value
 
 
 def smear_iterate(u, tmp, alpha, nsteps, want_plaq: bool = True):

@@ -238,6 +238,22 @@ int plaquette_launch(lqx_ctx* ctx, const lqx_field* const u[4], double* out) {
     return lqx_sum_partials(ctx, nblocks, 1, out);
 }
 
+// the plaquette sum over the sites of the time slices [t0, t1) only (NEXT-4: a rank's own slab)
+template <typename T>
+int plaquette_range_launch(lqx_ctx* ctx, const lqx_field* const u[4], int t0, int t1, double* out) {
+    const Geo& g = ctx->geo;
+    TileMap tm = Linear::map(g, kSlabZ);
+    const int grid = Linear::restrict_t(g, tm, t0, t1);
+    int rc = lqx_ensure_partials(ctx, (size_t)grid);
+    if (rc) return rc;
+    {
+        LqxTimed timed(ctx, LQX_K_PLAQUETTE);
+        k_plaquette<T, Linear><<<grid, Linear::THREADS, 0, ctx->stream>>>(g, tm, make_links<T>(u), ctx->d_partials);
+    }
+    LQX_LAUNCH_CHECK(ctx);
+    return lqx_sum_partials(ctx, grid, 1, out);
+}
+
 }  // namespace
 
 int lqx_pick_tile(const lqx_ctx* ctx, int first_choice) {
@@ -336,6 +352,32 @@ extern "C" int lqx_plaquette(const lqx_field* const u[4], double* plaq_sum, doub
     return LQX_OK;
 }
 
+extern "C" int lqx_plaquette_range(const lqx_field* const u[4], int t0, int t1, double* plaq_sum) {
+    lqx_ctx* ctx;
+    int rc = check_links(&ctx, u);
+    if (rc) return rc;
+    if (!plaq_sum) return LQX_EINVAL;
+    if (t0 < 0 || t1 > ctx->geo.L[3] || t0 >= t1) return lqx_fail(ctx, LQX_EINVAL, "plaquette_range: 0 <= t0 < t1 <= L3");
+    LQX_CUDA(ctx, cudaSetDevice(ctx->device));
+    rc = u[0]->prec == LQX_F32 ? plaquette_range_launch<float>(ctx, u, t0, t1, ctx->h_result)
+                               : plaquette_range_launch<double>(ctx, u, t0, t1, ctx->h_result);
+    if (rc) return rc;
+    return lqx_fetch_result(ctx, 1, plaq_sum);
+}
+
+extern "C" int lqx_field_slice(const lqx_field* f, int t, int64_t* offset_bytes, int64_t* nbytes) {
+    if (!f || !offset_bytes || !nbytes) return LQX_EINVAL;
+    lqx_ctx* ctx = f->ctx;
+    const Geo& g = ctx->geo;
+    const int64_t v3 = (int64_t)g.L[0] * g.L[1] * g.L[2];
+    if (t < 0 || t >= g.L[3]) return lqx_fail(ctx, LQX_EINVAL, "field_slice: t out of range");
+    if (v3 % 32 != 0) return lqx_fail(ctx, LQX_EGEOM, "field_slice: a time slice is contiguous only if L0*L1*L2 is a multiple of 32");
+    const int64_t per_site = 2 * (int64_t)(int)f->kind * (int64_t)(int)f->prec;
+    *offset_bytes = (int64_t)t * v3 * per_site;
+    *nbytes = v3 * per_site;
+    return LQX_OK;
+}
+
 static int check_smear_args(lqx_ctx** ctx_out, lqx_field* const uout[4], const lqx_field* const uin[4]) {
     lqx_ctx* ctx;
     int rc = check_links(&ctx, uin);
@@ -379,6 +421,20 @@ extern "C" int lqx_smear_step(lqx_field* const uout[4], const lqx_field* const u
     if (rc) return rc;
     if (plaq_in_or_null) return lqx_fetch_result(ctx, 1, plaq_in_or_null);
     return LQX_OK;
+}
+
+// NEXT-4 building block: the smear step of the time slices [t0, t1) only.  Asynchronous; the caller guarantees that the
+// input slices t0-1 .. t1 (periodic in the context's t extent) hold what the step should read -- on a t-slab with halo
+// slices that is "after the halo exchange".  Same per-site arithmetic as lqx_smear_step, bit for bit.
+extern "C" int lqx_smear_step_range(lqx_field* const uout[4], const lqx_field* const uin[4], double alpha, int t0, int t1) {
+    if (!uout || !uin) return LQX_EINVAL;
+    lqx_ctx* ctx;
+    int rc = check_smear_args(&ctx, uout, uin);
+    if (rc) return rc;
+    if (t0 < 0 || t1 > ctx->geo.L[3] || t0 >= t1) return lqx_fail(ctx, LQX_EINVAL, "smear_step_range: 0 <= t0 < t1 <= L3");
+    LQX_CUDA(ctx, cudaSetDevice(ctx->device));
+    rc = lqx_smear_launch_range_any(ctx, uout, uin, alpha, t0, t1);
+    return rc == 1 ? lqx_fail(ctx, LQX_EGEOM, "smear_step_range: no kernel map splits at these time slices") : rc;
 }
 
 extern "C" int lqx_smear_iterate(lqx_field* const u[4], lqx_field* const tmp[4], double alpha, int nsteps,

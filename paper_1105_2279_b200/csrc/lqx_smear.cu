@@ -542,13 +542,14 @@ int smear_launch_t(lqx_ctx* ctx, lqx_field* const uout[4], const lqx_field* cons
 
 // one smear step restricted to the time slices [t0, t1): the rolled kernel on a sub-grid (streamed host path)
 template <typename T>
-int smear_range_t(lqx_ctx* ctx, lqx_field* const uout[4], const lqx_field* const uin[4], double alpha, int t0, int t1) {
+int smear_range_t(lqx_ctx* ctx, lqx_field* const uout[4], const lqx_field* const uin[4], double alpha, int t0, int t1,
+                  bool force_linear) {
     const Geo& g = ctx->geo;
     LinksOut<T> o;
     for (int mu = 0; mu < 4; ++mu) o.u[mu] = (T*)uout[mu]->data;
     const Links<T> in = make_links<T>(uin);
     const T c0 = (T)(1.0 - alpha), c1 = (T)(alpha / 6.0);
-    const int choice = lqx_pick_tile(ctx, sizeof(T) == 4 ? 1 : 0);
+    const int choice = force_linear ? 0 : lqx_pick_tile(ctx, sizeof(T) == 4 ? 1 : 0);
     LQX_WITH_MAP(choice, {
         if (!MAP::splits_t(t0) || !MAP::splits_t(t1)) return 1;
         TileMap tm = MAP::map(g, kSlabZ);
@@ -565,8 +566,18 @@ int smear_range_t(lqx_ctx* ctx, lqx_field* const uout[4], const lqx_field* const
 
 int lqx_smear_launch_range(lqx_ctx* ctx, lqx_field* const uout[4], const lqx_field* const uin[4], double alpha, int t0,
                            int t1) {
-    return uin[0]->prec == LQX_F32 ? smear_range_t<float>(ctx, uout, uin, alpha, t0, t1)
-                                   : smear_range_t<double>(ctx, uout, uin, alpha, t0, t1);
+    int rc = uin[0]->prec == LQX_F32 ? smear_range_t<float>(ctx, uout, uin, alpha, t0, t1, false)
+                                     : smear_range_t<double>(ctx, uout, uin, alpha, t0, t1, false);
+    return rc;
+}
+// the same for ANY t0 < t1: where the 4-d tile in use does not split there, linear 128-site blocks do (every
+// kernel map evaluates the same per-site arithmetic, so the output does not depend on the choice)
+int lqx_smear_launch_range_any(lqx_ctx* ctx, lqx_field* const uout[4], const lqx_field* const uin[4], double alpha, int t0,
+                               int t1) {
+    int rc = lqx_smear_launch_range(ctx, uout, uin, alpha, t0, t1);
+    if (rc != 1) return rc;
+    return uin[0]->prec == LQX_F32 ? smear_range_t<float>(ctx, uout, uin, alpha, t0, t1, true)
+                                   : smear_range_t<double>(ctx, uout, uin, alpha, t0, t1, true);
 }
 
 int lqx_smear_launch(lqx_ctx* ctx, lqx_field* const uout[4], const lqx_field* const uin[4], double alpha, int only_mu,

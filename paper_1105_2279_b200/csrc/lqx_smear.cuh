@@ -59,6 +59,10 @@ int lqx_smear_launch(lqx_ctx* ctx, lqx_field* const uout[4], const lqx_field* co
 int lqx_smear_launch_range(lqx_ctx* ctx, lqx_field* const uout[4], const lqx_field* const uin[4], double alpha, int t0,
                            int t1);
 
+// ... for any t0 < t1 (falls back to linear blocks where the tile shape in use does not split at t0 / t1)
+int lqx_smear_launch_range_any(lqx_ctx* ctx, lqx_field* const uout[4], const lqx_field* const uin[4], double alpha, int t0,
+                               int t1);
+
 // shared-memory-staged smear step for fp32 (lqx_smear_staged.cu): LQX_OK, a negative status, or 1 if the
 // lattice is not a multiple of its 8x2x2x2 tile
 int lqx_smear_staged_launch(lqx_ctx* ctx, const Links<float>& in, const LinksOut<float>& out, float c0, float c1, double* plaq);

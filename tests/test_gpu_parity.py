@@ -1196,3 +1196,82 @@ def test_bench_line_contract():
     k = line["clocks"]
     assert k["sm_max_mhz"] > 0 and isinstance(k["reasons"], list)
     assert len(line["plaquette_avg_after_each_step"]) == 2 and all(abs(p) <= 1.0 for p in line["plaquette_avg_after_each_step"])
+
+
+# ------------------------------------------------------------------------------------------------
+# NEXT-4: decomposition along t (paper_1105_2279_b200/tsplit.py) on ONE GPU.  R ranks are emulated one after the other
+# in this process (the profiling guide: never run ranks that wait on one another on one GPU): each has its own context
+# on a local lattice of t-extent L3/R + 2, the halo exchange is a device copy between the ranks' fields.  The own slabs
+# concatenated must equal lqx_smear_step on the whole lattice BIT FOR BIT, and the global plaquette must agree.
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+@pytest.mark.parametrize("gdims,world", [((8, 4, 4, 8), 1), ((8, 4, 4, 8), 2), ((4, 4, 2, 12), 3), ((16, 4, 2, 8), 2)])
+def test_tsplit_slabs_equal_the_single_gpu_step_bit_for_bit(lqx, gdims, world, prec):
+    import torch
+
+    from paper_1105_2279_b200 import tsplit
+    from tsplit_helpers import EmulatedRanks, gather_own, scatter_no_halo
+
+    P = _prec(lqx, prec)
+    u = _links(6, gdims, prec, "near_unit")
+    nsteps = 2
+    with lqx.Lattice(gdims) as lat:  # the single-GPU answer
+        fu = [lat.from_host(t) for t in u]
+        tmp = [lat.alloc(lqx.COLORMAT, P) for _ in range(4)]
+        want_plaqs = []
+        for _ in range(nsteps):
+            lqx.smear_step(tmp, fu, 0.5)
+            fu, tmp = tmp, fu
+            want_plaqs.append(lqx.plaquette(fu)[0])
+        want = [f.pop() for f in fu]
+    emu = EmulatedRanks(world)
+    lats = [lqx.Lattice(tsplit.local_dims(gdims, world)) for _ in range(world)]
+    try:
+        comms = [tsplit.SelfComm() if world == 1 else emu.comm(r) for r in range(world)]
+        ts = [tsplit.TSplit(tsplit.LqxBackend(lqx, lats[r]), comms[r], gdims) for r in range(world)]
+        cur = [[lats[r].from_host(scatter_no_halo(f, gdims, r, world)) for f in u] for r in range(world)]  # NaN halos
+        nxt = [[lats[r].alloc(lqx.COLORMAT, P) for _ in range(4)] for r in range(world)]
+        for step in range(nsteps):
+            if world == 1:
+                ts[0].smear_step(nxt[0], cur[0], 0.5, overlap=(step == 0))
+            else:
+                for r in range(world):
+                    comms[r].exchange(*ts[r]._halo_views(cur[r]))
+                torch.cuda.synchronize()
+                emu.flush()
+                for r in range(world):
+                    ts[r].smear_step(nxt[r], cur[r], 0.5, halos_fresh=True)
+            cur, nxt = nxt, cur
+            if world == 1:
+                p = ts[0].plaquette_sum(cur[0])
+            else:
+                for r in range(world):
+                    comms[r].exchange(*ts[r]._halo_views(cur[r]))
+                torch.cuda.synchronize()
+                emu.flush()
+                p = sum(ts[r].plaquette_sum(cur[r], halos_fresh=True) for r in range(world))
+            assert abs(p - want_plaqs[step]) <= RTOL[prec] * 1e-2 * max(abs(want_plaqs[step]), np.sqrt(18.0 * np.prod(gdims)))
+        for mu in range(4):
+            got = gather_own([cur[r][mu].pop() for r in range(world)], gdims)
+            assert np.array_equal(got, want[mu]), mu
+    finally:
+        for l in lats:
+            l.close()
+
+
+def test_tsplit_geometry_errors(lqx):
+    from paper_1105_2279_b200 import tsplit
+
+    with pytest.raises(ValueError):
+        tsplit.local_dims((4, 4, 4, 6), 4)
+    with pytest.raises(ValueError):
+        tsplit.local_dims((4, 4, 4, 4), 4)
+    with lqx.Lattice((3, 3, 3, 4)) as lat:  # V3 = 27: a time slice is not a contiguous range
+        f = lat.alloc(lqx.COLORMAT, lqx.F32)
+        with pytest.raises(lqx.LqxError):
+            f.slice_bytes(1)
+        u = [lat.alloc(lqx.COLORMAT, lqx.F32) for _ in range(4)]
+        o = [lat.alloc(lqx.COLORMAT, lqx.F32) for _ in range(4)]
+        with pytest.raises(lqx.LqxError):
+            lqx.smear_step_range(o, u, 0.5, 2, 2)
+        lqx.smear_step_range(o, u, 0.5, 1, 3)  # ranges themselves need no contiguity
