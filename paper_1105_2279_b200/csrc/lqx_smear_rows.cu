@@ -12,9 +12,9 @@
 //  * tile = ROWS whole x-rows (L0 x 2 x 2 x 2 sites, one thread per site), the tile's own links copied to
 //    shared memory in the blocked field layout.  x-neighbours wrap around inside the row, so they are
 //    ALWAYS in the tile and come out of shared memory at any alignment for 4 wavefronts per 128-bit chunk;
-//    y/z/t-neighbours are in the tile for half of the rows.  Each operand is fetched by a predicated pair
-//    ld.shared / ld.global.nc into the same registers: the lanes inside the tile cost shared wavefronts,
-//    the others read whole aligned rows through L1 -- no lane pays twice and nothing diverges.
+//    y/z/t-neighbours are in the tile for half of the rows.  Each operand is fetched by generic loads from a
+//    SELECTED address (tile in shared memory or field in global memory): nothing diverges, and a warp mixes the
+//    two spaces only where it straddles two rows of different y/z/t position (see fetch_mat).
 //  * persistent CTAs, one per SM, double-buffered: while tile k is multiplied the own links of tile k+1
 //    arrive by cp.async, so the fill never idles the FMA pipe and one barrier per tile suffices.
 //
