@@ -566,6 +566,14 @@ int smear_range_t(lqx_ctx* ctx, lqx_field* const uout[4], const lqx_field* const
 
 int lqx_smear_launch_range(lqx_ctx* ctx, lqx_field* const uout[4], const lqx_field* const uin[4], double alpha, int t0,
                            int t1) {
+    // fp32 with the default kernel selection: the row-tile kernel where its 2-slice tiles split at t0 / t1
+    const int v32 = ctx->opt_smear_variant ? ctx->opt_smear_variant : (ctx->tuned_smear_variant[0] ? ctx->tuned_smear_variant[0] : 9);
+    if (uin[0]->prec == LQX_F32 && v32 == 9) {
+        LinksOut<float> o;
+        for (int mu = 0; mu < 4; ++mu) o.u[mu] = (float*)uout[mu]->data;
+        const int rc9 = lqx_smear_rowlit_launch_range(ctx, make_links<float>(uin), o, (float)(1.0 - alpha), (float)(alpha / 6.0), t0, t1);
+        if (rc9 != 1) return rc9;
+    }
     int rc = uin[0]->prec == LQX_F32 ? smear_range_t<float>(ctx, uout, uin, alpha, t0, t1, false)
                                      : smear_range_t<double>(ctx, uout, uin, alpha, t0, t1, false);
     return rc;

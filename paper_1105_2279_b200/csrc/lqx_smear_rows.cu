@@ -31,6 +31,7 @@ struct RowMap {
     int zs;          // z-tiles per slab: tiles are visited y, z fastest inside a slab, then t, then the next slab,
                      // so that the +-t neighbour rows of a tile are still in L2 (as Tiled<>::site does)
     int ntiles;
+    int toff;        // first t-tile of the launch (a launch may cover a range of time slices: streamed host path, t-split)
 };
 
 // One colour matrix from the tile in shared memory (in) or from the field in global memory, by GENERIC loads from a
@@ -321,7 +322,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_smear_rowlit(const __grid_consta
         const int bt = rem / (rm.ny * rm.zs);
         rem -= bt * (rm.ny * rm.zs);
         const int bz = rem / rm.ny + k * rm.zs, by = rem % rm.ny;
-        x[0] = lx, x[1] = RY * by + ly, x[2] = RZ * bz + lz, x[3] = RT * bt + lt;
+        x[0] = lx, x[1] = RY * by + ly, x[2] = RZ * bz + lz, x[3] = RT * (bt + rm.toff) + lt;
         s = x[0] + g.L[0] * (x[1] + g.L[1] * (x[2] + g.L[2] * x[3]));
     }
     fill_async(buf0, link_floats, u, s, li);
@@ -394,13 +395,17 @@ __global__ void __launch_bounds__(MAXT, MINB) k_smear_rowlit(const __grid_consta
     }
 }
 
+// t0 < 0: the whole lattice; otherwise the time slices [t0, t1) only (both multiples of RT, else 1; no plaquette)
 template <int RY, int RZ, int RT, int MAXT, int MINB>
-int rowlit_launch(lqx_ctx* ctx, const Links<float>& in, const LinksOut<float>& out, float c0, float c1, double* plaq) {
+int rowlit_launch(lqx_ctx* ctx, const Links<float>& in, const LinksOut<float>& out, float c0, float c1, double* plaq,
+                  int t0 = -1, int t1 = -1) {
     const Geo& g = ctx->geo;
     const int nthr = g.L[0] * RY * RZ * RT;
     if (nthr > MAXT || g.L[1] % RY || g.L[2] % RZ || g.L[3] % RT || (size_t)g.Vpad * 72 >= ((size_t)1 << 32)) return 1;
+    if (t0 >= 0 && (t0 % RT || t1 % RT || plaq)) return 1;
     RowMap rm;
-    rm.ny = g.L[1] / RY, rm.nz = g.L[2] / RZ, rm.nt = g.L[3] / RT;
+    rm.ny = g.L[1] / RY, rm.nz = g.L[2] / RZ, rm.nt = t0 >= 0 ? (t1 - t0) / RT : g.L[3] / RT;
+    rm.toff = t0 >= 0 ? t0 / RT : 0;
     rm.ntiles = rm.ny * rm.nz * rm.nt;
     int target = ctx->opt_block > 0 ? ctx->opt_block : kSlabZ;
     rm.zs = 1;
@@ -431,6 +436,7 @@ int rows_launch(lqx_ctx* ctx, const Links<float>& in, const LinksOut<float>& out
     if (nthr > MAXT || g.L[1] % RY || g.L[2] % RZ || g.L[3] % RT || (size_t)g.Vpad * 72 >= ((size_t)1 << 32)) return 1;
     RowMap rm;
     rm.ny = g.L[1] / RY, rm.nz = g.L[2] / RZ, rm.nt = g.L[3] / RT;
+    rm.toff = 0;
     rm.ntiles = rm.ny * rm.nz * rm.nt;
     // slab thickness in z: the largest divisor of nz that keeps a slab at most kSlabZ sites thick
     int target = ctx->opt_block > 0 ? ctx->opt_block : kSlabZ;
@@ -491,4 +497,10 @@ int lqx_smear_rowlit_launch(lqx_ctx* ctx, const Links<float>& in, const LinksOut
     if (rc != 1) return rc;
     if (t == 6) rc = rowlit_launch<2, 2, 2, 384, 1>(ctx, in, out, c0, c1, plaq);
     return rc;
+}
+
+// the default fp32 kernel on the time slices [t0, t1) only: LQX_OK, a negative status, or 1 if the row tiles do not
+// fit the lattice or do not split at t0 / t1 (the caller then launches the rolled kernel, which is bit-identical)
+int lqx_smear_rowlit_launch_range(lqx_ctx* ctx, const Links<float>& in, const LinksOut<float>& out, float c0, float c1, int t0, int t1) {
+    return rowlit_launch<2, 2, 2, 384, 2>(ctx, in, out, c0, c1, nullptr, t0, t1);
 }
