@@ -401,7 +401,8 @@ int rowlit_launch(lqx_ctx* ctx, const Links<float>& in, const LinksOut<float>& o
                   int t0 = -1, int t1 = -1) {
     const Geo& g = ctx->geo;
     const int nthr = g.L[0] * RY * RZ * RT;
-    if (nthr > MAXT || g.L[1] % RY || g.L[2] % RZ || g.L[3] % RT || (size_t)g.Vpad * 72 >= ((size_t)1 << 32)) return 1;
+    // whole warps only: the CTA-wide reductions shuffle with a full mask
+    if (nthr > MAXT || nthr % 32 || g.L[1] % RY || g.L[2] % RZ || g.L[3] % RT || (size_t)g.Vpad * 72 >= ((size_t)1 << 32)) return 1;
     if (t0 >= 0 && (t0 % RT || t1 % RT || plaq)) return 1;
     RowMap rm;
     rm.ny = g.L[1] / RY, rm.nz = g.L[2] / RZ, rm.nt = t0 >= 0 ? (t1 - t0) / RT : g.L[3] / RT;
@@ -433,7 +434,8 @@ template <int RY, int RZ, int RT, int MAXT>
 int rows_launch(lqx_ctx* ctx, const Links<float>& in, const LinksOut<float>& out, float c0, float c1, double* plaq) {
     const Geo& g = ctx->geo;
     const int nthr = g.L[0] * RY * RZ * RT;
-    if (nthr > MAXT || g.L[1] % RY || g.L[2] % RZ || g.L[3] % RT || (size_t)g.Vpad * 72 >= ((size_t)1 << 32)) return 1;
+    // whole warps only: the CTA-wide reductions shuffle with a full mask
+    if (nthr > MAXT || nthr % 32 || g.L[1] % RY || g.L[2] % RZ || g.L[3] % RT || (size_t)g.Vpad * 72 >= ((size_t)1 << 32)) return 1;
     RowMap rm;
     rm.ny = g.L[1] / RY, rm.nz = g.L[2] / RZ, rm.nt = g.L[3] / RT;
     rm.toff = 0;

@@ -345,8 +345,10 @@ def test_staple_smear_plaquette(lqx, dims, prec):
 # staged in shared memory, 7 the tile's own links in shared memory and the halo through L1, 8 plane-ordered 42-product evaluation on
 # whole-x-row tiles in shared memory with persistent double-buffered CTAs) and every
 # CTA tile shape that divides the lattice, against the truth oracle; 16x8x4x4 spans several tiles in every
-# direction for all shapes, 8x4x4x2 is exactly one 8x4x4x2 tile (every neighbour wraps into the same tile)
-@pytest.mark.parametrize("dims", [(16, 8, 4, 4), (8, 4, 4, 2), (4, 4, 4, 4)])
+# direction for all shapes, 8x4x4x2 is exactly one 8x4x4x2 tile (every neighbour wraps into the same tile); 12x6x4x2 has
+# row tiles of 96 threads and y-tiles of 2 and 3 rows, 6x4x2x4 has rows that are not whole warps (the row-tile kernels
+# hand over to the rolled kernel there)
+@pytest.mark.parametrize("dims", [(16, 8, 4, 4), (8, 4, 4, 2), (4, 4, 4, 4), (12, 6, 4, 2), (6, 4, 2, 4)])
 @pytest.mark.parametrize("prec", ["f32", "f64"])
 @pytest.mark.parametrize("variant", [1, 2, 3, 4, 6, 7, 8, 9])
 def test_smear_variants_and_tiles(lqx, dims, prec, variant):
