@@ -362,7 +362,7 @@ def test_smear_variants_and_tiles(lqx, dims, prec, variant):
         scale = np.sqrt(18.0 * lat.volume)
         lat.set_option("smear_variant", variant)
         first = None
-        for tile in (-1, 0, 1, 2, 3, 4, 5, 6):
+        for tile in (-1, 0, 1, 2, 3, 4, 5, 6, 7):
             lat.set_option("tile", tile)
             for o in out:
                 lqx.scale(o, 0.0, o)
