@@ -553,6 +553,8 @@ int lqx_smear_rowlit_launch(lqx_ctx* ctx, const Links<float>& in, const LinksOut
     if (rc != 1) return rc;
     if (t == 2 || t <= 0) rc = rowlit_launch<2, 2, 1, 192, 4>(ctx, in, out, c0, c1, plaq);
     if (rc != 1) return rc;
+    if (t <= 0) rc = rowlit_launch<2, 2, 1, 384, 2>(ctx, in, out, c0, c1, plaq);  // rows of 49 .. 96 sites: four-row tiles
+    if (rc != 1) return rc;
     if (t == 3) rc = rowlit_launch<2, 2, 1, 192, 3>(ctx, in, out, c0, c1, plaq);
     if (rc != 1) return rc;
     if (t == 4) rc = rowlit_launch<2, 3, 1, 288, 2>(ctx, in, out, c0, c1, plaq);
