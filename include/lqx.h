@@ -304,7 +304,7 @@ int lqx_tuned(const lqx_ctx* ctx, int kernel_class, lqx_prec prec, int out[4]);
  * threads per site, 6 = operands staged in shared memory with cp.async (fp32), 7 = the CTA tile's own links in
  * shared memory and the halo through L1, 8 = plane-ordered 42-product evaluation on whole-x-row tiles, persistent
  * double-buffered CTAs (fp32), 9 = the literal evaluation of 3 on whole-x-row tiles whose own links sit in shared
- * memory (fp32; same summation order as 3, bit-identical); variants fall back to 3 where their tiles do not fit
+ * memory (both precisions; same summation order as 3, bit-identical); variants fall back to 3 where their tiles do not fit
  * the lattice.
  * "tile" -1 = automatic, 0 = linear 128-site blocks, 1..6 = CTA tile shape (8x4x4x2, 8x4x2x2,
  * 4x4x4x2, 16x4x2x2, 16x2x2x2, 32x2x2x2) of the nearest-neighbour kernels, used if it divides the

@@ -460,8 +460,7 @@ int smear_launch_t(lqx_ctx* ctx, lqx_field* const uout[4], const lqx_field* cons
         void operator()() const { c->last_smear_variant = 3, c->last_smear_kernel = "k_smear_rolled", c->last_smear_lane_ops = 48 * 108 + 144; }
     } fell_back = {ctx};
     if (variant == 9) {
-        int rc = 1;
-        if (sizeof(T) == 4) rc = lqx_smear_rowlit_launch(ctx, reinterpret_cast<const Links<float>&>(in), reinterpret_cast<const LinksOut<float>&>(o), (float)c0, (float)c1, plaq);
+        const int rc = lqx_smear_rowlit_launch(ctx, in, o, c0, c1, plaq);
         if (rc <= 0) return rc;
         variant = 3;
         fell_back();

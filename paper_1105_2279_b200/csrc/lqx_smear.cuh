@@ -79,4 +79,5 @@ int lqx_smear_tile_launch(lqx_ctx* ctx, const Links<double>& in, const LinksOut<
 int lqx_smear_rows_launch(lqx_ctx* ctx, const Links<float>& in, const LinksOut<float>& out, float c0, float c1, double* plaq);
 // the literal evaluation on the same row tiles, two CTAs per SM (option "smear_variant" = 9)
 int lqx_smear_rowlit_launch(lqx_ctx* ctx, const Links<float>& in, const LinksOut<float>& out, float c0, float c1, double* plaq);
+int lqx_smear_rowlit_launch(lqx_ctx* ctx, const Links<double>& in, const LinksOut<double>& out, double c0, double c1, double* plaq);
 int lqx_smear_rowlit_launch_range(lqx_ctx* ctx, const Links<float>& in, const LinksOut<float>& out, float c0, float c1, int t0, int t1);

@@ -97,6 +97,58 @@ __device__ __forceinline__ void fill_async(float* buf, int link_floats, const Li
     }
 }
 
+// fp64 forms of the three helpers (variant 9 in double precision): a matrix is nine 128-bit chunks of two doubles,
+// 4608 bytes per 32-site block, no trailing half chunk
+__device__ __forceinline__ Mat3<double> fetch_mat(unsigned long long s_link, const double* g_link, bool in, int li, int gi) {
+    const int idx = in ? li : gi;
+    const unsigned long long off = (unsigned long long)(idx >> 5) * (32u * 18u * 8u) + (unsigned)(idx & 31) * 16u;
+    const unsigned long long a = (in ? s_link : (unsigned long long)g_link) + off;
+    double r[18];
+#pragma unroll
+    for (int q = 0; q < 9; ++q) asm volatile("ld.v2.f64 {%0,%1}, [%2];" : "=d"(r[2 * q]), "=d"(r[2 * q + 1]) : "l"(a + q * 512u));
+    Mat3<double> m;
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            m.re[i][j] = r[2 * (3 * i + j)];
+            m.im[i][j] = r[2 * (3 * i + j) + 1];
+        }
+    return m;
+}
+__device__ __forceinline__ Mat3<double> fetch_own_d(unsigned long long s_link_generic, int li) {
+    const unsigned sa = (unsigned)__cvta_generic_to_shared(reinterpret_cast<const void*>(s_link_generic)) + (unsigned)(li >> 5) * (32u * 18u * 8u) + (unsigned)(li & 31) * 16u;
+    double r[18];
+#pragma unroll
+    for (int q = 0; q < 9; ++q) asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(r[2 * q]), "=d"(r[2 * q + 1]) : "r"(sa + q * 512u));
+    Mat3<double> m;
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            m.re[i][j] = r[2 * (3 * i + j)];
+            m.im[i][j] = r[2 * (3 * i + j) + 1];
+        }
+    return m;
+}
+__device__ __forceinline__ void fill_async(double* buf, int link_reals, const Links<double>& u, int s, int li) {
+    const size_t goff = (size_t)(s >> 5) * (32 * 18) + (size_t)(s & 31) * 2;
+    const int soff = (li >> 5) * (32 * 18) + (li & 31) * 2;
+#pragma unroll
+    for (int mu = 0; mu < 4; ++mu) {
+        const double* g = u.u[mu] + goff;
+        double* d = buf + mu * link_reals + soff;
+#pragma unroll
+        for (int q = 0; q < 9; ++q) __pipeline_memcpy_async(d + q * 64, g + q * 64, 16);
+    }
+}
+template <typename T>
+__device__ __forceinline__ Mat3<T> fetch_own_t(unsigned long long s_link_generic, int li);
+template <>
+__device__ __forceinline__ Mat3<float> fetch_own_t<float>(unsigned long long a, int li) { return fetch_own(a, li); }
+template <>
+__device__ __forceinline__ Mat3<double> fetch_own_t<double>(unsigned long long a, int li) { return fetch_own_d(a, li); }
+
 // scheduling fence: every element of m must exist before any later (volatile) load is issued.  Without it the
 // compiler hoists the independent operand loads of all six planes to the top and spills kilobytes per thread.
 __device__ __forceinline__ void fence_mat(const Mat3<float>& m) {
@@ -334,16 +386,28 @@ constexpr int kTmemCols = 256;  // per CTA: three warps per lane quarter x 72 wo
 // loop (a third fewer integer instructions, no spills -- but 4 000 instructions of straight-line code per site instead of
 // 900 in loops, and with 24 warps at different places the instruction cache misses: 3.88 ms against 2.84 ms).
 // --------------------------------------------------------------------------------------------------------------
-template <bool PLAQ, int RY, int RZ, int RT, int MAXT, int MINB, bool TM>
+// type shims so that the kernel template compiles for double, where tensor memory is not used (TM = false)
+template <typename T>
+__device__ __forceinline__ Mat3<T> tmem_own(unsigned taddr);
+template <>
+__device__ __forceinline__ Mat3<float> tmem_own<float>(unsigned taddr) { return tmem_load_mat(taddr); }
+template <>
+__device__ __forceinline__ Mat3<double> tmem_own<double>(unsigned) { return zero_mat<double>(); }
+__device__ __forceinline__ void tmem_put(unsigned taddr, const Mat3<float>& m) { tmem_store_mat(taddr, m); }
+__device__ __forceinline__ void tmem_put(unsigned, const Mat3<double>&) {}
+__device__ __forceinline__ void tmem_wait_t(Mat3<float>& m) { tmem_wait(m); }
+__device__ __forceinline__ void tmem_wait_t(Mat3<double>&) {}
+
+template <typename T, bool PLAQ, int RY, int RZ, int RT, int MAXT, int MINB, bool TM>
 __global__ void __launch_bounds__(MAXT, MINB) k_smear_rowlit(const __grid_constant__ Geo g, const __grid_constant__ RowMap rm,
-                                                          const __grid_constant__ Links<float> u, const __grid_constant__ LinksOut<float> out,
-                                                          float c0, float c1, double* __restrict__ partials) {
+                                                          const __grid_constant__ Links<T> u, const __grid_constant__ LinksOut<T> out,
+                                                          T c0, T c1, double* __restrict__ partials) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int L0 = g.L[0];
     const int nthr = blockDim.x;
     const int npad = (nthr + 31) & ~31;
     const int link_floats = 18 * npad;
-    float* const buf0 = reinterpret_cast<float*>(smem_raw);
+    T* const buf0 = reinterpret_cast<T*>(smem_raw);
     const int li = threadIdx.x;
     const int lx = li % L0, row = li / L0;
     const int ly = row % RY, lz = (row / RY) % RZ, lt = row / (RY * RZ);
@@ -395,52 +459,52 @@ __global__ void __launch_bounds__(MAXT, MINB) k_smear_rowlit(const __grid_consta
         const int w = li >> 5;
         tm_own = tm_base_s + ((unsigned)((w & 3) * 32) << 16) + (unsigned)((w >> 2) * 72);
 #pragma unroll 1
-        for (int mu = 0; mu < 4; ++mu) tmem_store_mat(tm_own + 18 * mu, fetch_own((unsigned long long)(buf0 + mu * link_floats), li));
+        for (int mu = 0; mu < 4; ++mu) tmem_put(tm_own + 18 * mu, fetch_own_t<T>((unsigned long long)(buf0 + mu * link_floats), li));
         asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
     }
 
-    float pl = 0.f;
+    T pl = T(0);
 #pragma unroll 1
     for (int mu = 0; mu < 4; ++mu) {
-        const float* umu_g = u.u[mu];
+        const T* umu_g = u.u[mu];
         const unsigned long long umu_t = (unsigned long long)(buf0 + mu * link_floats);
         const int xpmu = gnb(mu, true);
         const bool in_pmu = (mask >> mu) & 1u;
         const int d_pmu = dloc(mu, true);
-        Mat3<float> acc = zero_mat<float>();
+        Mat3<T> acc = zero_mat<T>();
 #pragma unroll 1
         for (int nu = 3; nu >= 0; --nu) {  // upper: U_nu(x) U_mu(x+nu^) adj(U_nu(x+mu^))
             if (nu == mu) continue;
-            const float* unu_g = u.u[nu];
+            const T* unu_g = u.u[nu];
             const unsigned long long unu_t = (unsigned long long)(buf0 + nu * link_floats);
             const bool in_pnu = (mask >> nu) & 1u;
-            Mat3<float> own = TM ? tmem_load_mat(tm_own + 18 * nu) : fetch_own(unu_t, li);  // requested first, awaited last
-            const Mat3<float> second = fetch_mat(umu_t, umu_g, in_pnu, li + dloc(nu, true), gnb(nu, true));
-            if (TM) tmem_wait(own);
-            const Mat3<float> t = mul_nn(own, second);
+            Mat3<T> own = TM ? tmem_own<T>(tm_own + 18 * nu) : fetch_own_t<T>(unu_t, li);  // requested first, awaited last
+            const Mat3<T> second = fetch_mat(umu_t, umu_g, in_pnu, li + dloc(nu, true), gnb(nu, true));
+            if (TM) tmem_wait_t(own);
+            const Mat3<T> t = mul_nn(own, second);
             mac_na(acc, t, fetch_mat(unu_t, unu_g, in_pmu, li + d_pmu, xpmu));
         }
 #pragma unroll 1
         for (int nu = 0; nu < 4; ++nu) {  // lower: adj(U_nu(x-nu^)) U_mu(x-nu^) U_nu(x-nu^+mu^)
             if (nu == mu) continue;
-            const float* unu_g = u.u[nu];
+            const T* unu_g = u.u[nu];
             const unsigned long long unu_t = (unsigned long long)(buf0 + nu * link_floats);
             const bool in_mnu = (mask >> (4 + nu)) & 1u;
             const int xmnu = gnb(nu, false);
             const int l1 = li + dloc(nu, false);
-            const Mat3<float> t = mul_an(fetch_mat(unu_t, unu_g, in_mnu, l1, xmnu), fetch_mat(umu_t, umu_g, in_mnu, l1, xmnu));
+            const Mat3<T> t = mul_an(fetch_mat(unu_t, unu_g, in_mnu, l1, xmnu), fetch_mat(umu_t, umu_g, in_mnu, l1, xmnu));
             mac_nn(acc, t, fetch_mat(unu_t, unu_g, in_mnu && in_pmu, l1 + d_pmu, xmnu + (xpmu - s)));
         }
-        Mat3<float> umu = TM ? tmem_load_mat(tm_own + 18 * mu) : fetch_own(umu_t, li);
-        if (TM) tmem_wait(umu);
+        Mat3<T> umu = TM ? tmem_own<T>(tm_own + 18 * mu) : fetch_own_t<T>(umu_t, li);
+        if (TM) tmem_wait_t(umu);
         if (PLAQ) pl += re_tr_na(umu, acc);
-        Mat3<float> r;
+        Mat3<T> r;
 #pragma unroll
         for (int i = 0; i < 3; ++i)
 #pragma unroll
             for (int j = 0; j < 3; ++j) {
-                r.re[i][j] = fmaf(c1, acc.re[i][j], c0 * umu.re[i][j]);
-                r.im[i][j] = fmaf(c1, acc.im[i][j], c0 * umu.im[i][j]);
+                r.re[i][j] = fma(c1, acc.re[i][j], c0 * umu.re[i][j]);
+                r.im[i][j] = fma(c1, acc.im[i][j], c0 * umu.im[i][j]);
             }
         store_mat(out.u[mu], s, r);
     }
@@ -456,13 +520,13 @@ __global__ void __launch_bounds__(MAXT, MINB) k_smear_rowlit(const __grid_consta
 }
 
 // t0 < 0: the whole lattice; otherwise the time slices [t0, t1) only (both multiples of RT, else 1; no plaquette)
-template <int RY, int RZ, int RT, int MAXT, int MINB, bool TM = false>
-int rowlit_launch(lqx_ctx* ctx, const Links<float>& in, const LinksOut<float>& out, float c0, float c1, double* plaq,
+template <typename T, int RY, int RZ, int RT, int MAXT, int MINB, bool TM = false>
+int rowlit_launch(lqx_ctx* ctx, const Links<T>& in, const LinksOut<T>& out, T c0, T c1, double* plaq,
                   int t0 = -1, int t1 = -1) {
     const Geo& g = ctx->geo;
     const int nthr = g.L[0] * RY * RZ * RT;
     // whole warps only: the CTA-wide reductions shuffle with a full mask
-    if (nthr > MAXT || nthr % 32 || g.L[1] % RY || g.L[2] % RZ || g.L[3] % RT || (size_t)g.Vpad * 72 >= ((size_t)1 << 32)) return 1;
+    if (nthr > MAXT || nthr % 32 || g.L[1] % RY || g.L[2] % RZ || g.L[3] % RT || (size_t)g.Vpad * 18 * sizeof(T) >= ((size_t)1 << 32)) return 1;
     if (t0 >= 0 && (t0 % RT || t1 % RT || plaq)) return 1;
     RowMap rm;
     rm.ny = g.L[1] / RY, rm.nz = g.L[2] / RZ, rm.nt = t0 >= 0 ? (t1 - t0) / RT : g.L[3] / RT;
@@ -473,18 +537,18 @@ int rowlit_launch(lqx_ctx* ctx, const Links<float>& in, const LinksOut<float>& o
     for (int z = 1; z <= rm.nz; ++z)
         if (rm.nz % z == 0 && z * RZ <= target) rm.zs = z;
     const int npad = (nthr + 31) & ~31;
-    const size_t smem = (size_t)4 * 18 * npad * sizeof(float);
+    const size_t smem = (size_t)4 * 18 * npad * sizeof(T);
     const int grid = rm.ntiles;
-    if (plaq) LQX_CUDA(ctx, cudaFuncSetAttribute(k_smear_rowlit<true, RY, RZ, RT, MAXT, MINB, TM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    else LQX_CUDA(ctx, cudaFuncSetAttribute(k_smear_rowlit<false, RY, RZ, RT, MAXT, MINB, TM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    if (plaq) LQX_CUDA(ctx, cudaFuncSetAttribute(k_smear_rowlit<T, true, RY, RZ, RT, MAXT, MINB, TM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    else LQX_CUDA(ctx, cudaFuncSetAttribute(k_smear_rowlit<T, false, RY, RZ, RT, MAXT, MINB, TM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     if (plaq) {
         int rc = lqx_ensure_partials(ctx, (size_t)grid);
         if (rc) return rc;
     }
     {
         LqxTimed timed(ctx, LQX_K_SMEAR);
-        if (plaq) k_smear_rowlit<true, RY, RZ, RT, MAXT, MINB, TM><<<grid, nthr, smem, ctx->stream>>>(g, rm, in, out, c0, c1, ctx->d_partials);
-        else k_smear_rowlit<false, RY, RZ, RT, MAXT, MINB, TM><<<grid, nthr, smem, ctx->stream>>>(g, rm, in, out, c0, c1, nullptr);
+        if (plaq) k_smear_rowlit<T, true, RY, RZ, RT, MAXT, MINB, TM><<<grid, nthr, smem, ctx->stream>>>(g, rm, in, out, c0, c1, ctx->d_partials);
+        else k_smear_rowlit<T, false, RY, RZ, RT, MAXT, MINB, TM><<<grid, nthr, smem, ctx->stream>>>(g, rm, in, out, c0, c1, nullptr);
     }
     LQX_LAUNCH_CHECK(ctx);
     return plaq ? lqx_sum_partials(ctx, grid, 1, plaq) : LQX_OK;
@@ -549,26 +613,39 @@ int lqx_smear_rows_launch(lqx_ctx* ctx, const Links<float>& in, const LinksOut<f
 int lqx_smear_rowlit_launch(lqx_ctx* ctx, const Links<float>& in, const LinksOut<float>& out, float c0, float c1, double* plaq) {
     const int t = ctx->opt_tile;
     int rc = 1;
-    if (t == 1 || t <= 0) rc = rowlit_launch<2, 2, 2, 384, 2>(ctx, in, out, c0, c1, plaq);
+    if (t == 1 || t <= 0) rc = rowlit_launch<float, 2, 2, 2, 384, 2>(ctx, in, out, c0, c1, plaq);
     if (rc != 1) return rc;
-    if (t == 2 || t <= 0) rc = rowlit_launch<2, 2, 1, 192, 4>(ctx, in, out, c0, c1, plaq);
+    if (t == 2 || t <= 0) rc = rowlit_launch<float, 2, 2, 1, 192, 4>(ctx, in, out, c0, c1, plaq);
     if (rc != 1) return rc;
-    if (t <= 0) rc = rowlit_launch<2, 2, 1, 384, 2>(ctx, in, out, c0, c1, plaq);  // rows of 49 .. 96 sites: four-row tiles
+    if (t <= 0) rc = rowlit_launch<float, 2, 2, 1, 384, 2>(ctx, in, out, c0, c1, plaq);  // rows of 49 .. 96 sites: four-row tiles
     if (rc != 1) return rc;
-    if (t == 3) rc = rowlit_launch<2, 2, 1, 192, 3>(ctx, in, out, c0, c1, plaq);
+    if (t == 3) rc = rowlit_launch<float, 2, 2, 1, 192, 3>(ctx, in, out, c0, c1, plaq);
     if (rc != 1) return rc;
-    if (t == 4) rc = rowlit_launch<2, 3, 1, 288, 2>(ctx, in, out, c0, c1, plaq);
+    if (t == 4) rc = rowlit_launch<float, 2, 3, 1, 288, 2>(ctx, in, out, c0, c1, plaq);
     if (rc != 1) return rc;
-    if (t == 5) rc = rowlit_launch<3, 2, 1, 288, 2>(ctx, in, out, c0, c1, plaq);
+    if (t == 5) rc = rowlit_launch<float, 3, 2, 1, 288, 2>(ctx, in, out, c0, c1, plaq);
     if (rc != 1) return rc;
-    if (t == 6) rc = rowlit_launch<2, 2, 2, 384, 1>(ctx, in, out, c0, c1, plaq);
+    if (t == 6) rc = rowlit_launch<float, 2, 2, 2, 384, 1>(ctx, in, out, c0, c1, plaq);
     if (rc != 1) return rc;
-    if (t == 7) rc = rowlit_launch<2, 2, 2, 384, 2, true>(ctx, in, out, c0, c1, plaq);  // own links re-read from tensor memory
+    if (t == 7) rc = rowlit_launch<float, 2, 2, 2, 384, 2, true>(ctx, in, out, c0, c1, plaq);  // own links re-read from tensor memory
     return rc;
 }
 
 // the default fp32 kernel on the time slices [t0, t1) only: LQX_OK, a negative status, or 1 if the row tiles do not
 // fit the lattice or do not split at t0 / t1 (the caller then launches the rolled kernel, which is bit-identical)
 int lqx_smear_rowlit_launch_range(lqx_ctx* ctx, const Links<float>& in, const LinksOut<float>& out, float c0, float c1, int t0, int t1) {
-    return rowlit_launch<2, 2, 2, 384, 2>(ctx, in, out, c0, c1, nullptr, t0, t1);
+    return rowlit_launch<float, 2, 2, 2, 384, 2>(ctx, in, out, c0, c1, nullptr, t0, t1);
+}
+
+// variant 9 in double precision: four-row tiles (L0 x 2 x 2 x 1 sites; 72 KB of shared memory at L0 = 32), as many CTAs per
+// SM as the 168 registers of the fp64 literal evaluation allow.  Option "tile": 1 = 2x2x1 rows, 2 = 2x1x2, 3 = 2x2x2
+int lqx_smear_rowlit_launch(lqx_ctx* ctx, const Links<double>& in, const LinksOut<double>& out, double c0, double c1, double* plaq) {
+    const int t = ctx->opt_tile;
+    int rc = 1;
+    if (t == 1 || t <= 0) rc = rowlit_launch<double, 2, 2, 1, 128, 3>(ctx, in, out, c0, c1, plaq);
+    if (rc != 1) return rc;
+    if (t == 2) rc = rowlit_launch<double, 2, 1, 2, 128, 3>(ctx, in, out, c0, c1, plaq);
+    if (rc != 1) return rc;
+    if (t == 3) rc = rowlit_launch<double, 2, 2, 2, 256, 1>(ctx, in, out, c0, c1, plaq);
+    return rc;
 }

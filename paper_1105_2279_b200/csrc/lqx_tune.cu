@@ -119,9 +119,9 @@ extern "C" int lqx_autotune(lqx_ctx* ctx, int kernel_class, lqx_prec prec, int r
         // (variant, tile): the literal kernel on row tiles (fp32) and on 4-d tiles / linear blocks.  The other variants
         // are measured slower on every lattice tried and are options, not candidates.
         static const int cand32[][2] = {{9, 1}, {9, 2}, {3, 1}, {3, 2}, {3, 4}, {3, 5}, {3, 0}};
-        static const int cand64[][2] = {{3, 0}, {3, 2}, {3, 3}, {3, 5}};
+        static const int cand64[][2] = {{3, 0}, {3, 2}, {3, 3}, {3, 5}, {9, 1}};
         const int(*cand)[2] = pi == 0 ? cand32 : cand64;
-        const int ncand = pi == 0 ? 7 : 4;
+        const int ncand = pi == 0 ? 7 : 5;
         for (int k = 0; k < ncand; ++k) {
             ctx->opt_smear_variant = cand[k][0], ctx->opt_tile = cand[k][1];
             const double ms = timer.median_ms([&] { return lqx_smear_step(o, u, 0.5, nullptr); }, reps);
