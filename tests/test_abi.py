@@ -81,3 +81,20 @@ def test_product_path_does_not_reference_the_oracle():
             text = open(os.path.join(ROOT, "oracle", fn)).read()
             assert "paper_1105_2279_b200" not in text.replace("paper_1105_2279_b200/csrc", ""), fn
             assert "lqx_internal" not in text, fn
+
+
+def test_bench_looks_up_ncu_captures_by_kernel_and_precision():
+    """bench.py attaches the DRAM traffic of a committed ncu capture to its roofline block only if that capture is of
+    the kernel (and precision) that ran: the lookup must find the round-2 captures by name and refuse unknown kernels."""
+    import bench
+
+    cap, src = bench._ncu_capture("k_smear_rowlit", "f32")
+    assert cap is not None and src.startswith("profiles/r02") and "rowlit" in src
+    traffic = cap["dram__bytes_read.sum"] + cap["dram__bytes_write.sum"]
+    assert 6.1e9 < traffic < 9e9  # configs[3]: 6.115 GB algorithmic per launch
+    assert 0 < cap["l1tex__data_pipe_lsu_wavefronts.avg.pct_of_peak_sustained_elapsed"] < 100
+    c32, s32 = bench._ncu_capture("k_smear_rolled", "f32")
+    c64, s64 = bench._ncu_capture("k_smear_rolled", "f64")
+    assert c32 is not None and c64 is not None and s32 != s64
+    none, why = bench._ncu_capture("k_no_such_kernel", "f32")
+    assert none is None and "k_no_such_kernel" in why
