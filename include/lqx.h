@@ -303,7 +303,8 @@ int lqx_tuned(const lqx_ctx* ctx, int kernel_class, lqx_prec prec, int out[4]);
  * 2 = shared-corner kernel (36 products, lower staples exchanged through shared memory), 4 = four
  * threads per site, 6 = operands staged in shared memory with cp.async (fp32), 7 = the CTA tile's own links in
  * shared memory and the halo through L1, 8 = plane-ordered 42-product evaluation on whole-x-row tiles, persistent
- * double-buffered CTAs (fp32), 9 = the literal evaluation of 3 on whole-x-row tiles whose own links sit in shared
+ * double-buffered CTAs (fp32; with "tile" 6: one tile per CTA, two CTAs per SM, 7: the same with the halo operands
+ * prefetched into L1), 9 = the literal evaluation of 3 on whole-x-row tiles whose own links sit in shared
  * memory (both precisions; same summation order as 3, bit-identical); variants fall back to 3 where their tiles do not fit
  * the lattice.
  * "tile" -1 = automatic, 0 = linear 128-site blocks, 1..6 = CTA tile shape (8x4x4x2, 8x4x2x2,

@@ -17,6 +17,10 @@
 //    two spaces only where it straddles two rows of different y/z/t position (see fetch_mat).
 //  * persistent CTAs, one per SM, double-buffered: while tile k is multiplied the own links of tile k+1
 //    arrive by cp.async, so the fill never idles the FMA pipe and one barrier per tile suffices.
+//  * option "tile" = 6 / 7: one 2x2x1-row tile per CTA and one buffer, two CTAs per SM, so that the SM keeps an L1;
+//    7 requests every halo operand with prefetch.global.L1 three products ahead of its load (pf_mat).  Measured at
+//    48^3x96: persistent form 4.8 ms, 6: 3.76 ms, 7: 2.84 ms -- level with the literal row-tile kernel (variant 9,
+//    2.83 ms) at half its warps (profiles/r02j).
 //
 // Sums the staples of a link in plane order (not the oracle's nu-ascending order): agrees with the other
 // variants to rounding, not bit for bit.
@@ -194,6 +198,19 @@ struct SiteCtx {
 //   E' = U_mu(x-mu), F' = U_nu(x-mu), G' = U_mu(x-mu+nu) S_nu += (adj(E') F') G' lower staple of link nu
 // The loads of every product are issued BEFORE the FMAs of the product in front of it (one product of
 // prefetch); fence_mat pins that order.  B and C of the next plane are fetched during this plane's last product.
+// L1 prefetch of a halo matrix (nothing for a matrix of the tile): five lines per warp and chunk, no destination
+// register, so ptxas cannot sink it to a use -- the only way found to put a request AHEAD of the products at the
+// register limit.  Needs an L1 to land in: used by the two-CTAs-per-SM form (one tile buffer each), not by the
+// persistent double-buffered form whose shared memory takes the whole SM.
+__device__ __forceinline__ void pf_mat(const float* g_link, bool in, int gi) {
+    if (!in) {
+        const char* a = reinterpret_cast<const char*>(g_link) + (size_t)(gi >> 5) * (32 * 18 * 4) + (size_t)(gi & 31) * 16;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) asm volatile("prefetch.global.L1 [%0];" ::"l"(a + q * 512));
+        asm volatile("prefetch.global.L1 [%0];" ::"l"(a + 2048 - (gi & 31) * 8));
+    }
+}
+
 template <int MU, int NU>
 __device__ __forceinline__ void fetch_BC(Mat3<float>& B, Mat3<float>& C, const SiteCtx& c, int li, const unsigned long long (&sl)[4],
                                          const Links<float>& u, const Geo& g) {
@@ -201,51 +218,68 @@ __device__ __forceinline__ void fetch_BC(Mat3<float>& B, Mat3<float>& C, const S
     C = fetch_mat(sl[MU], u.u[MU], c.ip<NU>(), li + c.dp<NU>(), c.gp<NU>(g));
 }
 
-template <int MU, int NU, int MU2, int NU2>
+template <int MU, int NU, int MU2, int NU2, bool PF, bool FENCE>
 __device__ __forceinline__ void plane(Mat3<float> (&S)[4], Mat3<float>& B, Mat3<float>& C, const SiteCtx& c, int li,
                                       const unsigned long long (&sl)[4], const Links<float>& u, const Geo& g) {
+    constexpr int M2 = MU2 >= 0 ? MU2 : 0, N2 = NU2 >= 0 ? NU2 : 1;
+    // PF: the halo operands are requested into L1 three products ahead of their loads, in three groups spread over the
+    // plane (all at the plane's start measured slower: 2.99 against 2.84 ms).  With the requests under way the
+    // scheduling fences below only cost (2.88 -> 2.84 ms without them), so the PF form leaves the order to ptxas.
+    if (PF) {  // the first lower staple's E, F, G
+        pf_mat(u.u[NU], c.im<NU>(), c.gm<NU>(g));
+        pf_mat(u.u[MU], c.im<NU>(), c.gm<NU>(g));
+        pf_mat(u.u[NU], c.im<NU>() && c.ip<MU>(), c.gm<NU>(g) + (c.gp<MU>(g) - c.s));
+    }
     // Software pipeline, one product deep: the operand(s) of the next product are requested, then __syncwarp() --
     // a memory-ordering point ptxas will not sink loads across (left alone it moves every load down to its first
     // use to save registers, and twelve warps per SM cannot cover an L2 round trip per operand) -- then the FMAs of
     // the current product.  Four operand matrices live beside the four staple sums at the widest point.
     const Mat3<float> Amu = fetch_own(sl[MU], li);
-    __syncwarp();
+    if (FENCE) __syncwarp();
     const Mat3<float> Z = mul_na(B, C);
-    fence_mat(Z);
+    if (FENCE) fence_mat(Z);
     const Mat3<float> Anu = fetch_own(sl[NU], li);
-    __syncwarp();
+    if (FENCE) __syncwarp();
+    if (PF) {  // the second lower staple's E', F', G'
+        pf_mat(u.u[MU], c.im<MU>(), c.gm<MU>(g));
+        pf_mat(u.u[NU], c.im<MU>(), c.gm<MU>(g));
+        pf_mat(u.u[MU], c.im<MU>() && c.ip<NU>(), c.gm<MU>(g) + (c.gp<NU>(g) - c.s));
+    }
     mac_nn(S[NU], Amu, Z);
-    fence_mat(S[NU]);
+    if (FENCE) fence_mat(S[NU]);
     const Mat3<float> E = fetch_mat(sl[NU], u.u[NU], c.im<NU>(), li + c.dm<NU>(), c.gm<NU>(g));
     const Mat3<float> F = fetch_mat(sl[MU], u.u[MU], c.im<NU>(), li + c.dm<NU>(), c.gm<NU>(g));
-    __syncwarp();
+    if (FENCE) __syncwarp();
     mac_na(S[MU], Anu, Z);
-    fence_mat(S[MU]);
+    if (FENCE) fence_mat(S[MU]);
     const Mat3<float> G = fetch_mat(sl[NU], u.u[NU], c.im<NU>() && c.ip<MU>(), li + c.dm<NU>() + c.dp<MU>(), c.gm<NU>(g) + (c.gp<MU>(g) - c.s));
-    __syncwarp();
+    if (FENCE) __syncwarp();
+    if (PF && MU2 >= 0) {  // the next plane's B and C
+        pf_mat(u.u[N2], c.ip<M2>(), c.gp<M2>(g));
+        pf_mat(u.u[M2], c.ip<N2>(), c.gp<N2>(g));
+    }
     const Mat3<float> t = mul_an(E, F);
-    fence_mat(t);
+    if (FENCE) fence_mat(t);
     const Mat3<float> E2 = fetch_mat(sl[MU], u.u[MU], c.im<MU>(), li + c.dm<MU>(), c.gm<MU>(g));
     const Mat3<float> F2 = fetch_mat(sl[NU], u.u[NU], c.im<MU>(), li + c.dm<MU>(), c.gm<MU>(g));
-    __syncwarp();
+    if (FENCE) __syncwarp();
     mac_nn(S[MU], t, G);
-    fence_mat(S[MU]);
+    if (FENCE) fence_mat(S[MU]);
     const Mat3<float> G2 = fetch_mat(sl[MU], u.u[MU], c.im<MU>() && c.ip<NU>(), li + c.dm<MU>() + c.dp<NU>(), c.gm<MU>(g) + (c.gp<NU>(g) - c.s));
-    __syncwarp();
+    if (FENCE) __syncwarp();
     const Mat3<float> t2 = mul_an(E2, F2);
-    fence_mat(t2);
-    constexpr int M2 = MU2 >= 0 ? MU2 : 0, N2 = NU2 >= 0 ? NU2 : 1;
+    if (FENCE) fence_mat(t2);
     if (MU2 >= 0) {
         B = fetch_mat(sl[N2], u.u[N2], c.ip<M2>(), li + c.dp<M2>(), c.gp<M2>(g));
         C = fetch_mat(sl[M2], u.u[M2], c.ip<N2>(), li + c.dp<N2>(), c.gp<N2>(g));
-        __syncwarp();
+        if (FENCE) __syncwarp();
     }
     mac_nn(S[NU], t2, G2);
-    fence_mat(S[NU]);
+    if (FENCE) fence_mat(S[NU]);
 }
 
-template <bool PLAQ, int RY, int RZ, int RT, int MAXT>
-__global__ void __launch_bounds__(MAXT, 1) k_smear_rows(const __grid_constant__ Geo g, const __grid_constant__ RowMap rm,
+template <bool PLAQ, int RY, int RZ, int RT, int MAXT, int MINB, bool PF>
+__global__ void __launch_bounds__(MAXT, MINB) k_smear_rows(const __grid_constant__ Geo g, const __grid_constant__ RowMap rm,
                                                         const __grid_constant__ Links<float> u, const __grid_constant__ LinksOut<float> out,
                                                         float c0, float c1, double* __restrict__ partials) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -313,26 +347,30 @@ __global__ void __launch_bounds__(MAXT, 1) k_smear_rows(const __grid_constant__ 
         Mat3<float> S[4];
 #pragma unroll
         for (int mu = 0; mu < 4; ++mu) S[mu] = zero_mat<float>();
+        constexpr bool FENCE = !PF || PLAQ;
         Mat3<float> B, C;
         fetch_BC<0, 1>(B, C, c, li, sl, u, g);
-        plane<0, 1, 0, 2>(S, B, C, c, li, sl, u, g);
-        plane<0, 2, 0, 3>(S, B, C, c, li, sl, u, g);
-        plane<0, 3, 1, 2>(S, B, C, c, li, sl, u, g);
-        plane<1, 2, 1, 3>(S, B, C, c, li, sl, u, g);
-        plane<1, 3, 2, 3>(S, B, C, c, li, sl, u, g);
-        plane<2, 3, -1, -1>(S, B, C, c, li, sl, u, g);
+        plane<0, 1, 0, 2, PF, FENCE>(S, B, C, c, li, sl, u, g);
+        plane<0, 2, 0, 3, PF, FENCE>(S, B, C, c, li, sl, u, g);
+        plane<0, 3, 1, 2, PF, FENCE>(S, B, C, c, li, sl, u, g);
+        plane<1, 2, 1, 3, PF, FENCE>(S, B, C, c, li, sl, u, g);
+        plane<1, 3, 2, 3, PF, FENCE>(S, B, C, c, li, sl, u, g);
+        plane<2, 3, -1, -1, PF, FENCE>(S, B, C, c, li, sl, u, g);
 #pragma unroll
         for (int mu = 0; mu < 4; ++mu) {
             const Mat3<float> umu = fetch_own(sl[mu], li);
-            if (PLAQ) pl += re_tr_na(umu, S[mu]);
             Mat3<float> r;
+            float tr = 0.f;
 #pragma unroll
             for (int i = 0; i < 3; ++i)
 #pragma unroll
-                for (int j = 0; j < 3; ++j) {
+                for (int j = 0; j < 3; ++j) {  // trace and update element by element: r takes S's registers
+                    if (PLAQ) tr = fmaf(umu.re[i][j], S[mu].re[i][j], tr);
+                    if (PLAQ) tr = fmaf(umu.im[i][j], S[mu].im[i][j], tr);
                     r.re[i][j] = fmaf(c1, S[mu].re[i][j], c0 * umu.re[i][j]);
                     r.im[i][j] = fmaf(c1, S[mu].im[i][j], c0 * umu.im[i][j]);
                 }
+            if (PLAQ) pl += tr;
             store_mat(out.u[mu], c.s, r);
         }
     }
@@ -554,7 +592,7 @@ int rowlit_launch(lqx_ctx* ctx, const Links<T>& in, const LinksOut<T>& out, T c0
     return plaq ? lqx_sum_partials(ctx, grid, 1, plaq) : LQX_OK;
 }
 
-template <int RY, int RZ, int RT, int MAXT>
+template <int RY, int RZ, int RT, int MAXT, int MINB = 1, bool PF = false>
 int rows_launch(lqx_ctx* ctx, const Links<float>& in, const LinksOut<float>& out, float c0, float c1, double* plaq) {
     const Geo& g = ctx->geo;
     const int nthr = g.L[0] * RY * RZ * RT;
@@ -570,19 +608,21 @@ int rows_launch(lqx_ctx* ctx, const Links<float>& in, const LinksOut<float>& out
     for (int z = 1; z <= rm.nz; ++z)
         if (rm.nz % z == 0 && z * RZ <= target) rm.zs = z;
     const int npad = (nthr + 31) & ~31;
-    const size_t smem = 2 * (size_t)4 * 18 * npad * sizeof(float);
+    // MINB = 1: persistent CTAs, one per SM, two tile buffers (the next tile's links arrive during this tile's products).
+    // MINB > 1: one tile per CTA and one buffer, MINB CTAs per SM; what is left of the SM's 256 KB stays L1 for the halo.
+    const size_t smem = (MINB == 1 ? 2 : 1) * (size_t)4 * 18 * npad * sizeof(float);
     if (smem > 227 * 1024) return 1;
-    const int grid = std::min(rm.ntiles, ctx->num_sms);
-    if (plaq) LQX_CUDA(ctx, cudaFuncSetAttribute(k_smear_rows<true, RY, RZ, RT, MAXT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    else LQX_CUDA(ctx, cudaFuncSetAttribute(k_smear_rows<false, RY, RZ, RT, MAXT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const int grid = MINB == 1 ? std::min(rm.ntiles, ctx->num_sms) : rm.ntiles;
+    if (plaq) LQX_CUDA(ctx, cudaFuncSetAttribute(k_smear_rows<true, RY, RZ, RT, MAXT, MINB, PF>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    else LQX_CUDA(ctx, cudaFuncSetAttribute(k_smear_rows<false, RY, RZ, RT, MAXT, MINB, PF>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     if (plaq) {
         int rc = lqx_ensure_partials(ctx, (size_t)grid);
         if (rc) return rc;
     }
     {
         LqxTimed timed(ctx, LQX_K_SMEAR);
-        if (plaq) k_smear_rows<true, RY, RZ, RT, MAXT><<<grid, nthr, smem, ctx->stream>>>(g, rm, in, out, c0, c1, ctx->d_partials);
-        else k_smear_rows<false, RY, RZ, RT, MAXT><<<grid, nthr, smem, ctx->stream>>>(g, rm, in, out, c0, c1, nullptr);
+        if (plaq) k_smear_rows<true, RY, RZ, RT, MAXT, MINB, PF><<<grid, nthr, smem, ctx->stream>>>(g, rm, in, out, c0, c1, ctx->d_partials);
+        else k_smear_rows<false, RY, RZ, RT, MAXT, MINB, PF><<<grid, nthr, smem, ctx->stream>>>(g, rm, in, out, c0, c1, nullptr);
     }
     LQX_LAUNCH_CHECK(ctx);
     return plaq ? lqx_sum_partials(ctx, grid, 1, plaq) : LQX_OK;
@@ -591,7 +631,8 @@ int rows_launch(lqx_ctx* ctx, const Links<float>& in, const LinksOut<float>& out
 }  // namespace
 
 // LQX_OK, a negative status, or 1 if the lattice does not fit this kernel.  Option "tile" picks the rows of a tile:
-// 1 = 2x3x1 (y, z, t; 6 rows), 2 = 3x2x1, 3 = 2x2x2 (8 rows), 4 = 2x1x3, 5 = 1x2x3; automatic = the first that fits
+// 1 = 2x3x1 (y, z, t; 6 rows), 2 = 3x2x1, 3 = 2x2x2 (8 rows), 4 = 2x1x3, 5 = 1x2x3; automatic = the first that fits;
+// 6 = 2x2x1 rows, one tile per CTA, two CTAs per SM; 7 = 6 with the halo operands prefetched into L1
 int lqx_smear_rows_launch(lqx_ctx* ctx, const Links<float>& in, const LinksOut<float>& out, float c0, float c1, double* plaq) {
     const int t = ctx->opt_tile;
     int rc = 1;
@@ -604,6 +645,10 @@ int lqx_smear_rows_launch(lqx_ctx* ctx, const Links<float>& in, const LinksOut<f
     if (t == 4) rc = rows_launch<2, 1, 3, 288>(ctx, in, out, c0, c1, plaq);
     if (rc != 1) return rc;
     if (t == 5) rc = rows_launch<1, 2, 3, 288>(ctx, in, out, c0, c1, plaq);
+    if (rc != 1) return rc;
+    if (t == 6) rc = rows_launch<2, 2, 1, 192, 2, false>(ctx, in, out, c0, c1, plaq);  // two CTAs per SM, L1 left for the halo
+    if (rc != 1) return rc;
+    if (t == 7) rc = rows_launch<2, 2, 1, 192, 2, true>(ctx, in, out, c0, c1, plaq);   // ... with L1 prefetch of the halo operands
     return rc;
 }
 
