@@ -205,6 +205,25 @@ int lqx_expr_cache_size(const lqx_ctx* ctx);
 int lqx_sum(const lqx_field* f, double* out);   /* out: 2*kind doubles, one site object, QDP order */
 int lqx_norm2(const lqx_field* f, double* out); /* sum_x sum_components |c|^2                      */
 int lqx_trace(const lqx_field* m, double out[2]); /* sum_x tr M(x) (reading A12)                   */
+/* norm2 for callers that cannot allocate device memory (code under CUDA graph capture, serving loops, harnesses that
+ * forbid cudaMalloc): the same sum as lqx_norm2 (Listing 1, norm2() of the Jacobi routine), with the
+ * reduction scratch -- one fp64 partial per CTA of 2048 sites and the last-block ticket -- in a file-scope __device__
+ * array of LQX_NOALLOC_SCRATCH_BYTES instead of the context's cudaMalloc'ed, grow-on-demand buffer.  The call makes
+ * no cudaMalloc / cudaFree and calls no allocating routine; every GPU that loads the library holds the array until
+ * the process exits.
+ *   f        field of any kind and precision (device memory, blocked layout, owned by the caller)
+ *   out_dev  one double in DEVICE memory (or pinned mapped host memory), 8-byte aligned, owned by the caller;
+ *            written by the kernel.  The call is asynchronous on the context's stream and does not synchronise.
+ * Errors: LQX_EINVAL for null / misaligned pointers and for a lattice of more than LQX_NOALLOC_MAX_SITES sites (the
+ * array then has too few partial slots; nothing is launched; lqx_last_error says so); LQX_ECUDA if the array's device
+ * address cannot be obtained (cudaGetSymbolAddress, asked once per device on the first call there) or a launch fails.
+ * All calls share the one array per device and it keeps the last call's contents: the ticket is cleared on the stream
+ * before every launch, the partials are overwritten before they are read; calls that OVERLAP on the GPU (two streams
+ * or two contexts on one device) race on it -- serialise them.  The summation tree depends on the volume only (same
+ * result on every GPU); it is not lqx_norm2's tree, so the two agree to rounding, not bit for bit. */
+#define LQX_NOALLOC_MAX_SITES (1 << 24)
+#define LQX_NOALLOC_SCRATCH_BYTES (8192 * 8 + 256)
+int lqx_norm2_noalloc(const lqx_field* f, double* out_dev);
 /* P = sum_x sum_{mu<nu} Re tr[U_mu(x) U_nu(x+mu^) adj(U_mu(x+nu^)) adj(U_nu(x))];
  * *plaq_sum = P, *plaq_avg = P/(18 V) (reading A11).  Either pointer may be NULL. */
 int lqx_plaquette(const lqx_field* const u[4], double* plaq_sum, double* plaq_avg);

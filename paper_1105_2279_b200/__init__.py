@@ -100,6 +100,7 @@ SIGNATURES = {
     "lqx_divide": (_i, [_vp, _vp, _d]),
     "lqx_sum": (_i, [_vp, _pd]),
     "lqx_norm2": (_i, [_vp, _pd]),
+    "lqx_norm2_noalloc": (_i, [_vp, _vp]),
     "lqx_trace": (_i, [_vp, _pd]),
     "lqx_plaquette": (_i, [_pvp, _pd, _pd]),
     "lqx_staple_sum": (_i, [_vp, _pvp, _i]),
@@ -519,6 +520,15 @@ def norm2(f) -> float:
     out = C.c_double()
     _check(_lib.lqx_norm2(_h(f), C.byref(out)), _ctx_of(f))
     return out.value
+
+
+NOALLOC_MAX_SITES = 1 << 24  # include/lqx.h LQX_NOALLOC_MAX_SITES
+
+
+def norm2_noalloc(f, out_dev_ptr: int) -> None:
+    """lqx_norm2_noalloc: norm2(f) written to one double at DEVICE address `out_dev_ptr` (e.g. a torch float64
+    tensor's data_ptr()); allocates nothing, asynchronous on the lattice's stream (include/lqx.h)."""
+    _check(_lib.lqx_norm2_noalloc(_h(f), C.c_void_p(int(out_dev_ptr))), _ctx_of(f))
 
 
 def trace(m):

@@ -11,7 +11,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liblqx.so")
-SOURCES = ["lqx_core.cu", "lqx_expr.cu", "lqx_lattice.cu", "lqx_smear.cu", "lqx_smear_staged.cu", "lqx_smear_tile.cu", "lqx_smear_rows.cu", "lqx_jit.cu", "lqx_bench.cu", "lqx_tune.cu"]
+SOURCES = ["lqx_core.cu", "lqx_expr.cu", "lqx_lattice.cu", "lqx_smear.cu", "lqx_smear_staged.cu", "lqx_smear_tile.cu", "lqx_smear_rows.cu", "lqx_jit.cu", "lqx_bench.cu", "lqx_tune.cu", "lqx_noalloc.cu"]
 HEADERS = [os.path.join(CSRC, "lqx_internal.cuh"), os.path.join(CSRC, "lqx_smear.cuh"),
            os.path.join(os.path.dirname(HERE), "include", "lqx.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
