@@ -204,21 +204,112 @@ __global__ void __launch_bounds__(256) k_norm2(int V, const T* __restrict__ f, d
     }
     block_reduce_finish<1>(acc, partials, ticket, out);
 }
-// sum over sites of the site object -> NREAL doubles in QDP order
-template <typename T, int NREAL>
-__global__ void __launch_bounds__(256) k_sum(int V, const T* __restrict__ f, double* __restrict__ partials, unsigned int* ticket,
-                                             double* __restrict__ out) {
-    double acc[NREAL];
+// sum over sites of the site object -> NREAL doubles in QDP order.
+// A warp OWNS one 128-bit chunk position q of the site object (the blocked layout keeps chunk q of 32 consecutive
+// sites contiguous) and walks over the 32-site blocks: a thread then accumulates only the W = 4 (fp32) or 2 (fp64)
+// reals of its chunk -- 4 fp64 accumulators instead of the 2*kind of a thread-per-site loop (36 registers for a
+// colour matrix, which halved the occupancy: 38 us against 31 us for norm2 on the same 151 MB) -- and has UNR
+// independent 128-bit loads in flight.  SUB warps share a chunk position inside a CTA and are combined through
+// shared memory in a fixed order, so one CTA still produces one partial per component.  The pad lanes of the last
+// block are zero by the layout's invariant, so whole blocks are summed.
+template <typename T, int NREAL, int SUB>
+__global__ void __launch_bounds__(32 * SUB * ((NREAL + Vec128<T>::W - 1) / Vec128<T>::W), 64 / (SUB * ((NREAL + Vec128<T>::W - 1) / Vec128<T>::W)))
+    k_sum(int nblk, const T* __restrict__ f, double* __restrict__ partials, unsigned int* ticket, double* __restrict__ out) {
+    typedef typename Vec128<T>::type V128;
+    constexpr int W = Vec128<T>::W, NFULL = NREAL / W, NQ = (NREAL + W - 1) / W, UNR = 4;
+    __shared__ double sh[SUB][NQ * W];
+    __shared__ bool last;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int q = warp % NQ, sub = warp / NQ;
+    const int nblocks = gridDim.x;
+    double acc[W];
 #pragma unroll
-    for (int c = 0; c < NREAL; ++c) acc[c] = 0.0;
-    const int step = gridDim.x * blockDim.x;
-    for (int s = blockIdx.x * blockDim.x + threadIdx.x; s < V; s += step) {
-        T r[NREAL];
-        load_site<T, NREAL>(f, s, r);
+    for (int r = 0; r < W; ++r) acc[r] = 0.0;
+    const int stride = nblocks * SUB;
+    int b = blockIdx.x * SUB + sub;
+    if (q < NFULL) {  // a full chunk: 128 bits per site
+        static_assert((32 * NREAL * sizeof(T)) % sizeof(V128) == 0, "block pitch");
+        constexpr size_t BLK = (size_t)32 * NREAL * sizeof(T) / sizeof(V128);  // block pitch in 128-bit units
+        const V128* p = reinterpret_cast<const V128*>(f + (size_t)q * 32 * W) + lane;
+        for (; b + (UNR - 1) * stride < nblk; b += UNR * stride) {
+            V128 v[UNR];
 #pragma unroll
-        for (int c = 0; c < NREAL; ++c) acc[c] += (double)r[c];
+            for (int k = 0; k < UNR; ++k) v[k] = __ldg(p + (size_t)(b + k * stride) * BLK);
+#pragma unroll
+            for (int k = 0; k < UNR; ++k) {
+                T r[W];
+                unpack(v[k], r);
+#pragma unroll
+                for (int j = 0; j < W; ++j) acc[j] += (double)r[j];
+            }
+        }
+        for (; b < nblk; b += stride) {
+            T r[W];
+            unpack(__ldg(p + (size_t)b * BLK), r);
+#pragma unroll
+            for (int j = 0; j < W; ++j) acc[j] += (double)r[j];
+        }
+    } else {  // fp32 only: the trailing (re, im) pair, 64 bits per site
+        constexpr size_t BLK = (size_t)32 * NREAL * sizeof(T) / sizeof(float2);
+        const float2* p = reinterpret_cast<const float2*>(f + (size_t)NFULL * 32 * W) + lane;
+        for (; b + (UNR - 1) * stride < nblk; b += UNR * stride) {
+            float2 v[UNR];
+#pragma unroll
+            for (int k = 0; k < UNR; ++k) v[k] = __ldg(p + (size_t)(b + k * stride) * BLK);
+#pragma unroll
+            for (int k = 0; k < UNR; ++k) {
+                acc[0] += (double)v[k].x;
+                acc[1] += (double)v[k].y;
+            }
+        }
+        for (; b < nblk; b += stride) {
+            const float2 v = __ldg(p + (size_t)b * BLK);
+            acc[0] += (double)v.x;
+            acc[1] += (double)v.y;
+        }
     }
-    block_reduce_finish<NREAL>(acc, partials, ticket, out);
+#pragma unroll
+    for (int r = 0; r < W; ++r) {
+        double t = acc[r];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+        if (lane == 0) sh[sub][q * W + r] = t;
+    }
+    __syncthreads();
+    static_assert(NREAL <= 32, "one warp stores the CTA's partials");
+    if (warp == 0) {
+        if (lane < NREAL) {
+            double t = sh[0][lane];
+#pragma unroll
+            for (int k = 1; k < SUB; ++k) t += sh[k][lane];
+            partials[(size_t)lane * nblocks + blockIdx.x] = t;
+        }
+        __syncwarp();
+        if (lane == 0) {  // release-only ticket, as in block_reduce_finish
+            unsigned int t;
+            asm volatile("atom.release.gpu.global.add.u32 %0, [%1], 1;" : "=r"(t) : "l"(ticket) : "memory");
+            last = (t == (unsigned)(nblocks - 1));
+        }
+    }
+    __syncthreads();
+    if (!last) return;
+    __threadfence();  // acquire side, paid by the one finishing CTA
+    for (int c = warp; c < NREAL; c += (int)(blockDim.x >> 5)) {  // one warp per component, fixed order
+        const double* pc = partials + (size_t)c * nblocks;
+        double t0 = 0.0, t1 = 0.0, t2 = 0.0, t3 = 0.0;
+        int i = lane;
+        for (; i + 96 < nblocks; i += 128) {
+            const double a0 = __ldcg(pc + i), a1 = __ldcg(pc + i + 32), a2 = __ldcg(pc + i + 64), a3 = __ldcg(pc + i + 96);
+            t0 += a0, t1 += a1, t2 += a2, t3 += a3;
+        }
+        for (; i < nblocks; i += 32) t0 += __ldcg(pc + i);
+        double t = (t0 + t1) + (t2 + t3);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+        if (lane == 0) out[c] = t;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) *ticket = 0u;  // ready for the next launch on this stream
 }
 // sum_x tr M(x): diagonal elements (0,0),(1,1),(2,2) = QDP reals 0,1 / 8,9 / 16,17
 template <typename T>
@@ -403,25 +494,48 @@ extern "C" int lqx_norm2(const lqx_field* f, double* out) {
     return lqx_fetch_result(ctx, 1, out);
 }
 
+namespace {
+// one wave of CTAs: a fixed function of the lattice and the SM count only (deterministic summation tree)
+template <typename T, int NREAL, int SUB>
+int sum_launch(lqx_ctx* ctx, const lqx_field* f) {
+    constexpr int W = Vec128<T>::W, NQ = (NREAL + W - 1) / W, WARPS = NQ * SUB;
+    const int nblk = ctx->geo.Vpad / 32;
+    const int per_sm = std::max(1, std::min(32, 64 / WARPS));
+    const int grid = (int)std::max<long>(1, std::min<long>((nblk + SUB - 1) / SUB, (long)ctx->num_sms * per_sm));
+    int rc = lqx_ensure_partials(ctx, (size_t)grid * NREAL);
+    if (rc) return rc;
+    {
+        LqxTimed timed(ctx, LQX_K_REDUCE);
+        k_sum<T, NREAL, SUB><<<grid, 32 * WARPS, 0, ctx->stream>>>(nblk, (const T*)f->data, ctx->d_partials, ctx->d_ticket, ctx->h_result);
+    }
+    LQX_LAUNCH_CHECK(ctx);
+    return LQX_OK;
+}
+}  // namespace
+
 extern "C" int lqx_sum(const lqx_field* f, double* out) {
     if (!f || !out) return LQX_EINVAL;
     lqx_ctx* ctx = f->ctx;
     LQX_CUDA(ctx, cudaSetDevice(ctx->device));
     const int nc = 2 * (int)f->kind;
-    // the site-object sum keeps 2*kind fp64 accumulators per thread: fewer resident CTAs than the scalar reductions
-    const int grid = reduce_grid(ctx, 2, nc <= 6 ? 8 : (f->prec == LQX_F32 ? 4 : 3));
-    int rc = lqx_ensure_partials(ctx, (size_t)grid * nc);
-    if (rc) return rc;
-    const int V = ctx->geo.V;
-    {
-        LqxTimed timed(ctx, LQX_K_REDUCE);
-        if (f->prec == LQX_F32) {
-            LQX_BY_KIND(k_sum, float, f->kind, V, (const float*)f->data, ctx->d_partials, ctx->d_ticket, ctx->h_result)
-        } else {
-            LQX_BY_KIND(k_sum, double, f->kind, V, (const double*)f->data, ctx->d_partials, ctx->d_ticket, ctx->h_result)
+    int rc;
+    // SUB warps per chunk position, so that a CTA has 16-24 warps whatever the site object
+    if (f->prec == LQX_F32) {
+        switch ((int)f->kind) {
+            case LQX_COMPLEX: rc = sum_launch<float, 2, 16>(ctx, f); break;
+            case LQX_COLORVEC: rc = sum_launch<float, 6, 8>(ctx, f); break;
+            case LQX_COLORMAT: rc = sum_launch<float, 18, 4>(ctx, f); break;
+            default: rc = sum_launch<float, 24, 3>(ctx, f); break;
+        }
+    } else {
+        switch ((int)f->kind) {
+            case LQX_COMPLEX: rc = sum_launch<double, 2, 16>(ctx, f); break;
+            case LQX_COLORVEC: rc = sum_launch<double, 6, 6>(ctx, f); break;
+            case LQX_COLORMAT: rc = sum_launch<double, 18, 2>(ctx, f); break;
+            default: rc = sum_launch<double, 24, 2>(ctx, f); break;
         }
     }
-    LQX_LAUNCH_CHECK(ctx);
+    if (rc) return rc;
     return lqx_fetch_result(ctx, nc, out);
 }
 
