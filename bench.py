@@ -646,6 +646,9 @@ def run_ours(args):
         lat.set_option("smear_variant", args.smear_variant)
     if args.tile >= 0:
         lat.set_option("tile", args.tile)
+    for kv in args.opt:  # any other library option, e.g. --opt bulk_fill=1 (reproducible captures of optional code paths)
+        k, v = kv.split("=")
+        lat.set_option(k, int(v))
     if args.block:
         lat.set_option("block", args.block)
     tune_tables = None
@@ -850,6 +853,7 @@ def main():
                          "'kernels'): the command ncu wraps for the catalogue / hop / Jacobi kernels")
     ap.add_argument("--smear-variant", type=int, default=0, help="lqx option smear_variant (0 = library default / tuned)")
     ap.add_argument("--tile", type=int, default=-1, help="lqx option tile (-1 = automatic)")
+    ap.add_argument("--opt", action="append", default=[], metavar="KEY=INT", help="any other lqx_set_option, repeatable")
     ap.add_argument("--block", type=int, default=0, help="lqx option block (slab thickness of the row-tile kernels)")
     ap.add_argument("--only", default="smear", choices=["smear", "plaquette", "hop"],
                     help="with --kernel-only: the kernel to run (the command ncu wraps for that kernel)")

@@ -96,6 +96,7 @@ extern "C" int lqx_init(const int dims[4], int device, void* cuda_stream, lqx_ct
     }
     c->last_smear_variant = 0, c->last_smear_lane_ops = 0, c->last_smear_kernel = "";
     c->opt_tile = -1;
+    c->opt_bulk_fill = 0;
     c->opt_jacobi_block = c->opt_jacobi_sites = 0;
     c->timing = false;
     cudaDeviceProp prop;
@@ -196,6 +197,7 @@ extern "C" int lqx_set_option(lqx_ctx* ctx, const char* key, int value) {
     else if (!strcmp(key, "block")) ctx->opt_block = value;
     else if (!strcmp(key, "hop_block")) ctx->opt_hop_block = value;
     else if (!strcmp(key, "tile")) ctx->opt_tile = value;
+    else if (!strcmp(key, "bulk_fill")) ctx->opt_bulk_fill = value;
     else if (!strcmp(key, "jacobi_block")) ctx->opt_jacobi_block = value;
     else if (!strcmp(key, "jacobi_sites")) ctx->opt_jacobi_sites = value;
     else if (!strcmp(key, "time_kernels")) ctx->timing = value != 0;

@@ -56,6 +56,7 @@ struct lqx_ctx {
     int opt_hop_block;                    // CTA size of the hop kernel on linear blocks: 0 = default (128), 32, 64, 128, 256
     int opt_jacobi_block, opt_jacobi_sites;  // launch geometry of the Jacobi step (0 = default 128 x 1)
     int opt_tile;  // -1 = automatic, 0 = Linear, 1..3 = TileA..TileC (lqx_smear.cuh)
+    int opt_bulk_fill;  // row-tile smear kernel: 1 = fill the tile by TMA bulk copies where its rows are whole blocks (measured slower), 0 = cp.async
     // launch geometries kept by lqx_autotune (lqx_tune.cu), per precision (0 = fp32, 1 = fp64); 0 / -1 = not tuned.
     // An explicit option always wins over a tuned value, a tuned value over the built-in default.
     int tuned_smear_variant[2], tuned_smear_tile[2];

@@ -382,6 +382,33 @@ def test_smear_variants_and_tiles(lqx, dims, prec, variant):
                     assert np.array_equal(got[mu], first[mu]), (variant, tile, mu)
 
 
+# option "bulk_fill": the row-tile kernel's tile filled by TMA bulk copies (cp.async.bulk + mbarrier) instead of per-thread
+# cp.async, on lattices whose tile rows are whole 32-site blocks (16 and 32 sites per row; several tiles in z and t) --
+# same bytes in shared memory, so the output must be bit-identical, and it must agree with the oracle
+@pytest.mark.parametrize("dims", [(16, 8, 4, 4), (32, 4, 4, 6)])
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+def test_smear_row_tile_bulk_fill(lqx, dims, prec):
+    tv = orc.truth_variant(prec)
+    u = _links(6, dims, prec)
+    want = orc.smear_step(dims, u, 0.5, tv)
+    with lqx.Lattice(dims) as lat:
+        fu = [lat.from_host(t) for t in u]
+        out = [lat.alloc(lqx.COLORMAT, fu[0].prec) for _ in range(4)]
+        lat.set_option("smear_variant", 9)
+        got = {}
+        for bulk in (0, 1):
+            lat.set_option("bulk_fill", bulk)
+            for o in out:
+                lqx.scale(o, 0.0, o)
+            p = lqx.smear_step(out, fu, 0.5, want_plaq_in=True)
+            assert lat.smear_info()[2].startswith("k_smear_rowlit")
+            got[bulk] = ([o.pop() for o in out], p)
+        for mu in range(4):
+            assert site_rel_err(got[1][0][mu], want[mu]) < TOL[prec], mu
+            assert np.array_equal(got[1][0][mu], got[0][0][mu]), mu
+        assert got[1][1] == got[0][1]
+
+
 @pytest.mark.parametrize("prec", ["f32", "f64"])
 def test_unit_gauge_is_a_fixed_point(lqx, prec):
     dims = DIMS_EVEN
