@@ -526,8 +526,24 @@ def run_sweep(args):
 
 
 def _kernel_only_other(args, torch, lqx, li, lat, u):
-    """--kernel-only --only plaquette|hop: a few launches of that kernel on the workload's lattice (what ncu wraps)."""
+    """--kernel-only --only plaquette|hop|reduce: a few launches of that kernel on the workload's lattice (what ncu wraps)."""
     P = u[0].prec
+    if args.only == "reduce":
+        # the three standalone reductions on one link field of the workload's lattice, kernel time from the library's own
+        # event pairs (--workload c3: the 32^3x64 fp64 colour matrix of the configs[4] rows)
+        lat.set_option("time_kernels", 1)
+        rows = {}
+        for name, call in (("norm2", lqx.norm2), ("sum", lqx.sum), ("trace", lqx.trace)):
+            for _ in range(3):
+                call(u[0])
+            lat.kernel_time(lqx.K_REDUCE)
+            for _ in range(max(args.steps, 3)):
+                call(u[1]), call(u[2]), call(u[3]), call(u[0])  # four fields in turn
+            ms, n = lat.kernel_time(lqx.K_REDUCE)
+            rows[name] = ms / n
+        print(json.dumps({"kernel_only": "reduce", "workload": args.workload, "kernel_ms": rows}))
+        lat.close()
+        return
     if args.only == "plaquette":
         fn = lambda: lqx.plaquette(u)
     else:
@@ -855,7 +871,7 @@ def main():
     ap.add_argument("--tile", type=int, default=-1, help="lqx option tile (-1 = automatic)")
     ap.add_argument("--opt", action="append", default=[], metavar="KEY=INT", help="any other lqx_set_option, repeatable")
     ap.add_argument("--block", type=int, default=0, help="lqx option block (slab thickness of the row-tile kernels)")
-    ap.add_argument("--only", default="smear", choices=["smear", "plaquette", "hop"],
+    ap.add_argument("--only", default="smear", choices=["smear", "plaquette", "hop", "reduce"],
                     help="with --kernel-only: the kernel to run (the command ncu wraps for that kernel)")
     ap.add_argument("--tsplit", action="store_true",
                     help="NEXT-4 extra mode: one global lattice decomposed along t over the ranks (halo exchange), not replicas")

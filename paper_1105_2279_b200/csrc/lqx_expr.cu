@@ -187,7 +187,7 @@ __global__ void __launch_bounds__(128) k_mat_vec(int V, const T* __restrict__ m,
 // (lqx_internal.cuh) writes the result straight into pinned host memory.
 // ---------------------------------------------------------------------------------------------
 template <typename T, int NREAL>
-__global__ void __launch_bounds__(256) k_norm2(int V, const T* __restrict__ f, double* __restrict__ partials, unsigned int* ticket,
+__global__ void __launch_bounds__(256, 8) k_norm2(int V, const T* __restrict__ f, double* __restrict__ partials, unsigned int* ticket,
                                                double* __restrict__ out) {
     double acc[1] = {0.0};
     const int step = gridDim.x * blockDim.x;
