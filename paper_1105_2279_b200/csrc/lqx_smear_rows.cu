@@ -183,6 +183,27 @@ __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
         asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }" : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
 }
 
+// the updated link, stored with the streaming (evict-first) policy: it is not read again in this launch
+template <typename T>
+__device__ __forceinline__ void store_mat_cs(T* p, int s, const Mat3<T>& m) {
+    typedef typename Vec128<T>::type V;
+    constexpr int W = Vec128<T>::W, NFULL = 18 / W;
+    T r[18];
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            r[2 * (3 * i + j)] = m.re[i][j];
+            r[2 * (3 * i + j) + 1] = m.im[i][j];
+        }
+    T* blk = p + (size_t)(s >> 5) * (32 * 18);
+    const int lane = s & 31;
+    V* q = reinterpret_cast<V*>(blk) + lane;
+#pragma unroll
+    for (int c = 0; c < NFULL; ++c) __stcs(q + c * 32, pack(&r[c * W]));
+    if (18 % W != 0) __stcs(reinterpret_cast<float2*>(blk + NFULL * 32 * W) + lane, make_float2((float)r[NFULL * W], (float)r[NFULL * W + 1]));
+}
+
 // scheduling fence: every element of m must exist before any later (volatile) load is issued.  Without it the
 // compiler hoists the independent operand loads of all six planes to the top and spills kilobytes per thread.
 __device__ __forceinline__ void fence_mat(const Mat3<float>& m) {
@@ -598,7 +619,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_smear_rowlit(const __grid_consta
                 r.re[i][j] = fma(c1, acc.re[i][j], c0 * umu.re[i][j]);
                 r.im[i][j] = fma(c1, acc.im[i][j], c0 * umu.im[i][j]);
             }
-        store_mat(out.u[mu], s, r);
+        store_mat_cs(out.u[mu], s, r);
     }
     if (PLAQ) {
         double p[1] = {0.25 * (double)pl};
