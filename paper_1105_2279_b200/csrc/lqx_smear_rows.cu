@@ -91,8 +91,11 @@ __device__ __forceinline__ Mat3<float> fetch_own(unsigned long long s_link_gener
     return m;
 }
 
-// the four links of site s -> shared buffer slot li, asynchronously (4 x 16 B + 8 B per link)
+// the four links of site s -> shared buffer slot li, asynchronously (4 x 16 B + 8 B per link); the lines are marked
+// evict-last in L2 (the neighbouring tiles read them again as their halo): 2.836 -> 2.830 ms, 2.805 -> 2.798 on four-row tiles
 __device__ __forceinline__ void fill_async(float* buf, int link_floats, const Links<float>& u, int s, int li) {
+    unsigned long long pol;
+    asm("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
     const size_t goff = (size_t)(s >> 5) * (32 * 18) + (size_t)(s & 31) * 4;
     const int soff = (li >> 5) * (32 * 18) + (li & 31) * 4;
 #pragma unroll
@@ -100,8 +103,9 @@ __device__ __forceinline__ void fill_async(float* buf, int link_floats, const Li
         const float* g = u.u[mu] + goff;
         float* d = buf + mu * link_floats + soff;
 #pragma unroll
-        for (int q = 0; q < 4; ++q) __pipeline_memcpy_async(d + q * 128, g + q * 128, 16);
-        __pipeline_memcpy_async(d + 512 - (li & 31) * 2, g + 512 - (s & 31) * 2, 8);
+        for (int q = 0; q < 4; ++q)
+            asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2;" ::"r"((unsigned)__cvta_generic_to_shared(d + q * 128)), "l"(g + q * 128), "l"(pol) : "memory");
+        asm volatile("cp.async.ca.shared.global.L2::cache_hint [%0], [%1], 8, %2;" ::"r"((unsigned)__cvta_generic_to_shared(d + 512 - (li & 31) * 2)), "l"(g + 512 - (s & 31) * 2), "l"(pol) : "memory");
     }
 }
 
