@@ -318,7 +318,7 @@ typedef struct {
 } lqx_tune_row;
 int lqx_autotune(lqx_ctx* ctx, int kernel_class, lqx_prec prec, int reps, lqx_tune_row* rows, int max_rows, int* nrows);
 int lqx_tuned(const lqx_ctx* ctx, int kernel_class, lqx_prec prec, int out[4]);
-/* Options: "smear_variant" 0 = default (fp32: 9, fp64: 3), 3 = rolled literal kernel, 1 = first-cut literal kernel,
+/* Options: "smear_variant" 0 = default (9; 3 where its row tiles do not fit the lattice), 3 = rolled literal kernel, 1 = first-cut literal kernel,
  * 2 = shared-corner kernel (36 products, lower staples exchanged through shared memory), 4 = four
  * threads per site, 6 = operands staged in shared memory with cp.async (fp32), 7 = the CTA tile's own links in
  * shared memory and the halo through L1, 8 = plane-ordered 42-product evaluation on whole-x-row tiles, persistent

@@ -159,7 +159,7 @@ __global__ void __launch_bounds__(MAP::THREADS, MINB) k_smear_rolled(const __gri
             }
             const Mat3<T> umu = load_mat(umu_p, s);
             if (PLAQ) pl += re_tr_na(umu, acc);
-            store_mat(out.u[mu], s, smear_update(c0, c1, umu, acc));
+            store_mat_cs(out.u[mu], s, smear_update(c0, c1, umu, acc));
         }
         p[0] = 0.25 * (double)pl;
     }
@@ -444,7 +444,7 @@ int smear_launch_t(lqx_ctx* ctx, lqx_field* const uout[4], const lqx_field* cons
         int t;
         ~Restore() { c->opt_tile = t; }
     } restore = {ctx, tile_saved};
-    if (variant == 0 && sizeof(T) == 4) variant = 9;  // fp32 default: literal evaluation on row tiles (falls back to 3)
+    if (variant == 0) variant = 9;  // default in both precisions: literal evaluation on row tiles (falls back to 3 where they do not fit)
     // executed FMA lane-ops per site: 48 (variant 8: 42; variant 2: 36 + halo) products x 108 + update 4 x 36
     ctx->last_smear_lane_ops = 48 * 108 + 144;
     if (variant != 1 && variant != 2 && variant != 4 && variant != 6 && variant != 7 && variant != 8 && variant != 9) variant = 3;

@@ -117,7 +117,7 @@ __device__ __forceinline__ Mat3<double> fetch_mat(unsigned long long s_link, con
     const unsigned long long a = (in ? s_link : (unsigned long long)g_link) + off;
     double r[18];
 #pragma unroll
-    for (int q = 0; q < 9; ++q) asm volatile("ld.v2.f64 {%0,%1}, [%2];" : "=d"(r[2 * q]), "=d"(r[2 * q + 1]) : "l"(a + q * 512u));
+    for (int q = 0; q < 9; ++q) asm volatile("ld.cg.v2.f64 {%0,%1}, [%2];" : "=d"(r[2 * q]), "=d"(r[2 * q + 1]) : "l"(a + q * 512u));
     Mat3<double> m;
 #pragma unroll
     for (int i = 0; i < 3; ++i)
@@ -144,6 +144,8 @@ __device__ __forceinline__ Mat3<double> fetch_own_d(unsigned long long s_link_ge
     return m;
 }
 __device__ __forceinline__ void fill_async(double* buf, int link_reals, const Links<double>& u, int s, int li) {
+    unsigned long long pol;
+    asm("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
     const size_t goff = (size_t)(s >> 5) * (32 * 18) + (size_t)(s & 31) * 2;
     const int soff = (li >> 5) * (32 * 18) + (li & 31) * 2;
 #pragma unroll
@@ -151,7 +153,8 @@ __device__ __forceinline__ void fill_async(double* buf, int link_reals, const Li
         const double* g = u.u[mu] + goff;
         double* d = buf + mu * link_reals + soff;
 #pragma unroll
-        for (int q = 0; q < 9; ++q) __pipeline_memcpy_async(d + q * 64, g + q * 64, 16);
+        for (int q = 0; q < 9; ++q)
+            asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2;" ::"r"((unsigned)__cvta_generic_to_shared(d + q * 64)), "l"(g + q * 64), "l"(pol) : "memory");
     }
 }
 template <typename T>
@@ -185,27 +188,6 @@ __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
     unsigned ok = 0;
     while (!ok)
         asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }" : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
-}
-
-// the updated link, stored with the streaming (evict-first) policy: it is not read again in this launch
-template <typename T>
-__device__ __forceinline__ void store_mat_cs(T* p, int s, const Mat3<T>& m) {
-    typedef typename Vec128<T>::type V;
-    constexpr int W = Vec128<T>::W, NFULL = 18 / W;
-    T r[18];
-#pragma unroll
-    for (int i = 0; i < 3; ++i)
-#pragma unroll
-        for (int j = 0; j < 3; ++j) {
-            r[2 * (3 * i + j)] = m.re[i][j];
-            r[2 * (3 * i + j) + 1] = m.im[i][j];
-        }
-    T* blk = p + (size_t)(s >> 5) * (32 * 18);
-    const int lane = s & 31;
-    V* q = reinterpret_cast<V*>(blk) + lane;
-#pragma unroll
-    for (int c = 0; c < NFULL; ++c) __stcs(q + c * 32, pack(&r[c * W]));
-    if (18 % W != 0) __stcs(reinterpret_cast<float2*>(blk + NFULL * 32 * W) + lane, make_float2((float)r[NFULL * W], (float)r[NFULL * W + 1]));
 }
 
 // scheduling fence: every element of m must exist before any later (volatile) load is issued.  Without it the
