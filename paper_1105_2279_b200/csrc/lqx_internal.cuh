@@ -272,7 +272,8 @@ __device__ __forceinline__ void load_site_pinned(const T* __restrict__ base, int
         r[NFULL * W + 1] = (T)t.y;
     }
 }
-template <typename T, int NREAL>
+// STREAM: st.global.cs (evict-first) for results that no later part of the same pass reads
+template <typename T, int NREAL, bool STREAM = false>
 __device__ __forceinline__ void store_site(T* base, int s, const T (&r)[NREAL]) {
     typedef typename Vec128<T>::type V;
     constexpr int W = Vec128<T>::W, NFULL = NREAL / W;
@@ -280,9 +281,14 @@ __device__ __forceinline__ void store_site(T* base, int s, const T (&r)[NREAL]) 
     const int lane = s & 31;
     V* p = reinterpret_cast<V*>(blk) + lane;
 #pragma unroll
-    for (int q = 0; q < NFULL; ++q) p[q * 32] = pack(&r[q * W]);
+    for (int q = 0; q < NFULL; ++q) {
+        if (STREAM) __stcs(p + q * 32, pack(&r[q * W]));
+        else p[q * 32] = pack(&r[q * W]);
+    }
     if (NREAL % W != 0) {
-        reinterpret_cast<float2*>(blk + NFULL * 32 * W)[lane] = make_float2((float)r[NFULL * W], (float)r[NFULL * W + 1]);
+        const float2 h = make_float2((float)r[NFULL * W], (float)r[NFULL * W + 1]);
+        if (STREAM) __stcs(reinterpret_cast<float2*>(blk + NFULL * 32 * W) + lane, h);
+        else reinterpret_cast<float2*>(blk + NFULL * 32 * W)[lane] = h;
     }
 }
 
@@ -372,7 +378,7 @@ __device__ __forceinline__ void load_vecs(const T* p, int s, Vec3<T> (&v)[NSPIN]
             v[a].im[i] = r[2 * (3 * a + i) + 1];
         }
 }
-template <typename T, int NSPIN>
+template <typename T, int NSPIN, bool STREAM = false>
 __device__ __forceinline__ void store_vecs(T* p, int s, const Vec3<T> (&v)[NSPIN]) {
     T r[6 * NSPIN];
 #pragma unroll
@@ -382,7 +388,7 @@ __device__ __forceinline__ void store_vecs(T* p, int s, const Vec3<T> (&v)[NSPIN
             r[2 * (3 * a + i)] = v[a].re[i];
             r[2 * (3 * a + i) + 1] = v[a].im[i];
         }
-    store_site<T, 6 * NSPIN>(p, s, r);
+    store_site<T, 6 * NSPIN, STREAM>(p, s, r);
 }
 
 // C = A*B        (AB)_ij = sum_k A_ik B_kj

@@ -23,8 +23,6 @@ static inline Links<T> make_links(const lqx_field* const u[4]) {
 // L2 lines it would take are better spent on the input's halo (row-tile kernel fp32: 2.850 -> 2.836 ms at 48^3x96)
 template <typename T>
 __device__ __forceinline__ void store_mat_cs(T* p, int s, const Mat3<T>& m) {
-    typedef typename Vec128<T>::type V;
-    constexpr int W = Vec128<T>::W, NFULL = 18 / W;
     T r[18];
 #pragma unroll
     for (int i = 0; i < 3; ++i)
@@ -33,12 +31,7 @@ __device__ __forceinline__ void store_mat_cs(T* p, int s, const Mat3<T>& m) {
             r[2 * (3 * i + j)] = m.re[i][j];
             r[2 * (3 * i + j) + 1] = m.im[i][j];
         }
-    T* blk = p + (size_t)(s >> 5) * (32 * 18);
-    const int lane = s & 31;
-    V* q = reinterpret_cast<V*>(blk) + lane;
-#pragma unroll
-    for (int c = 0; c < NFULL; ++c) __stcs(q + c * 32, pack(&r[c * W]));
-    if (18 % W != 0) __stcs(reinterpret_cast<float2*>(blk + NFULL * 32 * W) + lane, make_float2((float)r[NFULL * W], (float)r[NFULL * W + 1]));
+    store_site<T, 18, true>(p, s, r);
 }
 
 // tile shapes the nearest-neighbour kernels are instantiated for (choice 1..6; 0 = Linear fallback).
