@@ -318,14 +318,17 @@ typedef struct {
 } lqx_tune_row;
 int lqx_autotune(lqx_ctx* ctx, int kernel_class, lqx_prec prec, int reps, lqx_tune_row* rows, int max_rows, int* nrows);
 int lqx_tuned(const lqx_ctx* ctx, int kernel_class, lqx_prec prec, int out[4]);
-/* Options: "smear_variant" 0 = default (9; 3 where its row tiles do not fit the lattice), 3 = rolled literal kernel, 1 = first-cut literal kernel,
+/* Options: "smear_variant" 0 = default (fp32 on lattices whose rows are 40 or 48 sites: 10; otherwise 9; 3 where the row tiles do
+ * not fit the lattice), 3 = rolled literal kernel, 1 = first-cut literal kernel,
  * 2 = shared-corner kernel (36 products, lower staples exchanged through shared memory), 4 = four
  * threads per site, 6 = operands staged in shared memory with cp.async (fp32), 7 = the CTA tile's own links in
  * shared memory and the halo through L1, 8 = plane-ordered 42-product evaluation on whole-x-row tiles, persistent
  * double-buffered CTAs (fp32; with "tile" 6: one tile per CTA, two CTAs per SM, 7: the same with the halo operands
  * prefetched into L1), 9 = the literal evaluation of 3 on whole-x-row tiles whose own links sit in shared
- * memory (both precisions; same summation order as 3, bit-identical); variants fall back to 3 where their tiles do not fit
- * the lattice.
+ * memory (both precisions; same summation order as 3, bit-identical), 10 = the per-link evaluation of 9 with the common
+ * factor of the two upper staples of a plane kept in tensor memory between the two links (fp32, rows of a multiple of 8 up
+ * to 48 sites: 42 products and 64 operand fetches per site; falls back to 9); variants fall back to 3 where their tiles do
+ * not fit the lattice.
  * "tile" -1 = automatic, 0 = linear 128-site blocks, 1..6 = CTA tile shape (8x4x4x2, 8x4x2x2,
  * 4x4x4x2, 16x4x2x2, 16x2x2x2, 32x2x2x2) of the nearest-neighbour kernels, used if it divides the
  * lattice.  "jacobi_block" (32, 64, 128, 256) and "jacobi_sites" (1, 2, 4): the paper's launch

@@ -500,7 +500,7 @@ extern "C" int lqx_smear_iterate(lqx_field* const u[4], lqx_field* const tmp[4],
 static int host_slab_thickness(const lqx_ctx* ctx, lqx_prec prec) {
     const Geo& g = ctx->geo;
     if (ctx->opt_host_slabs == 0) return 0;
-    if (ctx->opt_smear_variant != 0 && ctx->opt_smear_variant != 3) return 0;  // only the default kernel takes a t-range
+    if (ctx->opt_smear_variant != 0 && ctx->opt_smear_variant != 3 && ctx->opt_smear_variant != 9 && ctx->opt_smear_variant != 10) return 0;  // only the literal kernels take a t-range
     // automatic: at most 48 slabs (the three slabs left after the last upload are the un-overlapped tail: 48 slabs at
     // configs[3] measured 68-71 ms per call, 24: 72-75, 12: 76-78, serial: 119) of at least 4 MB per link, below
     // which the per-slab launches and copies cost more than the overlap gains; option "host_slabs" = n > 0 forces

@@ -439,26 +439,33 @@ int smear_launch_t(lqx_ctx* ctx, lqx_field* const uout[4], const lqx_field* cons
         variant = ctx->tuned_smear_variant[PI];
         if (ctx->opt_tile < 0) ctx->opt_tile = ctx->tuned_smear_tile[PI];
     }
+    if (variant == 0) variant = lqx_smear_default_variant(ctx, sizeof(T) == 4 ? LQX_F32 : LQX_F64);
     struct Restore {
         lqx_ctx* c;
         int t;
         ~Restore() { c->opt_tile = t; }
     } restore = {ctx, tile_saved};
-    if (variant == 0) variant = 9;  // default in both precisions: literal evaluation on row tiles (falls back to 3 where they do not fit)
     // executed FMA lane-ops per site: 48 (variant 8: 42; variant 2: 36 + halo) products x 108 + update 4 x 36
     ctx->last_smear_lane_ops = 48 * 108 + 144;
-    if (variant != 1 && variant != 2 && variant != 4 && variant != 6 && variant != 7 && variant != 8 && variant != 9) variant = 3;
+    if (variant != 1 && variant != 2 && variant != 4 && variant != 6 && variant != 7 && variant != 8 && variant != 9 && variant != 10) variant = 3;
     if (only_mu >= 0) variant = 1;
     ctx->last_smear_variant = variant;
-    ctx->last_smear_kernel = variant == 9 ? "k_smear_rowlit" : variant == 8 ? "k_smear_rows" : variant == 7 ? "k_smear_tile"
+    ctx->last_smear_kernel = variant == 10 ? "k_smear_rowz" : variant == 9 ? "k_smear_rowlit" : variant == 8 ? "k_smear_rows" : variant == 7 ? "k_smear_tile"
                            : variant == 6 ? "k_smear_staged" : variant == 4 ? "k_smear_mu4" : variant == 2 ? "k_smear_shared"
                            : variant == 1 ? "k_smear_gather" : "k_smear_rolled";
-    if (variant == 8) ctx->last_smear_lane_ops = 42 * 108 + 144;
+    if (variant == 8 || variant == 10) ctx->last_smear_lane_ops = 42 * 108 + 144;
     if (variant == 2) ctx->last_smear_lane_ops = 36 * 108 + 144;  // + the halo products of the tile in use
     struct Fallback {  // a variant whose tiles do not fit hands over to the rolled kernel
         lqx_ctx* c;
         void operator()() const { c->last_smear_variant = 3, c->last_smear_kernel = "k_smear_rolled", c->last_smear_lane_ops = 48 * 108 + 144; }
     } fell_back = {ctx};
+    if (variant == 10) {
+        int rc = 1;
+        if (sizeof(T) == 4) rc = lqx_smear_rowz_launch(ctx, reinterpret_cast<const Links<float>&>(in), reinterpret_cast<const LinksOut<float>&>(o), (float)c0, (float)c1, plaq);
+        if (rc <= 0) return rc;
+        variant = 9;  // fp64, or the lattice does not fit the eight-row tiles
+        ctx->last_smear_variant = 9, ctx->last_smear_kernel = "k_smear_rowlit", ctx->last_smear_lane_ops = 48 * 108 + 144;
+    }
     if (variant == 9) {
         const int rc = lqx_smear_rowlit_launch(ctx, in, o, c0, c1, plaq);
         if (rc <= 0) return rc;
@@ -563,11 +570,24 @@ int smear_range_t(lqx_ctx* ctx, lqx_field* const uout[4], const lqx_field* const
 
 }  // namespace
 
+int lqx_smear_default_variant(const lqx_ctx* ctx, lqx_prec prec) {
+    const int pi = prec == LQX_F32 ? 0 : 1;
+    if (ctx->opt_smear_variant) return ctx->opt_smear_variant;
+    if (ctx->tuned_smear_variant[pi]) return ctx->tuned_smear_variant[pi];
+    if (prec == LQX_F32 && lqx_smear_rowz_fits(ctx) && ctx->geo.L[0] * 8 > 256) return 10;
+    return 9;
+}
+
 int lqx_smear_launch_range(lqx_ctx* ctx, lqx_field* const uout[4], const lqx_field* const uin[4], double alpha, int t0,
                            int t1) {
-    // fp32 with the default kernel selection: the row-tile kernel where its 2-slice tiles split at t0 / t1
-    const int v32 = ctx->opt_smear_variant ? ctx->opt_smear_variant : (ctx->tuned_smear_variant[0] ? ctx->tuned_smear_variant[0] : 9);
-    if (uin[0]->prec == LQX_F32 && v32 == 9) {
+    // fp32: the kernel the whole-lattice step would run, on the range
+    const int v32 = lqx_smear_default_variant(ctx, LQX_F32);
+    if (uin[0]->prec == LQX_F32 && v32 == 10 && lqx_smear_rowz_fits(ctx)) {
+        LinksOut<float> o;
+        for (int mu = 0; mu < 4; ++mu) o.u[mu] = (float*)uout[mu]->data;
+        return lqx_smear_rowz_launch_range(ctx, make_links<float>(uin), o, (float)(1.0 - alpha), (float)(alpha / 6.0), t0, t1);
+    }
+    if (uin[0]->prec == LQX_F32 && (v32 == 9 || v32 == 10)) {
         LinksOut<float> o;
         for (int mu = 0; mu < 4; ++mu) o.u[mu] = (float*)uout[mu]->data;
         const int rc9 = lqx_smear_rowlit_launch_range(ctx, make_links<float>(uin), o, (float)(1.0 - alpha), (float)(alpha / 6.0), t0, t1);

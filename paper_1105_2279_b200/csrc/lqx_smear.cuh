@@ -95,4 +95,13 @@ int lqx_smear_rows_launch(lqx_ctx* ctx, const Links<float>& in, const LinksOut<f
 // the literal evaluation on the same row tiles, two CTAs per SM (option "smear_variant" = 9)
 int lqx_smear_rowlit_launch(lqx_ctx* ctx, const Links<float>& in, const LinksOut<float>& out, float c0, float c1, double* plaq);
 int lqx_smear_rowlit_launch(lqx_ctx* ctx, const Links<double>& in, const LinksOut<double>& out, double c0, double c1, double* plaq);
+// variant 10: variant 9's per-link evaluation with the upper staples' common factors kept in tensor memory (fp32)
+int lqx_smear_rowz_launch(lqx_ctx* ctx, const Links<float>& in, const LinksOut<float>& out, float c0, float c1, double* plaq);
+int lqx_smear_rowz_launch_range(lqx_ctx* ctx, const Links<float>& in, const LinksOut<float>& out, float c0, float c1, int t0, int t1);
+bool lqx_smear_rowz_fits(const lqx_ctx* ctx);
+// the variant a smear step of this precision runs when nothing narrower is asked for: the explicit option, else the
+// auto-tuner's choice, else 10 in fp32 where its eight-row tiles are 257-384 threads (full occupancy of registers, shared
+// and tensor memory; elsewhere its TMEM columns cost resident CTAs), else 9.  One rule for the whole-lattice step and for
+// t-ranges, so that a decomposed step is bit-identical to the single launch.
+int lqx_smear_default_variant(const lqx_ctx* ctx, lqx_prec prec);
 int lqx_smear_rowlit_launch_range(lqx_ctx* ctx, const Links<float>& in, const LinksOut<float>& out, float c0, float c1, int t0, int t1);

@@ -618,6 +618,178 @@ __global__ void __launch_bounds__(MAXT, MINB) k_smear_rowlit(const __grid_consta
     }
 }
 
+// --------------------------------------------------------------------------------------------------------------
+// Variant 10: the per-link evaluation of variant 9 with the upper staples' common factor kept in TENSOR MEMORY.
+// For a plane a < b the product Z'_ab = U_a(x+b^) adj(U_b(x+a^)) serves the upper staple of link a, U_b(x) Z'_ab, and of
+// link b, U_a(x) adj(Z'_ab).  Variant 8 uses this with all four staple sums live (168 registers, 12 warps per SM); here the
+// links are still processed one after the other with ONE accumulator (80 registers, 24 warps), and Z'_ab waits in the
+// thread's own TMEM lane from link a to link b: at most four matrices = 72 columns per warp (tcgen05.st / tcgen05.ld as a
+// per-thread scratchpad, no tensor-core instruction).  42 products and 64 operand fetches per site instead of 48 / 76, the
+// six saved operand pairs being neighbour fetches; in exchange 6 x 18 words written to and read from TMEM (256 / 64 B/clk).
+// The nu loop runs ASCENDING here (nu < mu consumes, nu > mu produces, so a slot is free before it is needed again) and the
+// upper staple is associated as U_nu(x) (U_mu(x+nu^) adj(U_nu(x+mu^))): agrees with the other variants to rounding.
+// Eight-row tiles only (three warps per TMEM lane quarter x 72 columns = 216 of the CTA's 256 columns; two CTAs per SM).
+// --------------------------------------------------------------------------------------------------------------
+template <bool PLAQ, int RY, int RZ, int RT, int MAXT, int MINB>
+__global__ void __launch_bounds__(MAXT, MINB) k_smear_rowz(const __grid_constant__ Geo g, const __grid_constant__ RowMap rm,
+                                                        const __grid_constant__ Links<float> u, const __grid_constant__ LinksOut<float> out,
+                                                        float c0, float c1, double* __restrict__ partials) {
+    typedef float T;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int L0 = g.L[0];
+    const int nthr = blockDim.x;
+    const int npad = (nthr + 31) & ~31;
+    const int link_floats = 18 * npad;
+    T* const buf0 = reinterpret_cast<T*>(smem_raw);
+    const int li = threadIdx.x;
+    const int lx = li % L0, row = li / L0;
+    const int ly = row % RY, lz = (row / RY) % RZ, lt = row / (RY * RZ);
+    int x[4];
+    int s;
+    {
+        const int tile = blockIdx.x;
+        const int per_slab = rm.ny * rm.zs * rm.nt;
+        const int k = tile / per_slab;
+        int rem = tile - k * per_slab;
+        const int bt = rem / (rm.ny * rm.zs);
+        rem -= bt * (rm.ny * rm.zs);
+        const int bz = rem / rm.ny + k * rm.zs, by = rem % rm.ny;
+        x[0] = lx, x[1] = RY * by + ly, x[2] = RZ * bz + lz, x[3] = RT * (bt + rm.toff) + lt;
+        s = x[0] + g.L[0] * (x[1] + g.L[1] * (x[2] + g.L[2] * x[3]));
+    }
+    fill_async(buf0, link_floats, u, s, li);
+    __pipeline_commit();
+    unsigned mask = (ly + 1 < RY ? 2u : 0u) | (lz + 1 < RZ ? 4u : 0u) | (lt + 1 < RT ? 8u : 0u) | (ly > 0 ? 32u : 0u) |
+                    (lz > 0 ? 64u : 0u) | (lt > 0 ? 128u : 0u) | 17u;  // x-neighbours are always in the tile
+#pragma unroll
+    for (int d = 0; d < 4; ++d) {
+        if (x[d] + 1 == g.L[d]) mask |= 1u << (8 + d);
+        if (x[d] == 0) mask |= 1u << (12 + d);
+    }
+    const int dpx = (lx + 1 == L0) ? -(L0 - 1) : 1, dmx = (lx == 0) ? (L0 - 1) : -1;
+    auto dloc = [&](int d, bool fwd) {
+        const int r = d == 1 ? L0 : (d == 2 ? RY * L0 : RY * RZ * L0);
+        return d == 0 ? (fwd ? dpx : dmx) : (fwd ? r : -r);
+    };
+    auto gnb = [&](int d, bool fwd) {
+        const int wrap = (g.L[d] - 1) * g.stride_site[d];
+        if (fwd) return ((mask >> (8 + d)) & 1u) ? s - wrap : s + g.stride_site[d];
+        return ((mask >> (12 + d)) & 1u) ? s + wrap : s - g.stride_site[d];
+    };
+    __shared__ unsigned tm_base_s;
+    // columns: 72 per warp of a lane quarter, rounded up to the power of two tcgen05.alloc takes
+    const unsigned tm_need = (unsigned)(((nthr >> 5) + 3) >> 2) * 72u;
+    const unsigned tm_cols = tm_need <= 128u ? 128u : 256u;
+    if ((li >> 5) == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(&tm_base_s)),
+                     "r"(tm_cols));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
+    __pipeline_wait_prior(0);
+    asm volatile("tcgen05.fence::before_thread_sync;");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;");
+    // this thread's scratch: the lane quarter of its warp, 72 columns per warp of a quarter, four slots of 18 columns
+    const unsigned tm_z = tm_base_s + ((unsigned)(((li >> 5) & 3) * 32) << 16) + (unsigned)((li >> 7) * 72);
+    // slot of plane (a, b), a < b, packed two bits per entry at index 4 a + b: (0,1) 0, (0,2) 1, (0,3) 2, (1,2) 0, (1,3) 3, (2,3) 0
+    constexpr unsigned kSlots = (0u << 2) | (1u << 4) | (2u << 6) | (0u << 12) | (3u << 14) | (0u << 22);
+
+    T pl = T(0);
+#pragma unroll 1
+    for (int mu = 0; mu < 4; ++mu) {
+        const T* umu_g = u.u[mu];
+        const unsigned long long umu_t = (unsigned long long)(buf0 + mu * link_floats);
+        const int xpmu = gnb(mu, true);
+        const bool in_pmu = (mask >> mu) & 1u;
+        const int d_pmu = dloc(mu, true);
+        Mat3<T> acc = zero_mat<T>();
+#pragma unroll 1
+        for (int nu = 0; nu < 4; ++nu) {  // upper: U_nu(x) [U_mu(x+nu^) adj(U_nu(x+mu^))]
+            if (nu == mu) continue;
+            const T* unu_g = u.u[nu];
+            const unsigned long long unu_t = (unsigned long long)(buf0 + nu * link_floats);
+            if (nu < mu) {  // the bracket is adj(Z'_{nu mu}), produced when link nu was processed
+                const unsigned slot = (kSlots >> (2 * (4 * nu + mu))) & 3u;
+                Mat3<T> z = tmem_load_mat(tm_z + 18 * slot);
+                const Mat3<T> own = fetch_own(unu_t, li);
+                tmem_wait(z);
+                mac_na(acc, own, z);
+            } else {  // produce Z'_{mu nu} and keep it for link nu
+                const bool in_pnu = (mask >> nu) & 1u;
+                const Mat3<T> second = fetch_mat(umu_t, umu_g, in_pnu, li + dloc(nu, true), gnb(nu, true));
+                const Mat3<T> z = mul_na(second, fetch_mat(unu_t, unu_g, in_pmu, li + d_pmu, xpmu));
+                const unsigned slot = (kSlots >> (2 * (4 * mu + nu))) & 3u;
+                tmem_store_mat(tm_z + 18 * slot, z);
+                mac_nn(acc, fetch_own(unu_t, li), z);
+                asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+            }
+        }
+#pragma unroll 1
+        for (int nu = 0; nu < 4; ++nu) {  // lower: adj(U_nu(x-nu^)) U_mu(x-nu^) U_nu(x-nu^+mu^)
+            if (nu == mu) continue;
+            const T* unu_g = u.u[nu];
+            const unsigned long long unu_t = (unsigned long long)(buf0 + nu * link_floats);
+            const bool in_mnu = (mask >> (4 + nu)) & 1u;
+            const int xmnu = gnb(nu, false);
+            const int l1 = li + dloc(nu, false);
+            const Mat3<T> t = mul_an(fetch_mat(unu_t, unu_g, in_mnu, l1, xmnu), fetch_mat(umu_t, umu_g, in_mnu, l1, xmnu));
+            mac_nn(acc, t, fetch_mat(unu_t, unu_g, in_mnu && in_pmu, l1 + d_pmu, xmnu + (xpmu - s)));
+        }
+        const Mat3<T> umu = fetch_own(umu_t, li);
+        if (PLAQ) pl += re_tr_na(umu, acc);
+        Mat3<T> r;
+#pragma unroll
+        for (int i = 0; i < 3; ++i)
+#pragma unroll
+            for (int j = 0; j < 3; ++j) {
+                r.re[i][j] = fma(c1, acc.re[i][j], c0 * umu.re[i][j]);
+                r.im[i][j] = fma(c1, acc.im[i][j], c0 * umu.im[i][j]);
+            }
+        store_mat_cs(out.u[mu], s, r);
+    }
+    if (PLAQ) {
+        double p[1] = {0.25 * (double)pl};
+        block_reduce_partial<1>(p, partials);
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;");
+    __syncthreads();
+    if ((li >> 5) == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tm_base_s), "r"(tm_cols));
+}
+
+// t0 < 0: the whole lattice; otherwise the time slices [t0, t1) only (both multiples of RT; no plaquette)
+template <int RY, int RZ, int RT, int MAXT, int MINB>
+int rowz_launch(lqx_ctx* ctx, const Links<float>& in, const LinksOut<float>& out, float c0, float c1, double* plaq, int t0 = -1, int t1 = -1) {
+    const Geo& g = ctx->geo;
+    const int nthr = g.L[0] * RY * RZ * RT;
+    // whole warps, and at most three warps per TMEM lane quarter (72 columns each of the CTA's 256)
+    if (nthr > MAXT || nthr % 32 || nthr > 384 || g.L[1] % RY || g.L[2] % RZ || g.L[3] % RT || (size_t)g.Vpad * 72 >= ((size_t)1 << 32)) return 1;
+    if (t0 >= 0 && (t0 % RT || t1 % RT || plaq)) return 1;
+    RowMap rm;
+    rm.ny = g.L[1] / RY, rm.nz = g.L[2] / RZ, rm.nt = t0 >= 0 ? (t1 - t0) / RT : g.L[3] / RT;
+    rm.toff = t0 >= 0 ? t0 / RT : 0;
+    rm.ntiles = rm.ny * rm.nz * rm.nt;
+    int target = ctx->opt_block > 0 ? ctx->opt_block : kSlabZ;
+    rm.zs = 1;
+    for (int z = 1; z <= rm.nz; ++z)
+        if (rm.nz % z == 0 && z * RZ <= target) rm.zs = z;
+    const int npad = (nthr + 31) & ~31;
+    const size_t smem = (size_t)4 * 18 * npad * sizeof(float);
+    const int grid = rm.ntiles;
+    if (plaq) LQX_CUDA(ctx, cudaFuncSetAttribute(k_smear_rowz<true, RY, RZ, RT, MAXT, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    else LQX_CUDA(ctx, cudaFuncSetAttribute(k_smear_rowz<false, RY, RZ, RT, MAXT, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    if (plaq) {
+        int rc = lqx_ensure_partials(ctx, (size_t)grid);
+        if (rc) return rc;
+    }
+    {
+        LqxTimed timed(ctx, LQX_K_SMEAR);
+        if (plaq) k_smear_rowz<true, RY, RZ, RT, MAXT, MINB><<<grid, nthr, smem, ctx->stream>>>(g, rm, in, out, c0, c1, ctx->d_partials);
+        else k_smear_rowz<false, RY, RZ, RT, MAXT, MINB><<<grid, nthr, smem, ctx->stream>>>(g, rm, in, out, c0, c1, nullptr);
+    }
+    LQX_LAUNCH_CHECK(ctx);
+    return plaq ? lqx_sum_partials(ctx, grid, 1, plaq) : LQX_OK;
+}
+
 // t0 < 0: the whole lattice; otherwise the time slices [t0, t1) only (both multiples of RT, else 1; no plaquette)
 template <typename T, int RY, int RZ, int RT, int MAXT, int MINB, bool TM = false, bool BULK = false>
 int rowlit_launch(lqx_ctx* ctx, const Links<T>& in, const LinksOut<T>& out, T c0, T c1, double* plaq,
@@ -762,4 +934,23 @@ int lqx_smear_rowlit_launch(lqx_ctx* ctx, const Links<double>& in, const LinksOu
     if (rc != 1) return rc;
     if (t == 3) rc = rowlit_launch<double, 2, 2, 2, 256, 1>(ctx, in, out, c0, c1, plaq);
     return rc;
+}
+
+// variant 10 (upper-staple factors kept in tensor memory; fp32).  It runs where a row pair is whole warps and a tile at most
+// 384 threads (L0 a multiple of 8, at most 48; L1, L2 even): eight-row tiles, four-row tiles where a t-range or the
+// lattice's t-extent is odd -- every tile shape evaluates the same per-site arithmetic.
+bool lqx_smear_rowz_fits(const lqx_ctx* ctx) {
+    const Geo& g = ctx->geo;
+    return g.L[0] % 8 == 0 && g.L[0] * 8 <= 384 && g.L[1] % 2 == 0 && g.L[2] % 2 == 0;
+}
+// LQX_OK, a negative status, or 1 if the lattice does not fit (the caller falls back to variant 9)
+int lqx_smear_rowz_launch(lqx_ctx* ctx, const Links<float>& in, const LinksOut<float>& out, float c0, float c1, double* plaq) {
+    if (!lqx_smear_rowz_fits(ctx)) return 1;
+    if (ctx->geo.L[3] % 2 == 0) return rowz_launch<2, 2, 2, 384, 2>(ctx, in, out, c0, c1, plaq);
+    return rowz_launch<2, 2, 1, 192, 2>(ctx, in, out, c0, c1, plaq);
+}
+int lqx_smear_rowz_launch_range(lqx_ctx* ctx, const Links<float>& in, const LinksOut<float>& out, float c0, float c1, int t0, int t1) {
+    if (!lqx_smear_rowz_fits(ctx)) return 1;
+    if (t0 % 2 == 0 && t1 % 2 == 0) return rowz_launch<2, 2, 2, 384, 2>(ctx, in, out, c0, c1, nullptr, t0, t1);
+    return rowz_launch<2, 2, 1, 192, 2>(ctx, in, out, c0, c1, nullptr, t0, t1);
 }

@@ -118,7 +118,7 @@ extern "C" int lqx_autotune(lqx_ctx* ctx, int kernel_class, lqx_prec prec, int r
             if (!(o[mu] = sc.get(ctx, LQX_COLORMAT, prec))) return lqx_fail(ctx, LQX_ENOMEM, "autotune: scratch fields");
         // (variant, tile): the literal kernel on row tiles (fp32) and on 4-d tiles / linear blocks.  The other variants
         // are measured slower on every lattice tried and are options, not candidates.
-        static const int cand32[][2] = {{9, 1}, {9, 2}, {3, 1}, {3, 2}, {3, 4}, {3, 5}, {3, 0}};
+        static const int cand32[][2] = {{10, 1}, {9, 1}, {9, 2}, {3, 1}, {3, 2}, {3, 4}, {3, 5}, {3, 0}};
         static const int cand64[][2] = {{3, 0}, {3, 2}, {3, 3}, {3, 5}, {9, 1}};
         const int(*cand)[2] = pi == 0 ? cand32 : cand64;
         const int ncand = pi == 0 ? 7 : 5;

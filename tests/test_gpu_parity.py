@@ -343,14 +343,15 @@ def test_staple_smear_plaquette(lqx, dims, prec):
 # every smear kernel variant (option "smear_variant": 1 literal gather, 2 shared-corner with the lower
 # staples exchanged through shared memory, 3 rolled literal = default, 4 four threads per site, 6 operands
 # staged in shared memory, 7 the tile's own links in shared memory and the halo through L1, 8 plane-ordered 42-product evaluation on
-# whole-x-row tiles in shared memory with persistent double-buffered CTAs) and every
+# whole-x-row tiles in shared memory with persistent double-buffered CTAs, 9 the literal evaluation on row tiles, 10 the same
+# with the upper staples' common factors kept in tensor memory: 42 products) and every
 # CTA tile shape that divides the lattice, against the truth oracle; 16x8x4x4 spans several tiles in every
 # direction for all shapes, 8x4x4x2 is exactly one 8x4x4x2 tile (every neighbour wraps into the same tile); 12x6x4x2 has
 # row tiles of 96 threads and y-tiles of 2 and 3 rows, 6x4x2x4 has rows that are not whole warps (the row-tile kernels
 # hand over to the rolled kernel there)
 @pytest.mark.parametrize("dims", [(16, 8, 4, 4), (8, 4, 4, 2), (4, 4, 4, 4), (12, 6, 4, 2), (6, 4, 2, 4)])
 @pytest.mark.parametrize("prec", ["f32", "f64"])
-@pytest.mark.parametrize("variant", [1, 2, 3, 4, 6, 7, 8, 9])
+@pytest.mark.parametrize("variant", [1, 2, 3, 4, 6, 7, 8, 9, 10])
 def test_smear_variants_and_tiles(lqx, dims, prec, variant):
     tv = orc.truth_variant(prec)
     u = _links(5, dims, prec)
@@ -750,7 +751,7 @@ def test_autotune_keeps_a_geometry_that_agrees_with_the_oracle(lqx, dims, prec):
             assert rows and all(r["ms"] > 0 and r["kernel_class"] == cls and r["prec"] == P for r in rows)
             assert sum(r["chosen"] for r in rows) == nkept
         t = lat.tuned(lqx.K_SMEAR, P)
-        assert t[0] in (3, 9)
+        assert t[0] in (3, 9, 10)
         hb, jb, js = lat.tuned(lqx.K_HOP, P)[:3]
         assert hb in (32, 64, 128, 256) and jb in (32, 64, 128, 256) and js in (1, 2, 4)
         assert lat.tuned(lqx.K_PLAQUETTE, P)[0] in (1, 2)
