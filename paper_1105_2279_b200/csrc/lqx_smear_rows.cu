@@ -703,6 +703,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_smear_rowz(const __grid_constant
         const bool in_pmu = (mask >> mu) & 1u;
         const int d_pmu = dloc(mu, true);
         Mat3<T> acc = zero_mat<T>();
+        asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");  // the factors stored while the earlier links were processed
 #pragma unroll 1
         for (int nu = 0; nu < 4; ++nu) {  // upper: U_nu(x) [U_mu(x+nu^) adj(U_nu(x+mu^))]
             if (nu == mu) continue;
@@ -721,7 +722,6 @@ __global__ void __launch_bounds__(MAXT, MINB) k_smear_rowz(const __grid_constant
                 const unsigned slot = (kSlots >> (2 * (4 * mu + nu))) & 3u;
                 tmem_store_mat(tm_z + 18 * slot, z);
                 mac_nn(acc, fetch_own(unu_t, li), z);
-                asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
             }
         }
 #pragma unroll 1
