@@ -11,6 +11,7 @@
 #include <vector>
 
 #include "lqx_internal.cuh"
+#include "lqx_smear.cuh"
 
 namespace {
 
@@ -121,10 +122,12 @@ extern "C" int lqx_autotune(lqx_ctx* ctx, int kernel_class, lqx_prec prec, int r
         static const int cand32[][2] = {{10, 1}, {9, 1}, {9, 2}, {3, 1}, {3, 2}, {3, 4}, {3, 5}, {3, 0}};
         static const int cand64[][2] = {{3, 0}, {3, 2}, {3, 3}, {3, 5}, {9, 1}};
         const int(*cand)[2] = pi == 0 ? cand32 : cand64;
-        const int ncand = pi == 0 ? 7 : 5;
+        const int ncand = pi == 0 ? (int)(sizeof(cand32) / sizeof(cand32[0])) : (int)(sizeof(cand64) / sizeof(cand64[0]));
         for (int k = 0; k < ncand; ++k) {
             ctx->opt_smear_variant = cand[k][0], ctx->opt_tile = cand[k][1];
-            const double ms = timer.median_ms([&] { return lqx_smear_step(o, u, 0.5, nullptr); }, reps);
+            // timed WITH the fused input plaquette, the form the iterated smearing launches (its per-CTA reduction costs the
+            // kernels differently: without it the fp64 rolled kernel measured 2.5 % ahead of the row-tile kernel, with it 6 % behind)
+            const double ms = timer.median_ms([&] { return lqx_smear_launch(ctx, o, u, 0.5, -1, ctx->h_result); }, reps);
             // a variant that fell back to another kernel on this lattice is not a candidate of its own
             if (ms > 0 && ctx->last_smear_variant == cand[k][0]) add(cand[k][0], cand[k][1], ms);
         }
