@@ -951,6 +951,6 @@ int lqx_smear_rowz_launch(lqx_ctx* ctx, const Links<float>& in, const LinksOut<f
 }
 int lqx_smear_rowz_launch_range(lqx_ctx* ctx, const Links<float>& in, const LinksOut<float>& out, float c0, float c1, int t0, int t1) {
     if (!lqx_smear_rowz_fits(ctx)) return 1;
-    if (t0 % 2 == 0 && t1 % 2 == 0) return rowz_launch<2, 2, 2, 384, 2>(ctx, in, out, c0, c1, nullptr, t0, t1);
+    if (t0 % 2 == 0 && t1 % 2 == 0 && ctx->geo.L[3] % 2 == 0) return rowz_launch<2, 2, 2, 384, 2>(ctx, in, out, c0, c1, nullptr, t0, t1);
     return rowz_launch<2, 2, 1, 192, 2>(ctx, in, out, c0, c1, nullptr, t0, t1);
 }

@@ -410,6 +410,37 @@ def test_smear_row_tile_bulk_fill(lqx, dims, prec):
         assert got[1][1] == got[0][1]
 
 
+# variant 10 (upper-staple factors kept in tensor memory): without the fused plaquette, on eight-row and four-row tiles
+# (odd t-extent), and on ranges of time slices with even and odd boundaries -- every launch shape evaluates the same per-site
+# arithmetic, so the ranges put together equal the whole-lattice step bit for bit; rows of 48, 16 and 8 sites
+@pytest.mark.parametrize("dims", [(48, 4, 4, 6), (16, 4, 6, 5), (8, 4, 4, 4)])
+def test_smear_variant_10_ranges_and_no_plaquette(lqx, dims):
+    prec = "f32"
+    tv = orc.truth_variant(prec)
+    u = _links(7, dims, prec)
+    want = orc.smear_step(dims, u, 0.5, tv)
+    with lqx.Lattice(dims) as lat:
+        fu = [lat.from_host(t) for t in u]
+        out = [lat.alloc(lqx.COLORMAT, fu[0].prec) for _ in range(4)]
+        lat.set_option("smear_variant", 10)
+        lqx.smear_step(out, fu, 0.5, want_plaq_in=False)
+        assert lat.smear_info()[2] == "k_smear_rowz"
+        full = [o.pop() for o in out]
+        for mu in range(4):
+            assert site_rel_err(full[mu], want[mu]) < TOL[prec], mu
+        lqx.smear_step(out, fu, 0.5, want_plaq_in=True)
+        for mu in range(4):
+            assert np.array_equal(out[mu].pop(), full[mu]), mu
+        L3 = dims[3]
+        for cuts in ([0, 2, L3], [0, 1, 3, L3], [0, L3 - 1, L3]):
+            for o in out:
+                lqx.scale(o, 0.0, o)
+            for t0, t1 in zip(cuts[:-1], cuts[1:]):
+                lqx.smear_step_range(out, fu, 0.5, t0, t1)
+            for mu in range(4):
+                assert np.array_equal(out[mu].pop(), full[mu]), (cuts, mu)
+
+
 @pytest.mark.parametrize("prec", ["f32", "f64"])
 def test_unit_gauge_is_a_fixed_point(lqx, prec):
     dims = DIMS_EVEN
