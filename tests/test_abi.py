@@ -98,3 +98,22 @@ def test_bench_looks_up_ncu_captures_by_kernel_and_precision():
     assert c32 is not None and c64 is not None and s32 != s64
     none, why = bench._ncu_capture("k_no_such_kernel", "f32")
     assert none is None and "k_no_such_kernel" in why
+
+
+def test_no_odd_descriptor_registers_in_the_library():
+    """ptxas 12.9 was seen to put the descriptor of a cache-hinted cp.async in an ODD uniform register pair
+    (`LDGSTS ... desc[UR1]`) in one instantiation of the smear kernel; the hardware rejects that as an illegal instruction
+    at run time (DESIGN.md sec.6.1 item 16).  Wide uniform operands must be even-aligned: scan the built library's SASS."""
+    import re
+    import shutil
+    import subprocess
+
+    import paper_1105_2279_b200 as lqx
+
+    cuobjdump = shutil.which("cuobjdump") or "/usr/local/cuda/bin/cuobjdump"
+    if not os.path.exists(cuobjdump):
+        pytest.skip("cuobjdump not available")
+    sass = subprocess.run([cuobjdump, "-sass", lqx.library_path()], capture_output=True, text=True, check=True).stdout
+    regs = {int(m) for m in re.findall(r"desc\[UR(\d+)\]", sass)}
+    assert regs, "no descriptor-based memory instructions found: is this the right library?"
+    assert not [r for r in regs if r % 2], sorted(regs)
