@@ -117,3 +117,5 @@ def test_no_odd_descriptor_registers_in_the_library():
     regs = {int(m) for m in re.findall(r"desc\[UR(\d+)\]", sass)}
     assert regs, "no descriptor-based memory instructions found: is this the right library?"
     assert not [r for r in regs if r % 2], sorted(regs)
+    # the same rule for 64-bit address operands held in register pairs
+    assert not [r for r in set(re.findall(r"\bU?R(\d+)\.64", sass)) if int(r) % 2]
