@@ -321,6 +321,38 @@ def test_staple_brute_force_tiny(dims):
             assert np.abs(s[sidx] - _brute_force_staple(U, dims, x, mu)).max() < 1e-14
 
 
+@pytest.mark.parametrize("dims", [(2, 2, 2, 2), (4, 6, 2, 4), (3, 5, 2, 4)])
+def test_staple_sum_equals_the_42_product_order(dims):
+    """The evaluation order of the GPU kernels k_smear_rows / k_smear_rowz (DESIGN.md sec.6.1 items 5 and 16) against the
+    literal oracle: for a plane a < b the ONE product Z' = U_a(x+b) adj(U_b(x+a)) gives the upper staple of link a,
+    U_b(x) Z', and of link b, U_a(x) adj(Z'); the lower staples stay literal.  42 products per site instead of 48, the
+    same staple sums (to rounding)."""
+    u = links(8, dims)
+    U = [cplx(t) for t in u]
+    sh = lambda f, sign, mu: cplx(orc.shift(dims, real2(f), sign, mu))
+    adj = lambda m: np.conj(np.swapaxes(m, -1, -2))
+    S = [np.zeros_like(U[0]) for _ in range(4)]
+    nprod = 0
+    for a in range(4):
+        for b in range(a + 1, 4):
+            z = sh(U[a], +1, b) @ adj(sh(U[b], +1, a))  # Z'_ab(x)
+            S[a] += U[b] @ z
+            S[b] += U[a] @ adj(z)
+            nprod += 3
+    for mu in range(4):
+        for nu in range(4):
+            if nu == mu:
+                continue
+            # lower staple of link mu in plane nu: adj(U_nu(x-nu)) U_mu(x-nu) U_nu(x-nu+mu)
+            t = adj(sh(U[nu], -1, nu)) @ sh(U[mu], -1, nu)
+            S[mu] += t @ sh(sh(U[nu], -1, nu), +1, mu)
+            nprod += 2
+    assert nprod == 42
+    for mu in range(4):
+        want = cplx(orc.staple_sum(dims, u, mu, "t64"))
+        assert np.abs(S[mu] - want).max() < 1e-13, mu
+
+
 def test_staple_abelian_closed_form():
     """diagonal U(1)^3 links with random phases: every staple is a sum/difference of phases."""
     dims = (4, 6, 2, 4)
